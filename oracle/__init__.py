@@ -1,0 +1,152 @@
+"""ORACLE -- test infrastructure only (see oracle.cpp header).
+
+Thin ctypes/numpy wrapper around `oracle.cpp`.  Only `tests/`, `__graft_entry__.smoke()` and
+`bench.py`'s cpu_baseline / `--impl reference` legs may import this package; nothing under
+`paper_1811_04165_b200/` does, and this package imports nothing from there.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.cpp with g++ (plain -O2, no contraction, single thread)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
+                               _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def delay_table(f_mhz, dm, t_samp_s: float, f_ref_mhz: Optional[float] = None) -> np.ndarray:
+    """int32 [ndm][nchan]; f_ref defaults to max f (DD.3)."""
+    f = np.ascontiguousarray(f_mhz, dtype=np.float64)
+    d = np.ascontiguousarray(dm, dtype=np.float64)
+    if f_ref_mhz is None:
+        f_ref_mhz = float(f.max())
+    out = np.empty((d.size, f.size), dtype=np.int32)
+    rc = _load().oracle_delay_table(_p(f), ctypes.c_int(f.size), ctypes.c_double(f_ref_mhz), _p(d),
+                                    ctypes.c_int(d.size), ctypes.c_double(t_samp_s), _p(out))
+    if rc != 0:
+        raise ValueError("oracle_delay_table rc=%d" % rc)
+    return out
+
+
+def dedisperse(X: np.ndarray, delay: np.ndarray, ns: int) -> np.ndarray:
+    """uint32 [nrows][ns] for the delay rows given (X: uint8 [nchan][in_stride])."""
+    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    nrows, nchan = delay.shape
+    assert nchan == X.shape[0]
+    Y = np.empty((nrows, ns), dtype=np.uint32)
+    rc = _load().oracle_dedisperse(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), _p(delay),
+                                   ctypes.c_int(nrows), ctypes.c_int(ns), _p(Y), ctypes.c_size_t(ns))
+    if rc != 0:
+        raise ValueError("oracle_dedisperse rc=%d (input too short for the delays?)" % rc)
+    return Y
+
+
+def subband_step1(X: np.ndarray, d1: np.ndarray, nsub: int, ns1: int) -> np.ndarray:
+    """uint32 S[ncoarse][nsub][ns1]."""
+    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    d1 = np.ascontiguousarray(d1, dtype=np.int32)
+    ncoarse, nchan = d1.shape
+    S = np.empty((ncoarse, nsub, ns1), dtype=np.uint32)
+    rc = _load().oracle_subband_step1(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]),
+                                      ctypes.c_int(nsub), _p(d1), ctypes.c_int(ncoarse), ctypes.c_int(ns1),
+                                      _p(S), ctypes.c_size_t(ns1))
+    if rc != 0:
+        raise ValueError("oracle_subband_step1 rc=%d" % rc)
+    return S
+
+
+def subband_step2(S: np.ndarray, d2: np.ndarray, ns: int) -> np.ndarray:
+    """uint32 Y[ncoarse*nfine][ns]; row a*nfine+b."""
+    assert S.dtype == np.uint32 and S.ndim == 3 and S.flags.c_contiguous
+    d2 = np.ascontiguousarray(d2, dtype=np.int32)
+    ncoarse, nsub, ns1 = S.shape
+    nfine = d2.shape[0]
+    assert d2.shape[1] == nsub
+    Y = np.empty((ncoarse * nfine, ns), dtype=np.uint32)
+    rc = _load().oracle_subband_step2(_p(S), ctypes.c_int(nsub), ctypes.c_size_t(ns1), ctypes.c_int(ns1),
+                                      _p(d2), ctypes.c_int(nfine), ctypes.c_int(ncoarse), ctypes.c_int(ns),
+                                      _p(Y), ctypes.c_size_t(ns))
+    if rc != 0:
+        raise ValueError("oracle_subband_step2 rc=%d" % rc)
+    return Y
+
+
+def subband_tables(f_mhz, t_samp_s: float, nsub: int, coarse_dm, fine_dm) -> Tuple[np.ndarray, np.ndarray]:
+    """(d1[ncoarse][nchan], d2[nfine][nsub]) for reading SB.1 "B" with SB.2 (subband reference =
+    highest channel frequency of the subband) -- both tables relative to the global f_ref."""
+    f = np.asarray(f_mhz, dtype=np.float64)
+    cps = f.size // nsub
+    assert cps * nsub == f.size
+    f_ref = float(f.max())
+    f_sub = f.reshape(nsub, cps).max(axis=1)
+    d1 = delay_table(f, coarse_dm, t_samp_s, f_ref)
+    d2 = delay_table(f_sub, fine_dm, t_samp_s, f_ref)
+    return d1, d2
+
+
+def integrate(Y: np.ndarray, w: int, ns: Optional[int] = None) -> np.ndarray:
+    """uint32 [nrows][ns // w] block sums of width w (INT.1, INT.2)."""
+    assert Y.dtype == np.uint32 and Y.ndim == 2 and Y.flags.c_contiguous
+    if ns is None:
+        ns = Y.shape[1]
+    nw = ns // w
+    out = np.empty((Y.shape[0], nw), dtype=np.uint32)
+    rc = _load().oracle_integrate(_p(Y), ctypes.c_size_t(Y.shape[1]), ctypes.c_int(Y.shape[0]),
+                                  ctypes.c_int(ns), ctypes.c_int(w), _p(out), ctypes.c_size_t(max(nw, 1)))
+    if rc != 0:
+        raise ValueError("oracle_integrate rc=%d" % rc)
+    return out
+
+
+def snr(V: np.ndarray, ddof: int = 0, n: Optional[int] = None) -> Tuple[np.ndarray, np.ndarray]:
+    """(snr float32 [nrows], argmax uint32 [nrows]) over the first n values of every row."""
+    assert V.dtype == np.uint32 and V.ndim == 2 and V.flags.c_contiguous
+    if n is None:
+        n = V.shape[1]
+    s = np.empty(V.shape[0], dtype=np.float32)
+    a = np.empty(V.shape[0], dtype=np.uint32)
+    rc = _load().oracle_snr(_p(V), ctypes.c_size_t(V.shape[1]), ctypes.c_int(V.shape[0]), ctypes.c_int(n),
+                            ctypes.c_int(ddof), _p(s), _p(a))
+    if rc != 0:
+        raise ValueError("oracle_snr rc=%d" % rc)
+    return s, a
+
+
+def search(Y: np.ndarray, widths: Sequence[int], ddof: int = 0):
+    """integrate + snr for every width: (planes dict w -> I_w, snr [nrows][nW], argmax [nrows][nW])."""
+    planes, S, A = {}, [], []
+    for w in widths:
+        I = Y if w == 1 else integrate(Y, w)
+        planes[w] = I
+        s, a = snr(np.ascontiguousarray(I), ddof)
+        S.append(s)
+        A.append(a)
+    return planes, np.stack(S, axis=1), np.stack(A, axis=1)
