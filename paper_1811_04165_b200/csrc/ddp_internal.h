@@ -1,0 +1,95 @@
+// Internal declarations shared by the host translation units of libddp (not part of the ABI).
+#ifndef DDP_INTERNAL_H_
+#define DDP_INTERNAL_H_
+
+#include <cstdint>
+#include <functional>
+#include <map>
+#include <string>
+#include <unordered_map>
+#include <utility>
+#include <vector>
+
+#include "../../include/ddp.h"
+#include "ddp_params.h"
+
+// Gene candidate arrays (BJ:cfg4; powers of two).
+static const int DDP_CAND_THREADS_T[] = {16, 32, 64, 128, 256, 512, 1024};
+static const int DDP_CAND_THREADS_DM[] = {1, 2, 4, 8, 16, 32};
+static const int DDP_CAND_SPT[] = {1, 2, 4, 8, 16};
+static const int DDP_CAND_DPT[] = {1, 2, 4, 8, 16};
+static const int DDP_CAND_UNROLL[] = {1, 2, 4, 8, 16};
+static const int DDP_CAND_STAGING[] = {0, 1, 2};
+static const int DDP_CAND_VEC[] = {1, 4, 8, 16};
+#define DDP_NGENES 7
+struct DdpGeneDomain { const int* v; int n; };
+const DdpGeneDomain* ddp_gene_domains();        // [DDP_NGENES], struct order of ddp_kcfg
+int* ddp_gene_ptr(ddp_kcfg* c, int gene);
+int ddp_gene_get(const ddp_kcfg& c, int gene);
+int ddp_gene_index(int gene, int value);        // -1 if not a candidate
+
+#define DDP_SMEM_LIMIT 232448                   // 227 KB per CTA on sm_100a
+
+// Geometry of one kernel as the validity rules see it.
+struct DdpKGeom {
+    int ns_k;      // time-axis length the kernel tiles
+    int ndm_k;     // DM-axis length the kernel tiles
+    int nred;      // reduction trip count (0 = no reduction loop rule)
+    int in_bytes;  // bytes per input element (1 or 4)
+};
+
+struct DdpCompiled;  // runtime kernel handle (ddp_rt.cpp)
+
+struct ddp_plan {
+    // problem
+    int nchan = 0, ndm = 0, nwidths = 0, ns = 0;
+    double tsamp = 0;
+    std::vector<double> freq, dms;
+    int widths[DDP_MAX_WIDTHS] = {0};
+    bool subband = false;
+    int nsub = 0, ncoarse = 0, nfine = 0, cps = 0;
+    double coarse_first = 0, coarse_step = 0, fine_step = 0;
+    int ddof = 0, device = 0;
+    std::string cache_dir;
+    // host tables
+    std::vector<int32_t> delay, d1, d2;
+    ddp_plan_info info;
+    // configurations + validity caches
+    ddp_kcfg kcfg[DDP_K_COUNT];
+    mutable std::map<int, int> spread_cache[3];              // dedisp kernel -> (TD -> max window spread)
+    mutable std::vector<ddp_kcfg> valid[DDP_K_COUNT];
+    mutable bool valid_built[DDP_K_COUNT] = {false, false, false, false, false};
+    // device side (ddp_rt.cpp)
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    int32_t *d_delay = nullptr, *d_d1 = nullptr, *d_d2 = nullptr;
+    uint32_t* d_sub = nullptr;
+    DdpCompiled* active[DDP_K_COUNT] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    void* rt = nullptr;  // per-plan runtime state (events), owned by ddp_rt.cpp
+    mutable std::string err;
+};
+
+// ---- ddp_plan.cpp (pure host)
+DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k);
+bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k);
+int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD);           // dedisp kernels only
+int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // staged row window (elements)
+size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
+bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::string* why);
+const std::vector<ddp_kcfg>& ddp_valid_set(const ddp_plan* p, ddp_kernel k);
+bool ddp_kcfg_equal(const ddp_kcfg& a, const ddp_kcfg& b);
+ddp_kernel ddp_slot_kernel(const ddp_plan* p, int slot);               // slot -> kernel, DDP_K_COUNT if unused
+ddp_status ddp_fail(const ddp_plan* p, ddp_status s, const std::string& msg);
+
+// ---- ddp_rt.cpp (CUDA)
+void ddp_rt_release(ddp_plan* p);
+ddp_status ddp_rt_activate(ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // compile/load, make active
+// Hardware fitness of a joint configuration (median of summed CUDA-event times); only the slots in
+// slot_mask are launched (brute force may time one kernel alone on the buffers of an earlier pass).
+ddp_status ddp_rt_time_pipeline_mask(ddp_plan* p, const ddp_tune_io* io, const ddp_kcfg cfg[DDP_NSLOTS], unsigned slot_mask,
+                                     double best_so_far, double* ms, double kernel_ms[DDP_NSLOTS], int64_t* n_timings);
+// NVRTC-compiles (on all host cores) every code shape of the list that is not known yet.
+void ddp_rt_precompile(const ddp_plan* p, const std::vector<std::pair<ddp_kernel, ddp_kcfg>>& list);
+int64_t ddp_rt_compile_count();
+
+#endif  // DDP_INTERNAL_H_

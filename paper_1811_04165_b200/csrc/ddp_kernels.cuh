@@ -1,0 +1,569 @@
+// Device templates of the single-pulse-search kernels, sm_100a.  ONE parameterised template per
+// kernel (BJ:north_star): the same text is compiled ahead of time by nvcc for the default
+// configurations (ddp_aot.cu) and at tune time by NVRTC for every other point of the search grid
+// (ddp_rt.cpp concatenates ddp_params.h + this file + one DDP_DEFINE_* line).  No standard headers.
+//
+// Compile-time axes (the "code shape" genes of ddp_kcfg): SPT samples per thread, DPT DMs per
+// thread, UNROLL reduction-loop unroll = rows per staging chunk, STAGING 0 direct / 1 shared memory
+// / 2 TMA bulk copy + mbarrier, VEC bytes per input load.  threads_t x threads_dm is the launch
+// shape (blockDim.x, blockDim.y); MAXT bounds it for register allocation.
+//
+// What is computed (P:n = PAPER.md line n; readings in DESIGN.md):
+//   dedisp   out[g][i][t] = sum_r in[g][r][t + delay[g][i][r]]            P:51, P:63, P:71 fn.4
+//   integ    I_w[i][j]    = sum_{k<w} Y[i][j*w + k], j < floor(ns/w)
+//   snr      (max - mean)/std per (DM, width), exact integer moments      P:63; BJ:cfg0
+#ifndef DDP_KERNELS_CUH_
+#define DDP_KERNELS_CUH_
+
+typedef unsigned char ddp_u8;
+typedef unsigned int ddp_u32;
+typedef unsigned long long ddp_u64;
+typedef long long ddp_i64;
+
+// ------------------------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ ddp_u32 ddp_dp4a(ddp_u32 a, ddp_u32 b, ddp_u32 c) {
+    ddp_u32 d;
+    asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ ddp_u32 ddp_shf_r(ddp_u32 lo, ddp_u32 hi, ddp_u32 sh) {
+    ddp_u32 d;
+    asm("shf.r.wrap.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(lo), "r"(hi), "r"(sh));
+    return d;
+}
+__device__ __forceinline__ ddp_u32 ddp_smem_addr(const void* p) {
+    return (ddp_u32)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void ddp_mbar_init(void* bar, ddp_u32 count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ddp_smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ddp_mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void ddp_mbar_expect_tx(void* bar, ddp_u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ddp_smem_addr(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void ddp_mbar_wait(void* bar, ddp_u32 parity) {
+    ddp_u32 ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(ddp_smem_addr(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+// TMA 1-D bulk copy global -> shared (SASS UBLKCP); 16-byte aligned src/dst, bytes % 16 == 0.
+__device__ __forceinline__ void ddp_bulk_g2s(void* dst, const void* src, ddp_u32 bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     ddp_smem_addr(dst)),
+                 "l"(src), "r"(bytes), "r"(ddp_smem_addr(bar))
+                 : "memory");
+}
+
+template <int V> struct DdpVec;
+template <> struct DdpVec<4> { typedef ddp_u32 type; };
+template <> struct DdpVec<8> { typedef uint2 type; };
+template <> struct DdpVec<16> { typedef uint4 type; };
+
+// ------------------------------------------------------------------------------------ window loads
+// acc[s] += ptr[s], s < SPT, for an arbitrarily aligned uint8 pointer.
+// VEC == 1: byte loads.  VEC >= 4: aligned VEC-byte loads covering the window, word-select stages
+// for the (VEC/4)-word misalignment, a funnel shift for the byte misalignment, then one
+// dp4a(word, one-hot, acc) per sample (extract + add in a single instruction).
+template <int SPT, int VEC>
+__device__ __forceinline__ void ddp_acc_window(const ddp_u8* ptr, ddp_u32 (&acc)[SPT]) {
+    if constexpr (VEC == 1 || SPT < 4) {
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) acc[s] += (ddp_u32)ptr[s];
+    } else {
+        constexpr int NW = SPT / 4 + VEC / 4;
+        const ddp_u64 a = (ddp_u64)ptr;
+        const ddp_u32 o = (ddp_u32)(a & (ddp_u64)(VEC - 1));
+        typedef typename DdpVec<VEC>::type vec_t;
+        const vec_t* base = (const vec_t*)(a - o);
+        union { vec_t v[NW * 4 / VEC]; ddp_u32 w[NW]; } r;
+#pragma unroll
+        for (int v = 0; v < NW * 4 / VEC; ++v) r.v[v] = base[v];
+        if constexpr (VEC >= 16) {
+            if (o & 8u) {
+#pragma unroll
+                for (int k = 0; k + 2 < NW; ++k) r.w[k] = r.w[k + 2];
+            }
+        }
+        if constexpr (VEC >= 8) {
+            if (o & 4u) {
+#pragma unroll
+                for (int k = 0; k + 1 < NW; ++k) r.w[k] = r.w[k + 1];
+            }
+        }
+        const ddp_u32 sh = (o & 3u) * 8u;
+#pragma unroll
+        for (int k = 0; k < SPT / 4; ++k) {
+            const ddp_u32 w = ddp_shf_r(r.w[k], r.w[k + 1], sh);
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[4 * k + b] = ddp_dp4a(w, 1u << (8 * b), acc[4 * k + b]);
+        }
+    }
+}
+
+// Same for uint32 elements: vector loads when the window happens to be VEC-aligned, else scalar.
+template <int SPT, int VEC>
+__device__ __forceinline__ void ddp_acc_window(const ddp_u32* ptr, ddp_u32 (&acc)[SPT]) {
+    constexpr int VE = VEC / 4;  // elements per vector
+    if constexpr (VE <= 1 || SPT < VE) {
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) acc[s] += ptr[s];
+    } else {
+        if ((((ddp_u64)ptr) & (ddp_u64)(VEC - 1)) == 0) {
+            typedef typename DdpVec<VEC>::type vec_t;
+            union { vec_t v[SPT / VE]; ddp_u32 w[SPT]; } r;
+#pragma unroll
+            for (int v = 0; v < SPT / VE; ++v) r.v[v] = ((const vec_t*)ptr)[v];
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) acc[s] += r.w[s];
+        } else {
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) acc[s] += ptr[s];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ dedispersion
+// Block = blockDim.x (time) x blockDim.y (DM) threads; tile = TT = blockDim.x*SPT samples by
+// TD = blockDim.y*DPT trials; grid = (time tiles, DM tiles, groups).  Thread (tx, ty) owns samples
+// tile_t + tx*SPT .. +SPT-1 of trials tile_dm + ty*DPT .. +DPT-1 in SPT*DPT uint32 registers.
+template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC>
+__device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int AL = 16 / (int)sizeof(IN_T);  // elements per 16 bytes
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int TT = blockDim.x * SPT, TD = blockDim.y * DPT;
+    const int g = blockIdx.z;
+    const int tile_t = blockIdx.x * TT;
+    const int tile_dm = blockIdx.y * TD;
+    const int t0 = tile_t + tx * SPT;
+    const IN_T* in_g = (const IN_T*)p.in + (ddp_i64)g * p.in_group_stride;
+    const int* dl = p.delay + (ddp_i64)g * p.delay_group_off;
+
+    ddp_u32 acc[DPT][SPT];
+    int drow[DPT];  // delay-table row offset of each owned trial (clamped to the last trial)
+#pragma unroll
+    for (int j = 0; j < DPT; ++j) {
+        int dm = tile_dm + ty * DPT + j;
+        dm = dm < p.ndm ? dm : p.ndm - 1;
+        drow[j] = dm * p.delay_dm_stride;
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) acc[j][s] = 0u;
+    }
+
+    if constexpr (STAGING == 0) {
+        // Direct: every thread reads its delayed window straight from global memory (L1/L2 cached).
+        // Fully out-of-range threads are clamped into the row (results discarded); rows carry
+        // SPT + 16 bytes of slack beyond nsamp_in (in_stride_min), so threads with any valid sample
+        // are never clamped.
+        const ddp_i64 lim = p.in_row_len - (SPT + AL);
+        for (int r0 = 0; r0 < p.nred; r0 += UNROLL) {
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) {
+                const int r = r0 + u;
+                const IN_T* row = in_g + (ddp_i64)r * p.in_row_stride;
+#pragma unroll
+                for (int j = 0; j < DPT; ++j) {
+                    ddp_i64 off = (ddp_i64)t0 + dl[drow[j] + r];
+                    off = off < lim ? off : lim;
+                    ddp_acc_window<SPT, VEC>(row + off, acc[j]);
+                }
+            }
+        }
+    } else {
+        // Staged: per chunk of UNROLL reduction rows the block copies, for each row, the union of
+        // the windows its TD trials need -- [tile_t + dmin, tile_t + TT + dmax), delays being
+        // non-decreasing in the trial index -- into shared memory, from the 16-byte aligned-down
+        // start (the residual `carry` is added to the read index).  STAGING 1: cooperative VEC-wide
+        // copy, single buffer.  STAGING 2: TMA bulk copies issued by one thread, completion on an
+        // mbarrier, two buffers so chunk k+1 lands while chunk k is summed.
+        const int i_lo = tile_dm;
+        const int i_hi = (tile_dm + TD < p.ndm ? tile_dm + TD : p.ndm) - 1;
+        const int tid = ty * blockDim.x + tx;
+        const int nthreads = blockDim.x * blockDim.y;
+        const int win = p.win;  // elements per staged row, multiple of AL
+        constexpr int NBUF = STAGING == 2 ? 2 : 1;
+        IN_T* sbuf = (IN_T*)ddp_smem;
+        ddp_u64* mbar = (ddp_u64*)(ddp_smem + (size_t)NBUF * UNROLL * win * sizeof(IN_T));
+        const int nchunks = p.nred / UNROLL;
+
+        if constexpr (STAGING == 2) {
+            if (tid == 0) {
+                ddp_mbar_init(&mbar[0], 1);
+                ddp_mbar_init(&mbar[1], 1);
+                ddp_mbar_fence_init();
+            }
+            __syncthreads();
+        }
+        // Issue the TMA copies of chunk k into buffer k & 1 (one thread).
+        auto tma_issue = [&](int k) {
+            IN_T* dst = sbuf + (size_t)(k & 1) * UNROLL * win;
+            ddp_u32 total = 0;
+            ddp_i64 a0s[UNROLL];
+            int lens[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) {
+                const int r = k * UNROLL + u;
+                const int dmin = dl[i_lo * p.delay_dm_stride + r];
+                const int dmax = dl[i_hi * p.delay_dm_stride + r];
+                const ddp_i64 src = (ddp_i64)tile_t + dmin;
+                const ddp_i64 a0 = src & ~(ddp_i64)(AL - 1);
+                ddp_i64 len = (src - a0) + TT + (dmax - dmin);
+                len = (len + AL - 1) & ~(ddp_i64)(AL - 1);
+                if (a0 + len > p.in_row_len) len = p.in_row_len - a0;
+                if (len > win) len = win;
+                if (len < 0) len = 0;
+                a0s[u] = a0;
+                lens[u] = (int)len;
+                total += (ddp_u32)(len * sizeof(IN_T));
+            }
+            ddp_mbar_expect_tx(&mbar[k & 1], total);
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) {
+                const int r = k * UNROLL + u;
+                if (lens[u] > 0)
+                    ddp_bulk_g2s(dst + (size_t)u * win, in_g + (ddp_i64)r * p.in_row_stride + a0s[u],
+                                 (ddp_u32)(lens[u] * sizeof(IN_T)), &mbar[k & 1]);
+            }
+        };
+        if constexpr (STAGING == 2) {
+            if (tid == 0) tma_issue(0);
+        }
+        for (int k = 0; k < nchunks; ++k) {
+            IN_T* buf = sbuf + (size_t)(STAGING == 2 ? (k & 1) : 0) * UNROLL * win;
+            if constexpr (STAGING == 1) {
+                __syncthreads();  // previous chunk fully consumed
+                typedef typename DdpVec<(VEC >= 4 ? VEC : 4)>::type vec_t;
+                constexpr int VE = (int)(sizeof(vec_t) / sizeof(IN_T));
+#pragma unroll
+                for (int u = 0; u < UNROLL; ++u) {
+                    const int r = k * UNROLL + u;
+                    const int dmin = dl[i_lo * p.delay_dm_stride + r];
+                    const int dmax = dl[i_hi * p.delay_dm_stride + r];
+                    const ddp_i64 src = (ddp_i64)tile_t + dmin;
+                    const ddp_i64 a0 = src & ~(ddp_i64)(AL - 1);
+                    ddp_i64 len = (src - a0) + TT + (dmax - dmin);
+                    len = (len + AL - 1) & ~(ddp_i64)(AL - 1);
+                    if (a0 + len > p.in_row_len) len = p.in_row_len - a0;
+                    if (len > win) len = win;
+                    const vec_t* s = (const vec_t*)(in_g + (ddp_i64)r * p.in_row_stride + a0);
+                    vec_t* d = (vec_t*)(buf + (size_t)u * win);
+                    const int nv = (int)(len / VE);
+                    for (int i = tid; i < nv; i += nthreads) d[i] = s[i];
+                }
+                __syncthreads();
+            } else {
+                if (tid == 0 && k + 1 < nchunks) tma_issue(k + 1);  // buffer (k+1)&1 was released at the end of k-1
+                ddp_mbar_wait(&mbar[k & 1], (ddp_u32)((k >> 1) & 1));
+            }
+#pragma unroll
+            for (int u = 0; u < UNROLL; ++u) {
+                const int r = k * UNROLL + u;
+                const int dmin = dl[i_lo * p.delay_dm_stride + r];
+                const int carry = (int)(((ddp_i64)tile_t + dmin) & (ddp_i64)(AL - 1));
+                const IN_T* row = buf + (size_t)u * win + carry + tx * SPT - dmin;
+#pragma unroll
+                for (int j = 0; j < DPT; ++j) ddp_acc_window<SPT, VEC>(row + dl[drow[j] + r], acc[j]);
+            }
+            if constexpr (STAGING == 2) __syncthreads();  // release buffer k&1 for chunk k+2
+        }
+    }
+
+    // Epilogue: uint32 sums, vector stores where the whole group of samples is in range.
+#pragma unroll
+    for (int j = 0; j < DPT; ++j) {
+        const int dm = tile_dm + ty * DPT + j;
+        if (dm >= p.ndm) continue;
+        ddp_u32* o = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride + t0;
+        if (SPT >= 4 && t0 + SPT <= p.ns) {
+#pragma unroll
+            for (int s = 0; s + 3 < SPT; s += 4)
+                *(uint4*)(o + s) = make_uint4(acc[j][s], acc[j][s + 1], acc[j][s + 2], acc[j][s + 3]);
+        } else {
+#pragma unroll
+            for (int s = 0; s < SPT; ++s)
+                if (t0 + s < p.ns) o[s] = acc[j][s];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ integration
+// Tile = TT = blockDim.x*SPT consecutive samples of one row; every width divides TT (host rule).
+// Per row: SPT samples per thread (vector loads), thread-local running sums, warp inclusive scan of
+// the thread totals with shuffles, cross-warp offsets through shared memory, the tile's exclusive
+// prefix P[0..TT] written to (bank-padded) shared memory, then I_w[j] = P[(j+1)w] - P[jw] for every
+// width with coalesced stores.  Exact in uint32 because the true sums are < 2^32 (plan check).
+__device__ __forceinline__ int ddp_pad(int i) { return i + (i >> 5); }
+
+template <int SPT, int DPT, int UNROLL, int STAGING, int VEC>
+__device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int VE = (VEC >= 4 ? VEC : 4) / 4;  // elements per load
+    constexpr int LV = VE < SPT ? VE : SPT;       // elements per load actually usable
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int TT = blockDim.x * SPT;
+    const int lane = tx & 31, wx = tx >> 5;
+    const int nwx = (blockDim.x + 31) >> 5;
+    const int prow = ddp_pad(TT) + 2;  // padded prefix row length
+    ddp_u32* P = (ddp_u32*)ddp_smem + (size_t)ty * prow;
+    ddp_u32* wtot = (ddp_u32*)ddp_smem + (size_t)blockDim.y * prow + ty * 32;
+    // raw staging area (STAGING 1/2): one tile per ty
+    ddp_u32* raw = (ddp_u32*)ddp_smem + (size_t)blockDim.y * (prow + 32) + (size_t)ty * TT;
+    ddp_u64* mbar = (ddp_u64*)((ddp_u32*)ddp_smem + (size_t)blockDim.y * (prow + 32 + TT));
+    const int ns4 = (p.ns + 3) & ~3;  // rows are readable up to here (out_stride is a multiple of 4)
+    ddp_u32 tma_phase = 0;
+    if constexpr (STAGING == 2) {
+        if (tx == 0 && ty == 0) {
+            ddp_mbar_init(mbar, blockDim.y);
+            ddp_mbar_fence_init();
+        }
+        __syncthreads();
+    }
+
+    for (int it = 0; it < p.tiles_per_block; ++it) {
+        const int tile_t = (blockIdx.x * p.tiles_per_block + it) * TT;
+        if (tile_t >= p.ns) break;  // uniform over the block
+#pragma unroll 1
+        for (int j = 0; j < DPT; ++j) {
+            const int dm = blockIdx.y * (blockDim.y * DPT) + ty * DPT + j;
+            const bool live = dm < p.ndm;
+            const ddp_u32* row = p.in + (ddp_i64)(live ? dm : 0) * p.in_stride;
+            const int t0 = tile_t + tx * SPT;
+            ddp_u32 x[SPT];
+            if constexpr (STAGING == 0) {
+#pragma unroll
+                for (int v = 0; v < SPT / LV; ++v) {
+                    const int t = t0 + v * LV;
+                    if (LV > 1 && t + LV <= ns4) {
+                        typedef typename DdpVec<LV * 4>::type vec_t;
+                        union { vec_t v; ddp_u32 w[LV]; } r;
+                        r.v = *(const vec_t*)(row + t);
+#pragma unroll
+                        for (int e = 0; e < LV; ++e) x[v * LV + e] = r.w[e];
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < LV; ++e) x[v * LV + e] = (t + e < p.ns) ? row[t + e] : 0u;
+                    }
+                }
+            } else {
+                // copy the raw tile (clipped to the readable row) to shared memory, then read it back
+                int len = ns4 - tile_t;
+                len = len < TT ? len : TT;
+                if constexpr (STAGING == 1) {
+                    for (int i = tx * 4; i < len; i += blockDim.x * 4) *(uint4*)(raw + i) = *(const uint4*)(row + tile_t + i);
+                    __syncthreads();
+                } else {
+                    if (tx == 0) {
+                        ddp_mbar_expect_tx(mbar, (ddp_u32)(len * 4));
+                        ddp_bulk_g2s(raw, row + tile_t, (ddp_u32)(len * 4), mbar);
+                    }
+                    ddp_mbar_wait(mbar, tma_phase);
+                    tma_phase ^= 1u;
+                }
+#pragma unroll
+                for (int s = 0; s < SPT; ++s) x[s] = (tx * SPT + s < len) ? raw[tx * SPT + s] : 0u;
+            }
+#pragma unroll
+            for (int s = 0; s < SPT; ++s)
+                if (t0 + s >= p.ns) x[s] = 0u;
+            // thread-local inclusive running sums
+#pragma unroll
+            for (int s = 1; s < SPT; ++s) x[s] += x[s - 1];
+            // warp inclusive scan of the thread totals
+            ddp_u32 incl = x[SPT - 1];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const ddp_u32 n = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += n;
+            }
+            if (lane == 31 || tx == (int)blockDim.x - 1) wtot[wx] = incl;
+            __syncthreads();
+            ddp_u32 base = incl - x[SPT - 1];  // exclusive within the warp
+            for (int w = 0; w < wx; ++w) base += wtot[w];
+            if (tx == 0) P[0] = 0u;
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) P[ddp_pad(tx * SPT + s + 1)] = base + x[s];
+            __syncthreads();
+            if (live) {
+                for (int k = 0; k < p.nplanes; ++k) {
+                    const int w = p.width[k];
+                    const int nout = TT / w;
+                    const int j0 = tile_t / w;
+                    ddp_u32* o = p.out + p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + j0;
+                    const int nvalid = p.plane_len[k] - j0;
+                    for (int jj = tx; jj < nout && jj < nvalid; jj += blockDim.x)
+                        o[jj] = P[ddp_pad((jj + 1) * w)] - P[ddp_pad(jj * w)];
+                }
+            }
+            __syncthreads();
+        }
+    }
+    (void)nwx;
+}
+
+// ------------------------------------------------------------------------------------ S/N
+// One block owns TD = blockDim.y*DPT whole series of one width (blockIdx.z); it walks them in chunks
+// of blockDim.x*SPT values.  Per thread: exact uint64 sum and sum of squares, max and its lowest
+// index.  Warp-shuffle tree, cross-warp through shared memory, then
+//   snr = ((n*max - S1)/n) / sqrt((n*S2 - S1^2) / (n*(n - ddof)))  with n*S2 - S1^2 exact in 128 bits,
+// finished in float64 and rounded once to float32 -- independent of block shape and reduction order.
+struct DdpMoments {
+    ddp_u64 s1, s2;
+    ddp_u32 mx, ix;
+};
+__device__ __forceinline__ void ddp_mom_add(DdpMoments& m, ddp_u32 v, ddp_u32 idx) {
+    m.s1 += v;
+    m.s2 += (ddp_u64)v * (ddp_u64)v;
+    if (v > m.mx) { m.mx = v; m.ix = idx; }  // indices visited in increasing order per thread
+}
+__device__ __forceinline__ void ddp_mom_merge(DdpMoments& m, ddp_u64 s1, ddp_u64 s2, ddp_u32 mx, ddp_u32 ix) {
+    m.s1 += s1;
+    m.s2 += s2;
+    if (mx > m.mx || (mx == m.mx && ix < m.ix)) { m.mx = mx; m.ix = ix; }
+}
+
+template <int SPT, int DPT, int UNROLL, int STAGING, int VEC>
+__device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int VE = (VEC >= 4 ? VEC : 4) / 4;
+    constexpr int LV = VE < SPT ? VE : SPT;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int k = blockIdx.z;
+    const int n = p.n[k];
+    const int n4 = (n + 3) & ~3;
+    const int CH = blockDim.x * SPT;  // values per chunk
+    const int lane = tx & 31, wx = tx >> 5;
+    const int nwx = (blockDim.x + 31) >> 5;
+    // shared: reduction scratch [blockDim.y][32] moments, then staging tiles
+    DdpMoments* red = (DdpMoments*)ddp_smem + (size_t)ty * 32;
+    constexpr int NBUF = STAGING == 2 ? 2 : 1;
+    ddp_u32* raw = (ddp_u32*)(ddp_smem + (size_t)blockDim.y * 32 * sizeof(DdpMoments)) + (size_t)ty * NBUF * CH;
+    ddp_u64* mbar = (ddp_u64*)(ddp_smem + (size_t)blockDim.y * 32 * sizeof(DdpMoments) +
+                               (size_t)blockDim.y * NBUF * CH * 4) + ty * 2;
+    if constexpr (STAGING == 2) {
+        if (tx == 0) {
+            ddp_mbar_init(&mbar[0], 1);
+            ddp_mbar_init(&mbar[1], 1);
+            ddp_mbar_fence_init();
+        }
+        __syncthreads();
+    }
+    ddp_u32 nwait = 0;  // chunks consumed so far by this ty row (TMA phase tracking)
+
+#pragma unroll 1
+    for (int j = 0; j < DPT; ++j) {
+        const int dm = blockIdx.y * (blockDim.y * DPT) + ty * DPT + j;
+        const bool live = dm < p.ndm;
+        const ddp_u32* row = p.base[k] + (ddp_i64)(live ? dm : 0) * p.stride[k];
+        DdpMoments m;
+        m.s1 = 0; m.s2 = 0; m.mx = 0; m.ix = 0xffffffffu;
+        const int nchunks = (n + CH - 1) / CH;
+        if constexpr (STAGING == 0) {
+#pragma unroll UNROLL
+            for (int c = 0; c < nchunks; ++c) {
+                const int t0 = c * CH + tx * SPT;
+#pragma unroll
+                for (int v = 0; v < SPT / LV; ++v) {
+                    const int t = t0 + v * LV;
+                    if (LV > 1 && t + LV <= n) {
+                        typedef typename DdpVec<LV * 4>::type vec_t;
+                        union { vec_t v; ddp_u32 w[LV]; } r;
+                        r.v = *(const vec_t*)(row + t);
+#pragma unroll
+                        for (int e = 0; e < LV; ++e) ddp_mom_add(m, r.w[e], (ddp_u32)(t + e));
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < LV; ++e)
+                            if (t + e < n) ddp_mom_add(m, row[t + e], (ddp_u32)(t + e));
+                    }
+                }
+            }
+        } else if constexpr (STAGING == 1) {
+            for (int c = 0; c < nchunks; ++c) {
+                int len = n4 - c * CH;
+                len = len < CH ? len : CH;
+                __syncthreads();
+                for (int i = tx * 4; i < len; i += blockDim.x * 4) *(uint4*)(raw + i) = *(const uint4*)(row + c * CH + i);
+                __syncthreads();
+#pragma unroll
+                for (int s = 0; s < SPT; ++s) {
+                    const int t = c * CH + tx * SPT + s;
+                    if (t < n) ddp_mom_add(m, raw[tx * SPT + s], (ddp_u32)t);
+                }
+            }
+        } else {
+            auto issue = [&](int c, int b) {
+                int len = n4 - c * CH;
+                len = len < CH ? len : CH;
+                ddp_mbar_expect_tx(&mbar[b], (ddp_u32)(len * 4));
+                ddp_bulk_g2s(raw + (size_t)b * CH, row + c * CH, (ddp_u32)(len * 4), &mbar[b]);
+            };
+            if (tx == 0 && nchunks > 0) issue(0, (int)(nwait & 1u));
+            for (int c = 0; c < nchunks; ++c) {
+                const int b = (int)(nwait & 1u);
+                if (tx == 0 && c + 1 < nchunks) issue(c + 1, b ^ 1);
+                ddp_mbar_wait(&mbar[b], (nwait >> 1) & 1u);
+                const ddp_u32* buf = raw + (size_t)b * CH;
+#pragma unroll
+                for (int s = 0; s < SPT; ++s) {
+                    const int t = c * CH + tx * SPT + s;
+                    if (t < n) ddp_mom_add(m, buf[tx * SPT + s], (ddp_u32)t);
+                }
+                ++nwait;
+                __syncthreads();  // buffer b free for chunk c+2
+            }
+        }
+        // warp tree (lowest index wins ties)
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) {
+            const ddp_u64 s1 = __shfl_down_sync(0xffffffffu, m.s1, d);
+            const ddp_u64 s2 = __shfl_down_sync(0xffffffffu, m.s2, d);
+            const ddp_u32 mx = __shfl_down_sync(0xffffffffu, m.mx, d);
+            const ddp_u32 ix = __shfl_down_sync(0xffffffffu, m.ix, d);
+            if (lane + d < 32) ddp_mom_merge(m, s1, s2, mx, ix);
+        }
+        __syncthreads();
+        if (lane == 0) red[wx] = m;
+        __syncthreads();
+        if (tx == 0 && live) {
+            for (int w = 1; w < nwx; ++w) ddp_mom_merge(m, red[w].s1, red[w].s2, red[w].mx, red[w].ix);
+            // exact: num = n*S2 - S1^2 >= 0 in 128 bits; top = n*max - S1 >= 0
+            const unsigned __int128 num = (unsigned __int128)m.s2 * (unsigned __int128)(ddp_u64)n -
+                                          (unsigned __int128)m.s1 * (unsigned __int128)m.s1;
+            float out = 0.0f;
+            ddp_u32 am = 0u;
+            if (num != 0) {
+                const double numd = (double)(ddp_u64)(num >> 64) * 18446744073709551616.0 + (double)(ddp_u64)num;
+                const double top = (double)((ddp_u64)n * (ddp_u64)m.mx - m.s1) / (double)n;
+                const double var = numd / ((double)n * (double)(n - p.ddof));
+                out = (float)(top / sqrt(var));
+                am = m.ix;
+            }
+            p.snr[(ddp_i64)dm * p.nwidths + k] = out;
+            if (p.argmax) p.argmax[(ddp_i64)dm * p.nwidths + k] = am;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------ entry points
+#define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                         \
+    extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpDedispParams p) {                 \
+        ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC>(p);                                      \
+    }
+#define DDP_DEFINE_INTEG(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                \
+    extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpIntegParams p) {                  \
+        ddp_integ_body<SPT, DPT, UNROLL, STAGING, VEC>(p);                                             \
+    }
+#define DDP_DEFINE_SNR(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                  \
+    extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpSnrParams p) {                    \
+        ddp_snr_body<SPT, DPT, UNROLL, STAGING, VEC>(p);                                               \
+    }
+
+#endif  // DDP_KERNELS_CUH_

@@ -1,0 +1,57 @@
+// Kernel parameter records (plain data, passed by value at launch).  Included by the host launch
+// code and by the device templates, both ahead-of-time (nvcc) and at tune time (NVRTC, where this
+// text is concatenated in front of ddp_kernels.cuh) -- so no standard headers here.
+#ifndef DDP_PARAMS_H_
+#define DDP_PARAMS_H_
+
+#define DDP_MAXW 16
+
+// One dedispersion-type launch: out[g][i][t] = sum_{r<nred} in[g][r][t + delay[g][i][r]].
+//   direct:        g = 0,           i = DM trial,   r = channel
+//   subband step 1: g = subband s,   i = coarse DM a, r = channel within the subband
+//   subband step 2: g = coarse DM a, i = fine DM b,   r = subband
+struct DdpDedispParams {
+    const void* in;              // rows of the input element type
+    unsigned int* out;           // uint32 sums
+    const int* delay;            // int32 delay table (device)
+    long long in_row_stride;     // elements between consecutive reduction rows r
+    long long in_group_stride;   // elements between the first rows of consecutive groups g
+    long long in_row_len;        // readable elements per input row (loads are clipped to it)
+    long long out_dm_stride;     // elements between consecutive i of one group
+    long long out_group_stride;  // elements between the i = 0 rows of consecutive groups
+    int delay_dm_stride;         // ints between consecutive i in the delay table
+    int delay_group_off;         // ints between consecutive g in the delay table
+    int nred;                    // reduction length
+    int ndm;                     // length of the i axis
+    int ns;                      // output samples per row
+    int win;                     // staged modes: elements of one staged row window in shared memory
+};
+
+// Integration: plane k holds I_w[i][j] = sum_{m<w} in[i][j*w+m] for w = width[k] > 1.
+struct DdpIntegParams {
+    const unsigned int* in;      // dedispersed series uint32 [ndm][in_stride]
+    unsigned int* out;           // base of the planes
+    long long in_stride;
+    long long plane_off[DDP_MAXW];
+    long long plane_stride[DDP_MAXW];
+    int plane_len[DDP_MAXW];     // n_w
+    int width[DDP_MAXW];
+    int nplanes;                 // widths > 1 only
+    int ndm;
+    int ns;
+    int tiles_per_block;         // consecutive time tiles one block walks (gene "unroll")
+};
+
+// S/N (BJ:cfg0): series k of row i = n[k] values at base[k] + i*stride[k].
+struct DdpSnrParams {
+    const unsigned int* base[DDP_MAXW];
+    long long stride[DDP_MAXW];
+    int n[DDP_MAXW];
+    float* snr;                  // [ndm][nwidths]
+    unsigned int* argmax;        // [ndm][nwidths] or null
+    int nwidths;
+    int ndm;
+    int ddof;
+};
+
+#endif  // DDP_PARAMS_H_

@@ -1,0 +1,468 @@
+// Host-only part of libddp: plan creation (delay tables, geometry), kernel-configuration validity,
+// nearest-valid repair and brute-force enumeration.  No CUDA calls here.
+//
+// P:n = PAPER.md line n; BJ = BASELINE.json; readings DD.x/SB.x/INT.x/SNR.x and rules V1-V7 are
+// listed in DESIGN.md.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+
+#include "ddp_internal.h"
+
+// ------------------------------------------------------------------------------------ genes
+static const DdpGeneDomain kDomains[DDP_NGENES] = {
+    {DDP_CAND_THREADS_T, 7}, {DDP_CAND_THREADS_DM, 6}, {DDP_CAND_SPT, 5}, {DDP_CAND_DPT, 5},
+    {DDP_CAND_UNROLL, 5},    {DDP_CAND_STAGING, 3},    {DDP_CAND_VEC, 4}};
+const DdpGeneDomain* ddp_gene_domains() { return kDomains; }
+int* ddp_gene_ptr(ddp_kcfg* c, int gene) {
+    switch (gene) {
+        case 0: return &c->threads_t;
+        case 1: return &c->threads_dm;
+        case 2: return &c->samples_per_thread;
+        case 3: return &c->dms_per_thread;
+        case 4: return &c->unroll;
+        case 5: return &c->staging;
+        default: return &c->vec_bytes;
+    }
+}
+int ddp_gene_get(const ddp_kcfg& c, int gene) { return *ddp_gene_ptr(const_cast<ddp_kcfg*>(&c), gene); }
+int ddp_gene_index(int gene, int value) {
+    for (int i = 0; i < kDomains[gene].n; ++i)
+        if (kDomains[gene].v[i] == value) return i;
+    return -1;
+}
+bool ddp_kcfg_equal(const ddp_kcfg& a, const ddp_kcfg& b) { return std::memcmp(&a, &b, sizeof(ddp_kcfg)) == 0; }
+
+ddp_status ddp_fail(const ddp_plan* p, ddp_status s, const std::string& msg) {
+    if (p) p->err = msg;
+    return s;
+}
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+static inline int pow2ceil(int x) {
+    int p = 1;
+    while (p < x) p <<= 1;
+    return p;
+}
+
+// ------------------------------------------------------------------------------------ delays
+// DD.1/DD.2 (BJ:north_star): floor(((K*DM) * (f^-2 - f_ref^-2)) / t_samp + 0.5) in float64, this
+// association; this file is compiled with -ffp-contract=off.
+static bool fill_delays(const double* f, int nf, double f_ref, const double* dm, int ndm, double tsamp,
+                        std::vector<int32_t>& out, int* maxv) {
+    const double kdm = 4.148808e3;
+    const double inv_ref2 = 1.0 / (f_ref * f_ref);
+    out.resize((size_t)ndm * nf);
+    int mx = 0;
+    for (int i = 0; i < ndm; ++i)
+        for (int c = 0; c < nf; ++c) {
+            const double g = 1.0 / (f[c] * f[c]) - inv_ref2;
+            const double x = ((kdm * dm[i]) * g) / tsamp;
+            const double r = std::floor(x + 0.5);
+            if (!(r >= 0.0 && r < 1.0e9)) return false;
+            const int32_t d = (int32_t)r;
+            out[(size_t)i * nf + c] = d;
+            if (d > mx) mx = d;
+        }
+    *maxv = mx;
+    return true;
+}
+
+// ------------------------------------------------------------------------------------ plan
+static void default_kcfgs(ddp_plan* p);
+
+extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mhz, int nchan, double t_samp_s,
+                                      const double* dm_list, int ndm, const int* widths, int nwidths, int nsamp_out,
+                                      const ddp_options* opt) {
+    if (!out) return DDP_E_ARG;
+    *out = nullptr;
+    if (!chan_freq_mhz || nchan <= 0 || !widths || nwidths <= 0 || nwidths > DDP_MAX_WIDTHS || nsamp_out <= 0)
+        return DDP_E_ARG;
+    if (!(t_samp_s > 0.0) || !std::isfinite(t_samp_s)) return DDP_E_ARG;
+    for (int c = 0; c < nchan; ++c)
+        if (!(chan_freq_mhz[c] > 0.0) || !std::isfinite(chan_freq_mhz[c])) return DDP_E_ARG;
+    for (int k = 0; k < nwidths; ++k) {
+        if (widths[k] < 1) return DDP_E_ARG;
+        if (k > 0 && widths[k] <= widths[k - 1]) return DDP_E_ARG;
+    }
+    if (nsamp_out / widths[nwidths - 1] < 2) return DDP_E_ARG;
+
+    ddp_plan* p = new ddp_plan();
+    p->nchan = nchan;
+    p->ns = nsamp_out;
+    p->tsamp = t_samp_s;
+    p->nwidths = nwidths;
+    p->freq.assign(chan_freq_mhz, chan_freq_mhz + nchan);
+    for (int k = 0; k < nwidths; ++k) p->widths[k] = widths[k];
+    if (opt) {
+        p->ddof = opt->snr_ddof;
+        p->device = opt->device;
+        if (opt->cache_dir) p->cache_dir = opt->cache_dir;
+    }
+    auto bail = [&](ddp_status s) {
+        delete p;
+        return s;
+    };
+    if (p->ddof != 0 && p->ddof != 1) return bail(DDP_E_ARG);
+    if (nsamp_out / widths[nwidths - 1] - p->ddof < 1) return bail(DDP_E_ARG);
+    const double f_ref = *std::max_element(p->freq.begin(), p->freq.end());  // DD.3
+
+    int max_delay = 0, max_d1 = 0, max_d2 = 0;
+    if (opt && opt->n_subbands > 0) {
+        p->subband = true;
+        p->nsub = opt->n_subbands;
+        p->ncoarse = opt->n_coarse;
+        p->nfine = opt->n_fine;
+        p->coarse_first = opt->coarse_dm_first;
+        p->coarse_step = opt->coarse_dm_step;
+        p->fine_step = opt->fine_dm_step;
+        if (p->ncoarse <= 0 || p->nfine <= 0) return bail(DDP_E_ARG);
+        if (!(p->coarse_first >= 0.0) || !(p->coarse_step >= 0.0) || !(p->fine_step >= 0.0)) return bail(DDP_E_ARG);
+        if (!std::isfinite(p->coarse_first) || !std::isfinite(p->coarse_step) || !std::isfinite(p->fine_step))
+            return bail(DDP_E_ARG);
+        if (nchan % p->nsub != 0) return bail(DDP_E_SHAPE);  // SB.3
+        if ((int64_t)p->ncoarse * p->nfine > (int64_t)std::numeric_limits<int>::max()) return bail(DDP_E_ARG);
+        p->cps = nchan / p->nsub;
+        p->ndm = p->ncoarse * p->nfine;
+        if (dm_list && ndm != p->ndm) return bail(DDP_E_ARG);
+        std::vector<double> A(p->ncoarse), F(p->nfine), fsub(p->nsub);
+        for (int a = 0; a < p->ncoarse; ++a) A[a] = p->coarse_first + a * p->coarse_step;
+        for (int b = 0; b < p->nfine; ++b) F[b] = b * p->fine_step;
+        p->dms.resize(p->ndm);
+        for (int a = 0; a < p->ncoarse; ++a)
+            for (int b = 0; b < p->nfine; ++b) p->dms[(size_t)a * p->nfine + b] = A[a] + F[b];
+        if (dm_list)
+            for (int i = 0; i < p->ndm; ++i)
+                if (dm_list[i] != p->dms[i]) return bail(DDP_E_ARG);
+        for (int s = 0; s < p->nsub; ++s)  // SB.2: subband reference = its highest channel frequency
+            fsub[s] = *std::max_element(p->freq.begin() + (size_t)s * p->cps, p->freq.begin() + (size_t)(s + 1) * p->cps);
+        if (!fill_delays(p->freq.data(), nchan, f_ref, A.data(), p->ncoarse, t_samp_s, p->d1, &max_d1)) return bail(DDP_E_ARG);
+        if (!fill_delays(fsub.data(), p->nsub, f_ref, F.data(), p->nfine, t_samp_s, p->d2, &max_d2)) return bail(DDP_E_ARG);
+        max_delay = max_d1 + max_d2;
+    } else {
+        if (!dm_list || ndm <= 0) return bail(DDP_E_ARG);
+        for (int i = 0; i < ndm; ++i) {
+            if (!(dm_list[i] >= 0.0) || !std::isfinite(dm_list[i])) return bail(DDP_E_ARG);
+            if (i > 0 && dm_list[i] < dm_list[i - 1]) return bail(DDP_E_ARG);
+        }
+        p->ndm = ndm;
+        p->dms.assign(dm_list, dm_list + ndm);
+        if (!fill_delays(p->freq.data(), nchan, f_ref, dm_list, ndm, t_samp_s, p->delay, &max_delay)) return bail(DDP_E_ARG);
+    }
+    if ((int64_t)nsamp_out + max_delay + 64 >= (int64_t)1 << 31) return bail(DDP_E_ARG);
+
+    // Overflow proofs (INT.5): uint32 sums and uint64 second moments must be exact.
+    const int wmax = widths[nwidths - 1];
+    if ((long double)255.0L * nchan * wmax >= 4294967296.0L) return bail(DDP_E_OVERFLOW);
+    if ((long double)255.0L * nchan * 255.0L * nchan * wmax * nsamp_out >= 18446744073709551616.0L)
+        return bail(DDP_E_OVERFLOW);
+
+    ddp_plan_info& I = p->info;
+    std::memset(&I, 0, sizeof(I));
+    I.subband = p->subband ? 1 : 0;
+    I.nchan = nchan;
+    I.ndm = p->ndm;
+    I.nwidths = nwidths;
+    I.nsamp_out = nsamp_out;
+    I.n_subbands = p->nsub;
+    I.n_coarse = p->ncoarse;
+    I.n_fine = p->nfine;
+    I.max_delay = max_delay;
+    I.max_d1 = max_d1;
+    I.max_d2 = max_d2;
+    I.nsamp_in_required = (int64_t)nsamp_out + max_delay;
+    I.in_stride_min = round_up(I.nsamp_in_required + 32, 16);
+    I.out_stride_min = round_up(nsamp_out, 4);
+    I.nsamp_sub = p->subband ? (int64_t)nsamp_out + max_d2 : 0;
+    I.sub_stride = p->subband ? round_up(I.nsamp_sub + 32, 32) : 0;
+    int64_t off = 0;
+    for (int k = 0; k < nwidths; ++k) {
+        I.widths[k] = widths[k];
+        I.plane_len[k] = nsamp_out / widths[k];
+        if (widths[k] == 1) {
+            I.plane_stride[k] = 0;
+            I.plane_offset[k] = -1;
+        } else {
+            I.plane_stride[k] = round_up(I.plane_len[k], 32);
+            I.plane_offset[k] = off;
+            off += I.plane_stride[k] * p->ndm;
+        }
+    }
+    I.integ_elems = off;
+    int64_t tbytes = p->subband ? round_up((int64_t)p->d1.size() * 4, 256) + round_up((int64_t)p->d2.size() * 4, 256)
+                                : round_up((int64_t)p->delay.size() * 4, 256);
+    int64_t sbytes = p->subband ? round_up((int64_t)p->ncoarse * p->nsub * I.sub_stride * 4, 256) : 0;
+    I.workspace_bytes = tbytes + sbytes + 256;
+    I.adds_dedisp = p->subband ? (double)p->ncoarse * nchan * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
+                               : (double)p->ndm * nchan * nsamp_out;
+    default_kcfgs(p);
+    *out = p;
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_plan_destroy(ddp_plan* plan) {
+    if (!plan) return DDP_E_ARG;
+    ddp_rt_release(plan);
+    delete plan;
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_plan_query(const ddp_plan* plan, ddp_plan_info* out) {
+    if (!plan || !out) return DDP_E_ARG;
+    *out = plan->info;
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_plan_get_delays(const ddp_plan* plan, int step, int32_t* host_out) {
+    if (!plan || !host_out) return DDP_E_ARG;
+    const std::vector<int32_t>* t = nullptr;
+    if (step == 0 && !plan->subband) t = &plan->delay;
+    if (step == 1 && plan->subband) t = &plan->d1;
+    if (step == 2 && plan->subband) t = &plan->d2;
+    if (!t) return ddp_fail(plan, DDP_E_ARG, "delay table step does not exist for this plan");
+    std::memcpy(host_out, t->data(), t->size() * sizeof(int32_t));
+    return DDP_OK;
+}
+
+// ------------------------------------------------------------------------------------ kernel geometry
+bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k) {
+    switch (k) {
+        case DDP_K_DIRECT: return !p->subband;
+        case DDP_K_SUB1:
+        case DDP_K_SUB2: return p->subband;
+        case DDP_K_INTEGRATE:
+        case DDP_K_SNR: return true;
+        default: return false;
+    }
+}
+ddp_kernel ddp_slot_kernel(const ddp_plan* p, int slot) {
+    switch (slot) {
+        case 0: return p->subband ? DDP_K_SUB1 : DDP_K_DIRECT;
+        case 1: return p->subband ? DDP_K_SUB2 : DDP_K_COUNT;
+        case 2: return DDP_K_INTEGRATE;
+        case 3: return DDP_K_SNR;
+        default: return DDP_K_COUNT;
+    }
+}
+DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k) {
+    DdpKGeom g{p->ns, p->ndm, 0, 4};
+    switch (k) {
+        case DDP_K_DIRECT: g = {p->ns, p->ndm, p->nchan, 1}; break;
+        case DDP_K_SUB1: g = {(int)p->info.nsamp_sub, p->ncoarse, p->cps, 1}; break;
+        case DDP_K_SUB2: g = {p->ns, p->nfine, p->nsub, 4}; break;
+        default: break;
+    }
+    return g;
+}
+
+// Largest (dmax - dmin) of any reduction row over any DM tile of TD trials: bounds the staged window.
+int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD) {
+    const int which = k == DDP_K_DIRECT ? 0 : (k == DDP_K_SUB1 ? 1 : 2);
+    auto it = p->spread_cache[which].find(TD);
+    if (it != p->spread_cache[which].end()) return it->second;
+    const std::vector<int32_t>& t = which == 0 ? p->delay : (which == 1 ? p->d1 : p->d2);
+    const int ni = which == 0 ? p->ndm : (which == 1 ? p->ncoarse : p->nfine);
+    const int nc = which == 2 ? p->nsub : p->nchan;
+    int mx = 0;
+    for (int lo = 0; lo < ni; lo += TD) {
+        const int hi = std::min(lo + TD, ni) - 1;
+        const int32_t* a = &t[(size_t)lo * nc];
+        const int32_t* b = &t[(size_t)hi * nc];
+        for (int c = 0; c < nc; ++c) mx = std::max(mx, b[c] - a[c]);
+    }
+    p->spread_cache[which][TD] = mx;
+    return mx;
+}
+int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    const DdpKGeom g = ddp_kgeom(p, k);
+    const int AL = 16 / g.in_bytes;
+    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
+    const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 2 * AL, AL);
+}
+size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
+    switch (k) {
+        case DDP_K_DIRECT:
+        case DDP_K_SUB1:
+        case DDP_K_SUB2: {
+            if (c.staging == 0) return 0;
+            const DdpKGeom g = ddp_kgeom(p, k);
+            const size_t row = (size_t)ddp_dedisp_win(p, k, c) * g.in_bytes;
+            return c.staging == 1 ? row * c.unroll : 2 * row * c.unroll + 16;
+        }
+        case DDP_K_INTEGRATE: {
+            const int64_t prow = ((TT + (TT >> 5) + 2) + 3) & ~(int64_t)3;
+            size_t b = (size_t)c.threads_dm * (prow + 32) * 4;
+            if (c.staging != 0) b += (size_t)c.threads_dm * TT * 4 + 16;
+            return b;
+        }
+        case DDP_K_SNR: {
+            size_t b = (size_t)c.threads_dm * 32 * 24;
+            if (c.staging != 0) b += (size_t)c.threads_dm * (c.staging == 2 ? 2 : 1) * TT * 4 + (size_t)c.threads_dm * 16;
+            return b;
+        }
+        default: return 0;
+    }
+}
+
+// Validity rules (from Table 3 P:136-152 + sm_100a limits).
+bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::string* why) {
+    auto no = [&](const char* m) {
+        if (why) *why = m;
+        return false;
+    };
+    if (!ddp_kernel_in_plan(p, k)) return no("kernel not part of this plan");
+    for (int g = 0; g < DDP_NGENES; ++g)
+        if (ddp_gene_index(g, ddp_gene_get(c, g)) < 0) return no("gene value outside its candidate array");
+    const DdpKGeom geo = ddp_kgeom(p, k);
+    const int64_t threads = (int64_t)c.threads_t * c.threads_dm;
+    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
+    const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    // V7: a gene the kernel does not read is pinned (snr reads `unroll` only with direct loads)
+    if (k == DDP_K_SNR && c.staging != 0 && c.unroll != 1) return no("V7: snr ignores unroll when staged; must be 1");
+    // V5: vector width vs. what a thread loads contiguously
+    if (geo.in_bytes == 1) {
+        if (c.vec_bytes > 1 && c.vec_bytes > c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread bytes");
+    } else {
+        if (c.vec_bytes < 4) return no("V5: uint32 input needs vec_bytes >= 4");
+        if (c.vec_bytes > 4 * c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread*4");
+    }
+    // V4: unroll divides the reduction trip count
+    if (geo.nred > 0 && geo.nred % c.unroll != 0) return no("V4: unroll does not divide the reduction length");
+    // V1: block size
+    if (threads < 32 || threads > 1024) return no("V1: threads per block outside 32..1024");
+    // V2: register budget
+    if (c.samples_per_thread * c.dms_per_thread > 128) return no("V2: samples_per_thread*dms_per_thread > 128");
+    // V3: tile not larger than the (power-of-two rounded) problem
+    if (TT > pow2ceil(geo.ns_k)) return no("V3: time tile larger than the problem");
+    if (TD > pow2ceil(geo.ndm_k)) return no("V3: DM tile larger than the problem");
+    if (k == DDP_K_INTEGRATE) {
+        for (int i = 0; i < p->nwidths; ++i)
+            if (p->widths[i] > 1 && TT % p->widths[i] != 0) return no("V3: a width does not divide the time tile");
+    }
+    // V6: staged window fits shared memory
+    if (ddp_smem_bytes(p, k, c) > DDP_SMEM_LIMIT) return no("V6: shared memory over 227 KB");
+    return true;
+}
+
+const std::vector<ddp_kcfg>& ddp_valid_set(const ddp_plan* p, ddp_kernel k) {
+    if (!p->valid_built[k]) {
+        std::vector<ddp_kcfg>& v = p->valid[k];
+        v.clear();
+        const DdpGeneDomain* D = kDomains;
+        ddp_kcfg c;
+        for (int a = 0; a < D[0].n; ++a)
+            for (int b = 0; b < D[1].n; ++b)
+                for (int s = 0; s < D[2].n; ++s)
+                    for (int d = 0; d < D[3].n; ++d)
+                        for (int u = 0; u < D[4].n; ++u)
+                            for (int g = 0; g < D[5].n; ++g)
+                                for (int w = 0; w < D[6].n; ++w) {
+                                    c = {D[0].v[a], D[1].v[b], D[2].v[s], D[3].v[d], D[4].v[u], D[5].v[g], D[6].v[w]};
+                                    if (ddp_kcfg_valid(p, k, c, nullptr)) v.push_back(c);
+                                }
+        p->valid_built[k] = true;
+    }
+    return p->valid[k];
+}
+
+extern "C" ddp_status ddp_check_kcfg(const ddp_plan* plan, ddp_kernel k, const ddp_kcfg* cfg) {
+    if (!plan || !cfg || k < 0 || k >= DDP_K_COUNT) return DDP_E_ARG;
+    std::string why;
+    if (!ddp_kcfg_valid(plan, k, *cfg, &why)) return ddp_fail(plan, DDP_E_CONFIG, why);
+    return DDP_OK;
+}
+
+// Nearest valid configuration (BJ:cfg4): minimise sum over genes of |index distance| in the
+// candidate arrays (= |delta log2| for the power-of-two genes); ties -> first in canonical order.
+// A gene value outside its array is first snapped to the nearest candidate (ties -> smaller).
+extern "C" ddp_status ddp_repair_kcfg(const ddp_plan* plan, ddp_kernel k, ddp_kcfg* inout) {
+    if (!plan || !inout || k < 0 || k >= DDP_K_COUNT) return DDP_E_ARG;
+    if (!ddp_kernel_in_plan(plan, k)) return ddp_fail(plan, DDP_E_CONFIG, "kernel not part of this plan");
+    int idx[DDP_NGENES];
+    for (int g = 0; g < DDP_NGENES; ++g) {
+        const int v = ddp_gene_get(*inout, g);
+        int best = 0;
+        long bestd = -1;
+        for (int i = 0; i < kDomains[g].n; ++i) {
+            const long d = std::labs((long)kDomains[g].v[i] - v);
+            if (bestd < 0 || d < bestd) { bestd = d; best = i; }
+        }
+        idx[g] = best;
+        *ddp_gene_ptr(inout, g) = kDomains[g].v[best];
+    }
+    if (ddp_kcfg_valid(plan, k, *inout, nullptr)) return DDP_OK;
+    const std::vector<ddp_kcfg>& V = ddp_valid_set(plan, k);
+    if (V.empty()) return ddp_fail(plan, DDP_E_CONFIG, "no valid configuration exists for this kernel");
+    int bestdist = 1 << 30;
+    const ddp_kcfg* best = nullptr;
+    for (const ddp_kcfg& c : V) {
+        int d = 0;
+        for (int g = 0; g < DDP_NGENES; ++g) d += std::abs(ddp_gene_index(g, ddp_gene_get(c, g)) - idx[g]);
+        if (d < bestdist) { bestdist = d; best = &c; }
+    }
+    *inout = *best;
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_enumerate_kcfgs(const ddp_plan* plan, ddp_kernel k, ddp_kcfg* out, size_t cap, size_t* n) {
+    if (!plan || !n || k < 0 || k >= DDP_K_COUNT) return DDP_E_ARG;
+    if (!ddp_kernel_in_plan(plan, k)) { *n = 0; return DDP_OK; }
+    const std::vector<ddp_kcfg>& V = ddp_valid_set(plan, k);
+    *n = V.size();
+    if (out)
+        for (size_t i = 0; i < V.size() && i < cap; ++i) out[i] = V[i];
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_get_kcfg(const ddp_plan* plan, ddp_kernel k, ddp_kcfg* out) {
+    if (!plan || !out || k < 0 || k >= DDP_K_COUNT) return DDP_E_ARG;
+    if (!ddp_kernel_in_plan(plan, k)) return ddp_fail(plan, DDP_E_CONFIG, "kernel not part of this plan");
+    *out = plan->kcfg[k];
+    return DDP_OK;
+}
+
+extern "C" ddp_status ddp_set_kcfg(ddp_plan* plan, ddp_kernel k, const ddp_kcfg* cfg) {
+    if (!plan || !cfg || k < 0 || k >= DDP_K_COUNT) return DDP_E_ARG;
+    std::string why;
+    if (!ddp_kcfg_valid(plan, k, *cfg, &why)) return ddp_fail(plan, DDP_E_CONFIG, why);
+    ddp_status s = ddp_rt_activate(plan, k, *cfg);  // DDP_OK without a device: compiled lazily at first launch
+    if (s != DDP_OK) return s;
+    plan->kcfg[k] = *cfg;
+    return DDP_OK;
+}
+
+// Default configurations: preferred shapes repaired into the plan's valid space.
+static void default_kcfgs(ddp_plan* p) {
+    const ddp_kcfg pref[DDP_K_COUNT] = {
+        /* direct    */ {64, 4, 8, 4, 8, 0, 4},
+        /* sub1      */ {64, 4, 8, 2, 8, 0, 4},
+        /* sub2      */ {128, 2, 4, 4, 4, 0, 16},
+        /* integrate */ {256, 1, 4, 1, 1, 0, 16},
+        /* snr       */ {256, 1, 4, 1, 4, 0, 16},
+    };
+    for (int k = 0; k < DDP_K_COUNT; ++k) {
+        p->kcfg[k] = pref[k];
+        if (ddp_kernel_in_plan(p, (ddp_kernel)k)) ddp_repair_kcfg(p, (ddp_kernel)k, &p->kcfg[k]);
+    }
+}
+
+extern "C" const char* ddp_status_str(ddp_status s) {
+    switch (s) {
+        case DDP_OK: return "ok";
+        case DDP_E_ARG: return "bad argument";
+        case DDP_E_SHAPE: return "bad shape/stride/alignment";
+        case DDP_E_OVERFLOW: return "accumulation could overflow";
+        case DDP_E_WORKSPACE: return "workspace missing or too small";
+        case DDP_E_CONFIG: return "invalid kernel configuration";
+        case DDP_E_COMPILE: return "kernel compilation failed";
+        case DDP_E_CUDA: return "CUDA error or no device";
+        case DDP_E_BUDGET: return "evaluation budget exhausted";
+        default: return "unknown status";
+    }
+}
+extern "C" const char* ddp_last_error(const ddp_plan* plan) { return plan ? plan->err.c_str() : ""; }
+extern "C" const char* ddp_version(void) { return "ddp 0.1 (sm_100a)"; }

@@ -1,0 +1,235 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bar (BASELINE.json north_star): dedispersion and integration bit-exact (uint8 in, uint32
+accumulate), S/N within 1e-5 relative, argmax exact.  Small cases span several tiles and ragged
+tails; full-size configs are checked on sampled DM rows the oracle computes one by one.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():  # collected on the CPU box, run on the B200 box
+    pytest.skip("no CUDA device", allow_module_level=True)
+
+import paper_1811_04165_b200 as ddp  # noqa: E402
+from synth import configs  # noqa: E402
+from synth.configs import SubbandPlan  # noqa: E402
+
+from gpu_common import (GpuSearch, assert_snr_close, compare_all, oracle_direct_rows, oracle_search,  # noqa: E402
+                        oracle_subband, u32)
+
+
+def small_direct(**kw):
+    base = dict(name="small_direct", nchan=80, nsamp_out=3001, ndm=37, widths=(1, 2, 4, 8, 16), n_pulses=3)
+    base.update(kw)
+    return configs.scaled(configs.apertif_direct(), **base)
+
+
+def small_subband(**kw):
+    base = dict(name="small_subband", nchan=96, nsamp_out=2500, ndm=30, widths=(1, 2, 4, 8), n_pulses=2,
+                subband=SubbandPlan(n_subbands=8, n_coarse=6, coarse_first=0.0, coarse_step=8.0, n_fine=5,
+                                    fine_step=0.25))
+    base.update(kw)
+    return configs.scaled(configs.apertif_direct(), **base)
+
+
+# ---------------------------------------------------------------------------------- whole pipeline
+def test_cfg0_full_pipeline_and_pulse_recovery():
+    cfg = configs.tiny()
+    g = GpuSearch(cfg)
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="cfg0")
+    S = g.buf["d_snr"].cpu().numpy()
+    i, k = np.unravel_index(np.argmax(S), S.shape)
+    assert cfg.dm_list()[i] == 17.0 and cfg.widths[k] == 4  # BJ:cfg0 pulse: DM 17, width 4
+    A = u32(g.buf["d_argmax"])
+    assert A[i, k] * 4 == 2000                               # t0 = 2000
+    g.close()
+
+
+def test_small_direct_ragged():
+    cfg = small_direct()
+    g = GpuSearch(cfg)
+    g.run_all()
+    compare_all(g, oracle_direct_rows(cfg, g.X), what="small_direct")
+    g.close()
+
+
+def test_small_subband_ragged_and_intermediate():
+    cfg = small_subband()
+    g = GpuSearch(cfg)
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    Sg = g.subband_intermediate()
+    assert np.array_equal(Sg, So), "subband intermediate S differs"
+    compare_all(g, Yo, what="small_subband")
+    # SB.6: rows with zero fine offset equal the direct result at the coarse DM
+    sb = cfg.subband
+    A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+    import oracle
+    Yd = oracle.dedisperse(g.X, oracle.delay_table(cfg.chan_freq_mhz(), A, cfg.t_samp_s), cfg.nsamp_out)
+    Yg = u32(g.buf["d_out"])[:: sb.n_fine, : cfg.nsamp_out]
+    assert np.array_equal(Yg, Yd)
+    g.close()
+
+
+# ---------------------------------------------------------------------------------- edge cases
+def test_single_dm_zero_is_channel_sum():
+    cfg = small_direct(name="dm0", ndm=1, nsamp_out=1000, widths=(1, 2), n_pulses=0)
+    g = GpuSearch(cfg)
+    Y = g.dedisperse()
+    assert np.array_equal(Y[0], g.X[:, :1000].astype(np.uint32).sum(axis=0))  # BJ: DM=0 == plain channel sum
+    g.close()
+
+
+def test_width_one_only_and_tiny_series():
+    cfg = small_direct(name="w1", ndm=3, nsamp_out=5, widths=(1,), nchan=16, n_pulses=0)
+    g = GpuSearch(cfg)
+    g.run_all()
+    compare_all(g, oracle_direct_rows(cfg, g.X), what="w1")
+    g.close()
+
+
+def test_saturated_input_maximum_values():
+    # all samples 255: the largest sums the accumulators can see for this shape (INT.5)
+    cfg = small_direct(name="sat", nchan=64, ndm=9, nsamp_out=2048, widths=(1, 2, 4, 8, 16, 32, 64, 128, 256), n_pulses=0)
+    probe = GpuSearch(cfg)
+    X = np.full_like(probe.X, 255)
+    probe.close()
+    g = GpuSearch(cfg, X=X)
+    Y, P, S, A = g.run_all()
+    assert (Y == 255 * 64).all()
+    assert (P[256] == 255 * 64 * 256).all()
+    assert (S == 0).all() and (A == 0).all()  # SNR.3: constant series -> 0, argmax 0
+    g.close()
+
+
+def test_error_behaviour():
+    cfg = small_direct(name="err", ndm=4, nsamp_out=512, widths=(1, 2), n_pulses=0)
+    plan = ddp.plan_from_config(cfg)
+    b = ddp.alloc_buffers(plan, bind=False)
+    with pytest.raises(ddp.DdpError) as e:
+        plan.dedisperse(b["d_in"], b["d_out"])
+    assert e.value.status == ddp.binding.E_WORKSPACE
+    plan.bind_workspace(b["workspace"])
+    with pytest.raises(ddp.DdpError) as e:
+        plan.dedisperse(b["d_in"], b["d_out"], in_stride=16)
+    assert e.value.status == ddp.binding.E_SHAPE
+    bad = ddp.Kcfg(64, 4, 8, 4, 7, 0, 4)
+    with pytest.raises(ddp.DdpError) as e:
+        plan.set_kcfg(ddp.K_DIRECT, bad)
+    assert e.value.status == ddp.binding.E_CONFIG
+    plan.destroy()
+
+
+# ---------------------------------------------------------------------------------- configuration sweep
+def _sample(cfgs, n, seed):
+    """n configurations: evenly strided over the canonical enumeration plus seeded random picks, so
+    that every staging mode and vector width appears."""
+    rng = np.random.default_rng(seed)
+    idx = set(np.linspace(0, len(cfgs) - 1, n // 2).astype(int).tolist())
+    idx |= set(rng.integers(0, len(cfgs), n - len(idx)).tolist())
+    return [cfgs[i] for i in sorted(idx)]
+
+
+@pytest.mark.parametrize("kernel", [ddp.K_DIRECT, ddp.K_INTEGRATE, ddp.K_SNR])
+def test_direct_plan_kernel_configuration_sweep(kernel):
+    cfg = small_direct(name="sweep", nchan=64, nsamp_out=2300, ndm=41, widths=(1, 2, 4, 8, 16, 32))
+    g = GpuSearch(cfg)
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="sweep default")
+    seen = set()
+    for c in _sample(g.plan.enumerate_kcfgs(kernel), 48, seed=kernel):
+        g.plan.set_kcfg(kernel, c)
+        seen.add((c.staging, c.vec_bytes))
+        if kernel == ddp.K_DIRECT:
+            g.buf["d_out"].fill_(-1)
+            g.dedisperse()
+        elif kernel == ddp.K_INTEGRATE:
+            g.buf["d_integ"].fill_(-1)
+            g.integrate()
+        g.buf["d_snr"].fill_(-7.0)
+        g.buf["d_argmax"].fill_(-1)
+        if kernel != ddp.K_SNR:
+            g.integrate()
+        g.snr()
+        compare_all(g, Yo, what="%s %r" % (ddp.KERNEL_NAMES[kernel], c))
+    assert {s for s, _ in seen} == {0, 1, 2}
+    g.close()
+
+
+@pytest.mark.parametrize("kernel", [ddp.K_SUB1, ddp.K_SUB2])
+def test_subband_plan_kernel_configuration_sweep(kernel):
+    cfg = small_subband(name="sweep_sb", nchan=128, nsamp_out=2100, ndm=24 * 8,
+                        subband=SubbandPlan(n_subbands=8, n_coarse=24, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=8, fine_step=0.25))
+    g = GpuSearch(cfg)
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    compare_all(g, Yo, what="sweep_sb default")
+    seen = set()
+    for c in _sample(g.plan.enumerate_kcfgs(kernel), 48, seed=kernel):
+        g.plan.set_kcfg(kernel, c)
+        seen.add(c.staging)
+        g.buf["d_out"].fill_(-1)
+        Y = g.dedisperse()
+        assert np.array_equal(g.subband_intermediate(), So), "S differs for %r" % c
+        assert np.array_equal(Y, Yo), "Y differs for %s %r" % (ddp.KERNEL_NAMES[kernel], c)
+    assert seen == {0, 1, 2}
+    g.close()
+
+
+# ---------------------------------------------------------------------------------- full-size configs
+def _sampled_rows(ndm, n, seed):
+    rng = np.random.default_rng(seed)
+    rows = {0, 1, ndm // 2, ndm - 2, ndm - 1} | set(rng.integers(0, ndm, n).tolist())
+    return np.array(sorted(rows))
+
+
+@pytest.mark.slow
+def test_cfg1_full_size_sampled_rows():
+    cfg = configs.apertif_direct()
+    g = GpuSearch(cfg)
+    g.run_all()
+    rows = _sampled_rows(cfg.ndm, 12, 1)
+    compare_all(g, oracle_direct_rows(cfg, g.X, rows), rows=rows, what="cfg1")
+    # every injected pulse is found at its DM (rows of the pulses' DMs carry the S/N maxima nearby)
+    S = g.buf["d_snr"].cpu().numpy()
+    for p in g.pulses:
+        i = int(round(p.dm / cfg.dm_step))
+        lo, hi = max(0, i - 8), min(cfg.ndm, i + 9)
+        assert S[lo:hi].max() > 6.0, "pulse %r not detected" % (p,)
+    g.close()
+
+
+@pytest.mark.slow
+def test_cfg2_full_size_sampled_rows_and_identity_rows():
+    cfg = configs.apertif_subband()
+    g = GpuSearch(cfg)
+    g.run_all()
+    sb = cfg.subband
+    coarse = np.array([0, 1, 31, 63])
+    So, Yo = oracle_subband(cfg, g.X, coarse)
+    Sg = g.subband_intermediate()[coarse]
+    assert np.array_equal(Sg, So)
+    rows = (coarse[:, None] * sb.n_fine + np.arange(sb.n_fine)[None, :]).reshape(-1)
+    compare_all(g, Yo, rows=rows, what="cfg2")
+    # SB.6 / BJ:cfg2: zero-fine-offset rows equal config 1's direct rows at the same DM
+    d = configs.apertif_direct()
+    Yd = oracle_direct_rows(d, g.X, coarse * sb.n_fine)
+    assert np.array_equal(u32(g.buf["d_out"])[coarse * sb.n_fine, : cfg.nsamp_out], Yd)
+    g.close()
+
+
+@pytest.mark.slow
+def test_cfg3_full_size_sampled_rows():
+    cfg = configs.ska_mid()
+    g = GpuSearch(cfg)
+    g.run_all()
+    rows = _sampled_rows(cfg.ndm, 5, 3)
+    compare_all(g, oracle_direct_rows(cfg, g.X, rows), rows=rows, what="cfg3")
+    g.close()
