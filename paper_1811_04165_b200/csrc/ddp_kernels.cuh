@@ -309,9 +309,10 @@ __device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
     constexpr int LV = VE < SPT ? VE : SPT;       // elements per load actually usable
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int TT = blockDim.x * SPT;
-    const int lane = tx & 31, wx = tx >> 5;
+    const int SW = blockDim.x < 32 ? blockDim.x : 32;  // shuffle segment: a warp may span several ty rows
+    const int lane = tx & (SW - 1), wx = tx >> 5;
     const int nwx = (blockDim.x + 31) >> 5;
-    const int prow = ddp_pad(TT) + 2;  // padded prefix row length
+    const int prow = (ddp_pad(TT) + 2 + 3) & ~3;  // padded prefix row length, multiple of 4 (ddp_smem_bytes)
     ddp_u32* P = (ddp_u32*)ddp_smem + (size_t)ty * prow;
     ddp_u32* wtot = (ddp_u32*)ddp_smem + (size_t)blockDim.y * prow + ty * 32;
     // raw staging area (STAGING 1/2): one tile per ty
@@ -380,10 +381,10 @@ __device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
             ddp_u32 incl = x[SPT - 1];
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
-                const ddp_u32 n = __shfl_up_sync(0xffffffffu, incl, d);
+                const ddp_u32 n = __shfl_up_sync(0xffffffffu, incl, d, SW);
                 if (lane >= d) incl += n;
             }
-            if (lane == 31 || tx == (int)blockDim.x - 1) wtot[wx] = incl;
+            if (lane == SW - 1) wtot[wx] = incl;
             __syncthreads();
             ddp_u32 base = incl - x[SPT - 1];  // exclusive within the warp
             for (int w = 0; w < wx; ++w) base += wtot[w];
@@ -439,7 +440,8 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
     const int n = p.n[k];
     const int n4 = (n + 3) & ~3;
     const int CH = blockDim.x * SPT;  // values per chunk
-    const int lane = tx & 31, wx = tx >> 5;
+    const int SW = blockDim.x < 32 ? blockDim.x : 32;  // shuffle segment: a warp may span several ty rows
+    const int lane = tx & (SW - 1), wx = tx >> 5;
     const int nwx = (blockDim.x + 31) >> 5;
     // shared: reduction scratch [blockDim.y][32] moments, then staging tiles
     DdpMoments* red = (DdpMoments*)ddp_smem + (size_t)ty * 32;
@@ -523,11 +525,11 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
         // warp tree (lowest index wins ties)
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1) {
-            const ddp_u64 s1 = __shfl_down_sync(0xffffffffu, m.s1, d);
-            const ddp_u64 s2 = __shfl_down_sync(0xffffffffu, m.s2, d);
-            const ddp_u32 mx = __shfl_down_sync(0xffffffffu, m.mx, d);
-            const ddp_u32 ix = __shfl_down_sync(0xffffffffu, m.ix, d);
-            if (lane + d < 32) ddp_mom_merge(m, s1, s2, mx, ix);
+            const ddp_u64 s1 = __shfl_down_sync(0xffffffffu, m.s1, d, SW);
+            const ddp_u64 s2 = __shfl_down_sync(0xffffffffu, m.s2, d, SW);
+            const ddp_u32 mx = __shfl_down_sync(0xffffffffu, m.mx, d, SW);
+            const ddp_u32 ix = __shfl_down_sync(0xffffffffu, m.ix, d, SW);
+            if (lane + d < SW) ddp_mom_merge(m, s1, s2, mx, ix);
         }
         __syncthreads();
         if (lane == 0) red[wx] = m;
