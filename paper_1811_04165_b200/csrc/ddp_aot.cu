@@ -5,20 +5,22 @@
 #include "ddp_params.h"
 #include "ddp_kernels.cuh"
 
-#define DDP_AOT_U8(S, D, U, G, V, T) DDP_DEFINE_DEDISP(ddp_dedisp_u8_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, ddp_u8, S, D, U, G, V, T)
-#define DDP_AOT_U32(S, D, U, G, V, T) DDP_DEFINE_DEDISP(ddp_dedisp_u32_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, ddp_u32, S, D, U, G, V, T)
+#define DDP_AOT_U8(S, D, U, G, V, T, W) DDP_DEFINE_DEDISP(ddp_dedisp_u8_s##S##_d##D##_u##U##_g##G##_v##V##_t##T##_w##W, ddp_u8, S, D, U, G, V, T, W)
+#define DDP_AOT_U32(S, D, U, G, V, T) DDP_DEFINE_DEDISP(ddp_dedisp_u32_s##S##_d##D##_u##U##_g##G##_v##V##_t##T##_w0, ddp_u32, S, D, U, G, V, T, 0)
 #define DDP_AOT_INTEG(S, D, U, G, V, T) DDP_DEFINE_INTEG(ddp_integ_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 #define DDP_AOT_SNR(S, D, U, G, V, T) DDP_DEFINE_SNR(ddp_snr_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 
 // plan defaults (ddp_plan.cpp::default_kcfgs)
-DDP_AOT_U8(8, 4, 8, 0, 4, 256)
-DDP_AOT_U8(8, 2, 8, 0, 4, 256)
+DDP_AOT_U8(16, 4, 8, 1, 16, 256, 1)
+DDP_AOT_U8(16, 2, 8, 1, 16, 256, 0)
 DDP_AOT_U32(4, 4, 4, 0, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 0, 16, 256)
 DDP_AOT_SNR(4, 1, 4, 0, 16, 256)
 // one instance of every staging mode per kernel (SASS evidence: LDS / UBLKCP paths)
-DDP_AOT_U8(16, 4, 8, 1, 16, 256)
-DDP_AOT_U8(16, 4, 8, 2, 16, 256)
+DDP_AOT_U8(8, 4, 8, 0, 4, 256, 0)
+DDP_AOT_U8(16, 4, 8, 1, 16, 256, 0)
+DDP_AOT_U8(16, 4, 8, 2, 16, 256, 1)
+DDP_AOT_U8(16, 4, 8, 2, 16, 256, 0)
 DDP_AOT_U32(4, 4, 4, 1, 16, 256)
 DDP_AOT_U32(4, 4, 4, 2, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 1, 16, 256)

@@ -294,6 +294,244 @@ __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
     }
 }
 
+// ------------------------------------------------------------------------------------ packed staged dedispersion
+// uint8 input, STAGING 1 (cooperative loads) or 2 (TMA bulk copies).  The inner loop is built for the
+// sm_100a issue limits measured in profiles/: one LDS.32 brings FOUR consecutive samples of one
+// (channel, trial) to a thread, LOP3 / PRMT split them into two registers of 2 x 16-bit lanes
+// (bytes 0,2 and bytes 1,3) and two IMADs (x * 1 + acc, the 1 being a run-time value so that the
+// adds go to the fma pipe while the extractions use the alu pipe) accumulate them: 5 issued
+// instructions per 4 adds.  16-bit lanes are exact for <= 257 channels (255 * 257 = 65535), so they
+// are flushed into uint32 totals every 256 channels (WIDE) or unpacked once at the end (!WIDE).
+//
+// Per chunk of U channels the block stages, for each channel, the window its TD trials need --
+// [tile_t + dmin, tile_t + TT + dmax), from the 16-byte aligned-down start -- as FOUR copies
+// shifted by 0..3 bytes (copy o, word q = window bytes 4q+o .. 4q+o+3), so that a thread's delayed
+// window is word aligned in one of them whatever the delay.  Thread tx of a warp owns the words
+// {32*K*(tx/32) + tx%32 + 32k, k < K}: every LDS.32 of a warp reads 32 consecutive words
+// (conflict free) and the 128k-byte steps are immediates.  The per-(trial, channel) shared-memory
+// offsets are computed once per chunk by one thread each (table `offs`), from the tile's delays
+// kept in shared memory per superchunk of 64 channels (`dls`).  Copies, offsets and delays are
+// double buffered: chunk c+1 is staged while chunk c is summed, one __syncthreads per chunk.
+template <int VW>
+__device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst, int cstride) {
+    ddp_u32 w[VW + 1];
+    if constexpr (VW == 4) {
+        const uint4 v = *(const uint4*)src;
+        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+    } else if constexpr (VW == 2) {
+        const uint2 v = *(const uint2*)src;
+        w[0] = v.x; w[1] = v.y;
+    } else {
+        w[0] = src[0];
+    }
+    w[VW] = src[VW];
+#pragma unroll
+    for (int o = 0; o < 4; ++o) {
+        ddp_u32 x[VW];
+#pragma unroll
+        for (int i = 0; i < VW; ++i) x[i] = o == 0 ? w[i] : ddp_shf_r(w[i], w[i + 1], 8u * o);
+        ddp_u32* d = dst + o * cstride;
+        if constexpr (VW == 4) *(uint4*)d = make_uint4(x[0], x[1], x[2], x[3]);
+        else if constexpr (VW == 2) *(uint2*)d = make_uint2(x[0], x[1]);
+        else d[0] = x[0];
+    }
+}
+
+template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE>
+__device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p) {
+    static_assert(SPT >= 4 && VEC >= 4, "packed staging works on whole 4-sample words");
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int K = SPT / 4;   // words per thread
+    constexpr int VW = VEC / 4;  // words per staging load
+    constexpr int SC = 64;       // channels per delay superchunk (multiple of every U)
+    constexpr int FL = 256;      // channels between flushes of the 16-bit lanes
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int nthreads = blockDim.x * blockDim.y;
+    const int tid = ty * blockDim.x + tx;
+    const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
+    const int TT = blockDim.x * SPT, TD = blockDim.y * DPT;
+    const int g = blockIdx.z;
+    const int tile_t = blockIdx.x * TT;
+    const int tile_dm = blockIdx.y * TD;
+    const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
+    const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)g * p.in_group_stride;
+    const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
+    const int win = p.win, winw = win >> 2;
+    const ddp_u32 one = (ddp_u32)p.one;
+
+    // shared-memory carve-up (ddp_smem_bytes mirrors it)
+    ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [2][U][4][winw]
+    ddp_u32* offs = copies + (size_t)2 * U * 4 * winw;           // [2][TD][U]   byte offsets into ddp_smem
+    int* dls = (int*)(offs + (((size_t)2 * TD * U + 3) & ~(size_t)3));  // [2][TD][SC], 16-byte aligned
+    unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
+    ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
+    const int nchunks = p.nred / U;
+
+    auto load_dls = [&](int s) {
+        int* d = dls + (size_t)(s & 1) * TD * SC;
+        const int r0 = s * SC;
+        for (int idx = tid; idx < TD * SC; idx += nthreads) {
+            const int j = idx / SC, cc = idx - j * SC;
+            if (r0 + cc < p.nred) d[idx] = dl[(ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride + r0 + cc];
+        }
+    };
+    // staged extent of reduction row r: aligned start (elements from the row start) and words to stage
+    auto row_extent = [&](int r, ddp_i64& a0, int& lenw) {
+        const int s = r / SC;
+        const int dmin = dls[(size_t)(s & 1) * TD * SC + (r - s * SC)];
+        a0 = ((ddp_i64)tile_t + dmin) & ~(ddp_i64)15;
+        ddp_i64 l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
+        lenw = (int)(l < winw ? (l < 0 ? 0 : l) : winw);
+    };
+    auto tma_issue = [&](int c) {  // one thread: raw windows of chunk c -> raw slot c & 1
+        unsigned char* dst = raw + (size_t)(c & 1) * U * (win + 16);
+        ddp_i64 a0s[U];
+        int lens[U];
+        ddp_u32 total = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            row_extent(c * U + u, a0s[u], lens[u]);
+            if (lens[u] > 0) total += (ddp_u32)lens[u] * 4u + 16u;
+        }
+        ddp_mbar_expect_tx(&mbar[c & 1], total);
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (lens[u] > 0)
+                ddp_bulk_g2s(dst + (size_t)u * (win + 16), in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0s[u],
+                             (ddp_u32)lens[u] * 4u + 16u, &mbar[c & 1]);
+    };
+    // chunk c -> the four shifted copies of buffer c & 1 (source: global memory, or the raw TMA slot)
+    auto stage = [&](int c) {
+        ddp_u32* cb = copies + (size_t)(c & 1) * U * 4 * winw;
+        const int upr = winw / VW;                 // load units per row
+        const int nvb = (upr + 31) >> 5;           // 32-unit blocks per row
+        for (int unit = warp; unit < U * nvb; unit += nwarps) {
+            const int u = unit / nvb, v = (unit - u * nvb) * 32 + lane;
+            ddp_i64 a0;
+            int lenw;
+            row_extent(c * U + u, a0, lenw);
+            if (v * VW < lenw) {
+                const ddp_u32* src;
+                if constexpr (STAGING == 2)
+                    src = (const ddp_u32*)(raw + ((size_t)(c & 1) * U + u) * (win + 16)) + v * VW;
+                else
+                    src = (const ddp_u32*)(in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0) + v * VW;
+                ddp_shift_store<VW>(src, cb + (size_t)u * 4 * winw + v * VW, winw);
+            }
+        }
+    };
+    auto prep_offs = [&](int c) {
+        ddp_u32* ob = offs + (size_t)(c & 1) * TD * U;
+        const ddp_u32 cbase = (ddp_u32)((size_t)(c & 1) * U * 4 * winw);
+        const int s = (c * U) / SC;
+        const int* d = dls + (size_t)(s & 1) * TD * SC + (c * U - s * SC);
+        for (int idx = tid; idx < TD * U; idx += nthreads) {
+            const int j = idx / U, u = idx - j * U;
+            const int dmin = d[u];
+            const int dd = d[(j < nd ? j : nd - 1) * SC + u];
+            const int pos = (int)(((ddp_i64)tile_t + dmin) & 15) + (dd - dmin);
+            ob[idx] = (cbase + (ddp_u32)((u * 4 + (pos & 3)) * winw + (pos >> 2))) * 4u;
+        }
+    };
+
+    ddp_u32 accE[DPT][K], accO[DPT][K];
+    ddp_u32 tot[WIDE ? DPT : 1][WIDE ? K : 1][4];
+#pragma unroll
+    for (int j = 0; j < DPT; ++j)
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            accE[j][k] = accO[j][k] = 0u;
+            if constexpr (WIDE) tot[j][k][0] = tot[j][k][1] = tot[j][k][2] = tot[j][k][3] = 0u;
+        }
+    const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
+
+    if constexpr (STAGING == 2) {
+        if (tid == 0) {
+            ddp_mbar_init(&mbar[0], 1);
+            ddp_mbar_init(&mbar[1], 1);
+            ddp_mbar_fence_init();
+        }
+    }
+    load_dls(0);
+    __syncthreads();
+    if constexpr (STAGING == 2) {
+        if (tid == 0) {
+            tma_issue(0);
+            if (nchunks > 1) tma_issue(1);
+        }
+        ddp_mbar_wait(&mbar[0], 0u);
+    }
+    stage(0);
+    prep_offs(0);
+    __syncthreads();
+
+    for (int c = 0; c < nchunks; ++c) {
+        const int r0 = c * U;
+        if (r0 % SC == 0 && r0 + SC < p.nred) load_dls(r0 / SC + 1);
+        if (c + 1 < nchunks) {
+            if constexpr (STAGING == 2) {
+                if (tid == 0 && c + 2 < nchunks) tma_issue(c + 2);  // slot c & 1 was converted during iteration c - 1
+                ddp_mbar_wait(&mbar[(c + 1) & 1], (ddp_u32)(((c + 1) >> 1) & 1));
+            }
+            stage(c + 1);
+            prep_offs(c + 1);
+        }
+        const ddp_u32* ob = offs + ((size_t)(c & 1) * TD + ty * DPT) * U;
+#pragma unroll
+        for (int j = 0; j < DPT; ++j) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const ddp_u32* wp = (const ddp_u32*)(ddp_smem + ob[j * U + u]) + wb;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    const ddp_u32 w = wp[32 * k];
+                    const ddp_u32 e = w & 0x00ff00ffu;
+                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
+                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accE[j][k]) : "r"(e), "r"(one));
+                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
+                }
+            }
+        }
+        if constexpr (WIDE) {
+            if ((r0 + U) % FL == 0) {
+#pragma unroll
+                for (int j = 0; j < DPT; ++j)
+#pragma unroll
+                    for (int k = 0; k < K; ++k) {
+                        tot[j][k][0] += accE[j][k] & 0xffffu;
+                        tot[j][k][1] += accO[j][k] & 0xffffu;
+                        tot[j][k][2] += accE[j][k] >> 16;
+                        tot[j][k][3] += accO[j][k] >> 16;
+                        accE[j][k] = accO[j][k] = 0u;
+                    }
+            }
+        }
+        __syncthreads();
+    }
+
+#pragma unroll
+    for (int j = 0; j < DPT; ++j) {
+        const int dm = tile_dm + ty * DPT + j;
+        if (dm >= p.ndm) continue;
+        ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = accO[j][k] & 0xffffu, v2 = accE[j][k] >> 16, v3 = accO[j][k] >> 16;
+            if constexpr (WIDE) {
+                v0 += tot[j][k][0]; v1 += tot[j][k][1]; v2 += tot[j][k][2]; v3 += tot[j][k][3];
+            }
+            const int t = tile_t + 4 * (wb + 32 * k);
+            if (t + 3 < p.ns) {
+                *(uint4*)(orow + t) = make_uint4(v0, v1, v2, v3);
+            } else {
+                if (t < p.ns) orow[t] = v0;
+                if (t + 1 < p.ns) orow[t + 1] = v1;
+                if (t + 2 < p.ns) orow[t + 2] = v2;
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------ integration
 // Tile = TT = blockDim.x*SPT consecutive samples of one row; every width divides TT (host rule).
 // Per row: SPT samples per thread (vector loads), thread-local running sums, warp inclusive scan of
@@ -555,9 +793,17 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
 }
 
 // ------------------------------------------------------------------------------------ entry points
-#define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                         \
+// uint8 input with staging takes the packed kernel; everything else the generic one.
+template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, bool WIDE>
+__device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
+    if constexpr (sizeof(IN_T) == 1 && STAGING != 0)
+        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE>(p);
+    else
+        ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC>(p);
+}
+#define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT, WIDE)                   \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpDedispParams p) {                 \
-        ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC>(p);                                      \
+        ddp_dedisp_entry<IN_T, SPT, DPT, UNROLL, STAGING, VEC, (WIDE) != 0>(p);                        \
     }
 #define DDP_DEFINE_INTEG(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpIntegParams p) {                  \

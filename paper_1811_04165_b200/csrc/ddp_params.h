@@ -25,6 +25,7 @@ struct DdpDedispParams {
     int ndm;                     // length of the i axis
     int ns;                      // output samples per row
     int win;                     // staged modes: elements of one staged row window in shared memory
+    int one;                     // the value 1, unknown to the compiler (packed kernel: adds issued as IMAD)
 };
 
 // Integration: plane k holds I_w[i][j] = sum_{m<w} in[i][j*w+m] for w = width[k] > 1.

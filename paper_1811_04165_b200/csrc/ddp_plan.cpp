@@ -280,6 +280,8 @@ int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const int AL = 16 / g.in_bytes;
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    if (g.in_bytes == 1)  // packed kernel: 16-byte carry + shifted-copy tail, in bytes, multiple of 16
+        return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 32, 16);
     return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 2 * AL, AL);
 }
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
@@ -291,6 +293,12 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (c.staging == 0) return 0;
             const DdpKGeom g = ddp_kgeom(p, k);
             const size_t row = (size_t)ddp_dedisp_win(p, k, c) * g.in_bytes;
+            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [2][U][4][win], offs [2][TD][U], dls [2][TD][64], raw, mbar
+                const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
+                size_t b = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+                if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
+                return b;
+            }
             return c.staging == 1 ? row * c.unroll : 2 * row * c.unroll + 16;
         }
         case DDP_K_INTEGRATE: {
@@ -326,6 +334,11 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
     // V5: vector width vs. what a thread loads contiguously
     if (geo.in_bytes == 1) {
         if (c.vec_bytes > 1 && c.vec_bytes > c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread bytes");
+        if (c.staging != 0) {  // the packed kernel works on whole 4-sample words, one warp per 32 of them
+            if (c.samples_per_thread < 4) return no("V5: staged uint8 input needs samples_per_thread >= 4");
+            if (c.vec_bytes < 4) return no("V5: staged uint8 input needs vec_bytes >= 4");
+            if (c.threads_t < 32) return no("V1: staged uint8 input needs threads_t >= 32");
+        }
     } else {
         if (c.vec_bytes < 4) return no("V5: uint32 input needs vec_bytes >= 4");
         if (c.vec_bytes > 4 * c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread*4");
@@ -438,8 +451,8 @@ extern "C" ddp_status ddp_set_kcfg(ddp_plan* plan, ddp_kernel k, const ddp_kcfg*
 // Default configurations: preferred shapes repaired into the plan's valid space.
 static void default_kcfgs(ddp_plan* p) {
     const ddp_kcfg pref[DDP_K_COUNT] = {
-        /* direct    */ {64, 4, 8, 4, 8, 0, 4},
-        /* sub1      */ {64, 4, 8, 2, 8, 0, 4},
+        /* direct    */ {64, 4, 16, 4, 8, 1, 16},
+        /* sub1      */ {64, 4, 16, 2, 8, 1, 16},
         /* sub2      */ {128, 2, 4, 4, 4, 0, 16},
         /* integrate */ {256, 1, 4, 1, 1, 0, 16},
         /* snr       */ {256, 1, 4, 1, 4, 0, 16},

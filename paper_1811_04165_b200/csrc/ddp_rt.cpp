@@ -225,22 +225,31 @@ const char* kind_tag(CodeKind ck) {
     static const char* t[] = {"ddp_dedisp_u8", "ddp_dedisp_u32", "ddp_integ", "ddp_snr"};
     return t[ck];
 }
-std::string kernel_name(ddp_kernel k, const ddp_kcfg& c) {
+// WIDE: the packed uint8 kernel keeps uint32 totals beside its 16-bit lanes only when the reduction
+// is longer than 256 rows (direct dedispersion); other code paths ignore the flag (normalised to 0).
+int wide_flag(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    return (code_kind(k) == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) ? 1 : 0;
+}
+std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     char b[160];
-    std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(code_kind(k)), c.samples_per_thread,
-                  c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, c.threads_t * c.threads_dm);
+    if (code_kind(k) == CK_DEDISP_U8 || code_kind(k) == CK_DEDISP_U32)
+        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(code_kind(k)), c.samples_per_thread,
+                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, c.threads_t * c.threads_dm, wide_flag(p, k, c));
+    else
+        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(code_kind(k)), c.samples_per_thread,
+                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, c.threads_t * c.threads_dm);
     return b;
 }
-std::string define_line(ddp_kernel k, const ddp_kcfg& c, const std::string& name) {
+std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, const std::string& name) {
     char b[320];
     const int maxt = c.threads_t * c.threads_dm;
     switch (code_kind(k)) {
         case CK_DEDISP_U8:
-            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u8, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
-                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt);
+            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u8, %d, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
+                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt, wide_flag(p, k, c));
             break;
         case CK_DEDISP_U32:
-            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u32, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
+            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u32, %d, %d, %d, %d, %d, %d, 0)\n", name.c_str(),
                           c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt);
             break;
         case CK_INTEG:
@@ -332,7 +341,7 @@ std::string lib_dir() {
 
 // Registry entry with a device image (or a failure record); no CUDA context needed.
 DdpCompiled* obtain_image(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
-    const std::string name = kernel_name(k, c);
+    const std::string name = kernel_name(p, k, c);
     {
         std::lock_guard<std::mutex> lk(g_reg_mu);
         auto it = g_reg.find(name);
@@ -344,7 +353,7 @@ DdpCompiled* obtain_image(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const std::string path = p->cache_dir.empty() ? std::string() : p->cache_dir + "/" + name + ".cubin";
     if (!path.empty()) have = read_file(path, K->cubin);
     if (!have) {
-        have = nvrtc_compile(name, define_line(k, c, name), K->cubin, K->log);
+        have = nvrtc_compile(name, define_line(p, k, c, name), K->cubin, K->log);
         if (have && !path.empty()) write_file_atomic(path, K->cubin);
     }
     K->failed = !have;
@@ -410,7 +419,7 @@ DdpCompiled* obtain_aot(const std::string& name) {
 
 // Ready-to-launch kernel of configuration c (context current).
 ddp_status get_kernel(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, DdpCompiled** out) {
-    const std::string name = kernel_name(k, c);
+    const std::string name = kernel_name(p, k, c);
     DdpCompiled* K = nullptr;
     {
         std::lock_guard<std::mutex> lk(g_reg_mu);
@@ -441,7 +450,7 @@ void ddp_rt_precompile(const ddp_plan* p, const std::vector<std::pair<ddp_kernel
         std::lock_guard<std::mutex> lk(g_reg_mu);
         std::unordered_map<std::string, int> seen;
         for (const auto& e : list) {
-            const std::string name = kernel_name(e.first, e.second);
+            const std::string name = kernel_name(p, e.first, e.second);
             if (g_reg.count(name) || seen.count(name)) continue;
             seen[name] = 1;
             todo.push_back(e);
@@ -630,6 +639,7 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
             break;
     }
     q.win = c.staging ? ddp_dedisp_win(p, k, c) : 0;
+    q.one = 1;
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     return launch(p, K, cdiv(q.ns, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,
