@@ -312,19 +312,32 @@ __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
 // offsets are computed once per chunk by one thread each (table `offs`), from the tile's delays
 // kept in shared memory per superchunk of 64 channels (`dls`).  Copies, offsets and delays are
 // double buffered: chunk c+1 is staged while chunk c is summed, one __syncthreads per chunk.
-template <int VW>
+template <int VW, bool GLOBAL>
 __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst, int cstride) {
     ddp_u32 w[VW + 1];
-    if constexpr (VW == 4) {
-        const uint4 v = *(const uint4*)src;
-        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
-    } else if constexpr (VW == 2) {
-        const uint2 v = *(const uint2*)src;
-        w[0] = v.x; w[1] = v.y;
+    if constexpr (GLOBAL) {  // read-only global data: LDG through the non-coherent path
+        if constexpr (VW == 4) {
+            const uint4 v = __ldg((const uint4*)src);
+            w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+        } else if constexpr (VW == 2) {
+            const uint2 v = __ldg((const uint2*)src);
+            w[0] = v.x; w[1] = v.y;
+        } else {
+            w[0] = __ldg(src);
+        }
+        w[VW] = __ldg(src + VW);
     } else {
-        w[0] = src[0];
+        if constexpr (VW == 4) {
+            const uint4 v = *(const uint4*)src;
+            w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+        } else if constexpr (VW == 2) {
+            const uint2 v = *(const uint2*)src;
+            w[0] = v.x; w[1] = v.y;
+        } else {
+            w[0] = src[0];
+        }
+        w[VW] = src[VW];
     }
-    w[VW] = src[VW];
 #pragma unroll
     for (int o = 0; o < 4; ++o) {
         ddp_u32 x[VW];
@@ -400,24 +413,24 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_bulk_g2s(dst + (size_t)u * (win + 16), in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0s[u],
                              (ddp_u32)lens[u] * 4u + 16u, &mbar[c & 1]);
     };
-    // chunk c -> the four shifted copies of buffer c & 1 (source: global memory, or the raw TMA slot)
+    // chunk c -> the four shifted copies of buffer c & 1 (source: global memory, or the raw TMA slot).
+    // Each row is split over `parts` warps (a power of two), so the per-row set-up is done once per warp.
+    const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
     auto stage = [&](int c) {
         ddp_u32* cb = copies + (size_t)(c & 1) * U * 4 * winw;
-        const int upr = winw / VW;                 // load units per row
-        const int nvb = (upr + 31) >> 5;           // 32-unit blocks per row
-        for (int unit = warp; unit < U * nvb; unit += nwarps) {
-            const int u = unit / nvb, v = (unit - u * nvb) * 32 + lane;
+        for (int unit = warp; unit < (U << parts_log2); unit += nwarps) {
+            const int u = unit >> parts_log2, part = unit & ((1 << parts_log2) - 1);
             ddp_i64 a0;
             int lenw;
             row_extent(c * U + u, a0, lenw);
-            if (v * VW < lenw) {
-                const ddp_u32* src;
-                if constexpr (STAGING == 2)
-                    src = (const ddp_u32*)(raw + ((size_t)(c & 1) * U + u) * (win + 16)) + v * VW;
-                else
-                    src = (const ddp_u32*)(in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0) + v * VW;
-                ddp_shift_store<VW>(src, cb + (size_t)u * 4 * winw + v * VW, winw);
-            }
+            const ddp_u32* src;
+            if constexpr (STAGING == 2)
+                src = (const ddp_u32*)(raw + ((size_t)(c & 1) * U + u) * (win + 16));
+            else
+                src = (const ddp_u32*)(in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0);
+            ddp_u32* dst = cb + (size_t)u * 4 * winw;
+            for (int v = ((part << 5) + lane) * VW; v < lenw; v += (32 << parts_log2) * VW)
+                ddp_shift_store<VW, STAGING == 1>(src + v, dst + v, winw);
         }
     };
     auto prep_offs = [&](int c) {
@@ -444,6 +457,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
             if constexpr (WIDE) tot[j][k][0] = tot[j][k][1] = tot[j][k][2] = tot[j][k][3] = 0u;
         }
     const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
+    const ddp_u32* lanep = (const ddp_u32*)ddp_smem + wb;
 
     if constexpr (STAGING == 2) {
         if (tid == 0) {
@@ -481,7 +495,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         for (int j = 0; j < DPT; ++j) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const ddp_u32* wp = (const ddp_u32*)(ddp_smem + ob[j * U + u]) + wb;
+                const ddp_u32* wp = (const ddp_u32*)((const unsigned char*)lanep + ob[j * U + u]);
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 w = wp[32 * k];

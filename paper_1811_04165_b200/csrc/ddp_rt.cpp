@@ -294,7 +294,11 @@ void write_file_atomic(const std::string& path, const std::vector<char>& data) {
 }
 
 // NVRTC: template text + one DDP_DEFINE_* line -> sm_100a cubin.  Host only, thread safe.
-bool nvrtc_compile(const std::string& name, const std::string& define, std::vector<char>& cubin, std::string& log) {
+// With DDP_KEEP_SOURCE=1 in the environment and a cache directory, the generated translation unit is
+// also written to <cache_dir>/<name>.cu and compiled under that path, so that profilers (ncu
+// --import-source) can map SASS back to the template text.
+bool nvrtc_compile(const std::string& name, const std::string& define, const std::string& cache_dir,
+                   std::vector<char>& cubin, std::string& log) {
     {
         std::lock_guard<std::mutex> lk(g_api_mu);
         if (!load_nvrtc_locked()) {
@@ -303,8 +307,14 @@ bool nvrtc_compile(const std::string& name, const std::string& define, std::vect
         }
     }
     const std::string src = std::string(ddp_kernel_source) + define;
+    std::string unit = name + ".cu";
+    const char* keep = std::getenv("DDP_KEEP_SOURCE");
+    if (keep && keep[0] == '1' && !cache_dir.empty()) {
+        unit = cache_dir + "/" + unit;
+        write_file_atomic(unit, std::vector<char>(src.begin(), src.end()));
+    }
     nvrtcProgram prog = nullptr;
-    nvrtcResult r = g_api.p_nvrtcCreateProgram(&prog, src.c_str(), (name + ".cu").c_str(), 0, nullptr, nullptr);
+    nvrtcResult r = g_api.p_nvrtcCreateProgram(&prog, src.c_str(), unit.c_str(), 0, nullptr, nullptr);
     if (r != NVRTC_SUCCESS) {
         log = std::string("nvrtcCreateProgram: ") + g_api.p_nvrtcGetErrorString(r);
         return false;
@@ -339,6 +349,18 @@ std::string lib_dir() {
     return ".";
 }
 
+// Disk-cache tag: FNV-1a of the template text, so that cubins of an older template are never reused.
+const std::string& source_tag() {
+    static const std::string tag = [] {
+        uint64_t h = 1469598103934665603ull;
+        for (const char* c = ddp_kernel_source; *c; ++c) h = (h ^ (unsigned char)*c) * 1099511628211ull;
+        char b[24];
+        std::snprintf(b, sizeof b, "%016llx", (unsigned long long)h);
+        return std::string(b);
+    }();
+    return tag;
+}
+
 // Registry entry with a device image (or a failure record); no CUDA context needed.
 DdpCompiled* obtain_image(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const std::string name = kernel_name(p, k, c);
@@ -350,10 +372,10 @@ DdpCompiled* obtain_image(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     DdpCompiled* K = new DdpCompiled();
     K->name = name;
     bool have = false;
-    const std::string path = p->cache_dir.empty() ? std::string() : p->cache_dir + "/" + name + ".cubin";
+    const std::string path = p->cache_dir.empty() ? std::string() : p->cache_dir + "/" + name + "." + source_tag() + ".cubin";
     if (!path.empty()) have = read_file(path, K->cubin);
     if (!have) {
-        have = nvrtc_compile(name, define_line(p, k, c, name), K->cubin, K->log);
+        have = nvrtc_compile(name, define_line(p, k, c, name), p->cache_dir, K->cubin, K->log);
         if (have && !path.empty()) write_file_atomic(path, K->cubin);
     }
     K->failed = !have;
