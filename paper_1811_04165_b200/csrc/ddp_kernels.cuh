@@ -396,22 +396,20 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         ddp_i64 l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
         lenw = (int)(l < winw ? (l < 0 ? 0 : l) : winw);
     };
-    auto tma_issue = [&](int c) {  // one thread: raw windows of chunk c -> raw slot c & 1
+    auto tma_issue = [&](int c) {  // warp 0, lane u < U: raw window of row u of chunk c -> raw slot c & 1
         unsigned char* dst = raw + (size_t)(c & 1) * U * (win + 16);
-        ddp_i64 a0s[U];
-        int lens[U];
-        ddp_u32 total = 0;
+        ddp_i64 a0 = 0;
+        int lenw = 0;
+        if (lane < U) row_extent(c * U + lane, a0, lenw);
+        const ddp_u32 bytes = lenw > 0 ? (ddp_u32)lenw * 4u + 16u : 0u;
+        ddp_u32 total = bytes;
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            row_extent(c * U + u, a0s[u], lens[u]);
-            if (lens[u] > 0) total += (ddp_u32)lens[u] * 4u + 16u;
-        }
-        ddp_mbar_expect_tx(&mbar[c & 1], total);
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (lens[u] > 0)
-                ddp_bulk_g2s(dst + (size_t)u * (win + 16), in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0s[u],
-                             (ddp_u32)lens[u] * 4u + 16u, &mbar[c & 1]);
+        for (int d = 16; d >= 1; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
+        if (lane == 0) ddp_mbar_expect_tx(&mbar[c & 1], total);
+        __syncwarp();
+        if (bytes)
+            ddp_bulk_g2s(dst + (size_t)lane * (win + 16), in_g + (ddp_i64)(c * U + lane) * p.in_row_stride + a0, bytes,
+                         &mbar[c & 1]);
     };
     // chunk c -> the four shifted copies of buffer c & 1 (source: global memory, or the raw TMA slot).
     // Each row is split over `parts` warps (a power of two), so the per-row set-up is done once per warp.
@@ -469,7 +467,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     load_dls(0);
     __syncthreads();
     if constexpr (STAGING == 2) {
-        if (tid == 0) {
+        if (warp == 0) {
             tma_issue(0);
             if (nchunks > 1) tma_issue(1);
         }
@@ -484,7 +482,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         if (r0 % SC == 0 && r0 + SC < p.nred) load_dls(r0 / SC + 1);
         if (c + 1 < nchunks) {
             if constexpr (STAGING == 2) {
-                if (tid == 0 && c + 2 < nchunks) tma_issue(c + 2);  // slot c & 1 was converted during iteration c - 1
+                if (warp == 0 && c + 2 < nchunks) tma_issue(c + 2);  // slot c & 1 was converted during iteration c - 1
                 ddp_mbar_wait(&mbar[(c + 1) & 1], (ddp_u32)(((c + 1) >> 1) & 1));
             }
             stage(c + 1);
