@@ -227,6 +227,8 @@ typedef struct {
     int64_t max_evals_per_kernel; /* 0 = every valid configuration; else an evenly strided subset     */
     int isolated;                 /* 0: candidate timed inside the whole pipeline (other kernels at the
                                      plan's current configuration); 1: the kernel under test alone     */
+    unsigned slots;               /* bit s set: search pipeline slot s (0 = all slots); slots left out
+                                     keep the plan's current configuration (resumable campaigns)        */
 } ddp_bf_params;
 typedef struct { uint64_t seed; int64_t max_evals; } ddp_rand_params;
 

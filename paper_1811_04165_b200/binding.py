@@ -90,7 +90,7 @@ class GaParams(C.Structure):
 
 
 class BfParams(C.Structure):
-    _fields_ = [("max_evals_per_kernel", C.c_int64), ("isolated", C.c_int)]
+    _fields_ = [("max_evals_per_kernel", C.c_int64), ("isolated", C.c_int), ("slots", C.c_uint)]
 
 
 class RandParams(C.Structure):
@@ -302,8 +302,8 @@ class Plan:
         self._check(lib().ddp_tune_ga(self._h, C.byref(io), C.byref(gp), C.byref(res)), "ddp_tune_ga")
         return self._pack(res, hist)
 
-    def tune_bruteforce(self, io: TuneIo, max_evals_per_kernel=0, isolated=0, history_cap=1 << 18) -> dict:
-        bp = BfParams(max_evals_per_kernel, isolated)
+    def tune_bruteforce(self, io: TuneIo, max_evals_per_kernel=0, isolated=0, slots=0, history_cap=1 << 18) -> dict:
+        bp = BfParams(max_evals_per_kernel, isolated, slots)
         res, hist = self._result(history_cap)
         self._check(lib().ddp_tune_bruteforce(self._h, C.byref(io), C.byref(bp), C.byref(res)),
                     "ddp_tune_bruteforce")

@@ -1,0 +1,208 @@
+"""Auto-tuning campaign driver (BASELINE.json configs[4]; section 3-4).
+
+    python -m paper_1811_04165_b200.campaign --workload cfg2 --stage ga random bf final \
+        --seeds 1 2 3 4 5 --out gpurun_out/campaign_cfg2.json
+
+Runs the three tuners of the C-ABI library on one workload's device buffers and records, per run,
+the best joint configuration, its fitness (median over 5 passes of the summed CUDA-event times of
+the pipeline's kernels -- P:189), the best-so-far curve against the number of evaluations
+(P:225 / Fig. 3 in the paper), and the evaluation / kernel-timing / compile counts:
+
+  ga      ddp_tune_ga, population 64, 50 generations, tournament 3, uniform crossover 0.8 per
+          kernel, mutation 0.05 per gene, elitism 2, repair to nearest valid     (BJ:cfg4)
+  random  ddp_tune_random with the evaluation budget its GA twin consumed
+  bf      ddp_tune_bruteforce, every valid configuration of every kernel
+  final   every finalist (BF winners, each GA / random best) re-timed with ddp_time_pipeline in
+          interleaved rounds, so that the comparison does not depend on clock drift between runs
+
+The report is rewritten after every run, so an interrupted campaign keeps what it measured.  This
+file only marshals arguments and stores numbers: tuners, timing harness and kernels are all behind
+the C ABI.  Inputs are the seeded synthetic filterbank of the workload (synth/, data only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _cfgs_to_lists(cfgs):
+    return [list(c.astuple()) for c in cfgs]
+
+
+def _load(path):
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh)
+    return {}
+
+
+def _store(path, report):
+    tmp = path + ".tmp"
+    with open(tmp, "w") as fh:
+        json.dump(report, fh)
+    os.replace(tmp, path)
+
+
+def _run_record(res, **extra):
+    rec = {"best": _cfgs_to_lists(res["best"]), "best_ms": res["best_ms"], "kernel_ms": res["kernel_ms"],
+           "n_fitness_calls": res["n_fitness_calls"], "n_kernel_timings": res["n_kernel_timings"],
+           "n_compiles": res["n_compiles"], "wall_seconds": res["wall_seconds"], "history": res["history"],
+           "sum_isolated_min_ms": res["sum_isolated_min_ms"]}
+    rec.update(extra)
+    return rec
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--stage", nargs="+", default=["ga", "random", "bf", "final"],
+                    choices=["ga", "random", "bf", "final"])
+    ap.add_argument("--seeds", nargs="+", type=int, default=[1, 2, 3, 4, 5])
+    ap.add_argument("--out", default="gpurun_out/campaign.json")
+    ap.add_argument("--population", type=int, default=64)
+    ap.add_argument("--generations", type=int, default=50)
+    ap.add_argument("--tournament", type=int, default=3)
+    ap.add_argument("--p-cross", type=float, default=0.8)
+    ap.add_argument("--p-mut", type=float, default=0.05)
+    ap.add_argument("--elitism", type=int, default=2)
+    ap.add_argument("--crossover-kind", type=int, default=0)
+    ap.add_argument("--mutation-kind", type=int, default=0)
+    ap.add_argument("--replacement", type=int, default=0)
+    ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--cutoff", type=float, default=3.0,
+                    help="abandon an evaluation whose first timed pass exceeds cutoff x best-so-far (0 = never)")
+    ap.add_argument("--bf-max-per-kernel", type=int, default=0, help="0 = exhaustive")
+    ap.add_argument("--bf-isolated", type=int, default=0)
+    ap.add_argument("--bf-slots", nargs="+", type=int, default=None, help="pipeline slots to search (default all)")
+    ap.add_argument("--final-rounds", type=int, default=3)
+    args = ap.parse_args(argv)
+
+    import torch
+    import paper_1811_04165_b200 as ddp
+    from synth import configs, filterbank
+
+    if not torch.cuda.is_available():
+        raise SystemExit("campaign: no CUDA device -- the tuners' hardware harness has no CPU fallback")
+    cfg = configs.ALL[args.workload]()
+    plan = ddp.plan_from_config(cfg)
+    info = plan.query()
+    buf = ddp.alloc_buffers(plan, "cuda:0")
+    X, _ = filterbank.make_filterbank(cfg, int(info.nsamp_in_required), int(info.in_stride_min))
+    buf["d_in"].copy_(torch.from_numpy(X))
+    torch.cuda.synchronize()
+    io = ddp.make_tune_io(buf["d_in"], buf["d_out"], buf["d_integ"], buf["d_snr"], buf["d_argmax"],
+                          reps=args.reps, warmup=1, cutoff_factor=args.cutoff)
+    slots = [s for s in range(ddp.DDP_NSLOTS) if not (s == 1 and not info.subband)]
+    slot_kernel = {0: ddp.K_SUB1 if info.subband else ddp.K_DIRECT, 1: ddp.K_SUB2, 2: ddp.K_INTEGRATE, 3: ddp.K_SNR}
+    defaults = [plan.get_kcfg(slot_kernel[s]) if s in slots else plan.get_kcfg(ddp.K_INTEGRATE) for s in range(4)]
+
+    def reset_defaults():
+        for s in slots:
+            plan.set_kcfg(slot_kernel[s], defaults[s])
+
+    os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
+    report = _load(args.out)
+    report.setdefault("workload", cfg.name)
+    report["gpu"] = torch.cuda.get_device_name(0)
+    report["host_cores"] = os.cpu_count()
+    report["space"] = {ddp.KERNEL_NAMES[slot_kernel[s]]: len(plan.enumerate_kcfgs(slot_kernel[s])) for s in slots}
+    report["ga_params"] = {"population": args.population, "generations": args.generations,
+                           "tournament": args.tournament, "p_cross": args.p_cross, "p_mut": args.p_mut,
+                           "elitism": args.elitism, "crossover_kind": args.crossover_kind,
+                           "mutation_kind": args.mutation_kind, "replacement": args.replacement,
+                           "reps": args.reps, "cutoff_factor": args.cutoff}
+    report["defaults"] = {ddp.KERNEL_NAMES[slot_kernel[s]]: list(defaults[s].astuple()) for s in slots}
+    ms, per = plan.time_pipeline(io, defaults)
+    report["defaults_ms"] = {"total": ms, "per_slot": per}
+    _store(args.out, report)
+    print("campaign %s on %s: defaults %.4f ms %s" % (cfg.name, report["gpu"], ms, per), flush=True)
+
+    if "ga" in args.stage:
+        for seed in args.seeds:
+            reset_defaults()
+            t0 = time.time()
+            res = plan.tune_ga(io, seed=seed, population=args.population, generations=args.generations,
+                               tournament=args.tournament, p_cross=args.p_cross, crossover_kind=args.crossover_kind,
+                               p_mut=args.p_mut, mutation_kind=args.mutation_kind, elitism=args.elitism,
+                               replacement=args.replacement)
+            report.setdefault("ga", {})[str(seed)] = _run_record(res, seed=seed)
+            _store(args.out, report)
+            print("ga seed %d: best %.4f ms after %d evaluations (%d compiles, %.0f s)" % (
+                seed, res["best_ms"], res["n_fitness_calls"], res["n_compiles"], time.time() - t0), flush=True)
+
+    if "random" in args.stage:
+        for seed in args.seeds:
+            reset_defaults()
+            twin = report.get("ga", {}).get(str(seed))
+            budget = twin["n_fitness_calls"] if twin else args.population + args.generations * (args.population - args.elitism)
+            t0 = time.time()
+            res = plan.tune_random(io, seed=seed, max_evals=budget)
+            report.setdefault("random", {})[str(seed)] = _run_record(res, seed=seed, budget=budget)
+            _store(args.out, report)
+            print("random seed %d: best %.4f ms after %d evaluations (%d compiles, %.0f s)" % (
+                seed, res["best_ms"], res["n_fitness_calls"], res["n_compiles"], time.time() - t0), flush=True)
+
+    if "bf" in args.stage:
+        todo = args.bf_slots if args.bf_slots is not None else slots
+        bf = report.setdefault("bf", {"winners": {}, "per_slot": {}})
+        for s in todo:
+            reset_defaults()
+            t0 = time.time()
+            res = plan.tune_bruteforce(io, max_evals_per_kernel=args.bf_max_per_kernel, isolated=args.bf_isolated,
+                                       slots=1 << s)
+            name = ddp.KERNEL_NAMES[slot_kernel[s]]
+            bf["winners"][name] = list(res["best"][s].astuple())
+            h = res["history"]
+            bf["per_slot"][name] = {"n_fitness_calls": res["n_fitness_calls"], "n_kernel_timings": res["n_kernel_timings"],
+                                    "n_compiles": res["n_compiles"], "wall_seconds": res["wall_seconds"],
+                                    "kernel_min_ms": res["sum_isolated_min_ms"],
+                                    "history_every_64": h[::64] + h[-1:], "exhaustive": args.bf_max_per_kernel == 0}
+            _store(args.out, report)
+            print("bf %s: min %.4f ms over %d configurations (%d compiles, %.0f s)" % (
+                name, res["sum_isolated_min_ms"], res["n_fitness_calls"], res["n_compiles"], time.time() - t0), flush=True)
+        if all(ddp.KERNEL_NAMES[slot_kernel[s]] in bf["winners"] for s in slots):
+            bf["n_fitness_calls"] = sum(v["n_fitness_calls"] for v in bf["per_slot"].values())
+            bf["sum_isolated_min_ms"] = sum(v["kernel_min_ms"] for v in bf["per_slot"].values())
+            _store(args.out, report)
+
+    if "final" in args.stage:
+        finalists = {"defaults": defaults}
+        bf = report.get("bf", {})
+        if bf and all(ddp.KERNEL_NAMES[slot_kernel[s]] in bf.get("winners", {}) for s in slots):
+            finalists["bf"] = [ddp.Kcfg(*bf["winners"][ddp.KERNEL_NAMES[slot_kernel[s]]]) if s in slots else defaults[s]
+                               for s in range(4)]
+        for kind in ("ga", "random"):
+            for seed, rec in report.get(kind, {}).items():
+                finalists["%s_%s" % (kind, seed)] = [ddp.Kcfg(*g) for g in rec["best"]]
+        io_final = ddp.make_tune_io(buf["d_in"], buf["d_out"], buf["d_integ"], buf["d_snr"], buf["d_argmax"],
+                                    reps=args.reps, warmup=1, cutoff_factor=0.0)
+        samples = {k: [] for k in finalists}
+        persl = {}
+        for _ in range(args.final_rounds):
+            for k, c in finalists.items():
+                ms, per = plan.time_pipeline(io_final, c)
+                samples[k].append(ms)
+                persl[k] = per
+        final = {k: {"ms": sorted(v)[len(v) // 2], "samples": v, "per_slot": persl[k],
+                     "cfg": _cfgs_to_lists(finalists[k])} for k, v in samples.items()}
+        report["final"] = final
+        best = min((k for k in final if k != "defaults"), key=lambda k: final[k]["ms"], default=None)
+        if best is not None:
+            report["tuned"] = {ddp.KERNEL_NAMES[slot_kernel[s]]: final[best]["cfg"][s] for s in slots}
+            report["tuned_from"] = best
+        _store(args.out, report)
+        for k, v in final.items():
+            print("final %-10s %.4f ms  %s" % (k, v["ms"], v["per_slot"]), flush=True)
+    plan.destroy()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -230,19 +230,25 @@ const char* kind_tag(CodeKind ck) {
 int wide_flag(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     return (code_kind(k) == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) ? 1 : 0;
 }
+// threads_t x threads_dm is a launch parameter; the code shape only sees it through
+// __launch_bounds__, whose register cap is the same (255) for every block of <= 256 threads.
+int maxt_bucket(const ddp_kcfg& c) {
+    const int t = c.threads_t * c.threads_dm;
+    return t <= 256 ? 256 : t;
+}
 std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     char b[160];
     if (code_kind(k) == CK_DEDISP_U8 || code_kind(k) == CK_DEDISP_U32)
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(code_kind(k)), c.samples_per_thread,
-                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, c.threads_t * c.threads_dm, wide_flag(p, k, c));
-    else
+                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt_bucket(c), wide_flag(p, k, c));
+    else  // integrate reads `unroll` at run time (tiles per block): not part of its code shape
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(code_kind(k)), c.samples_per_thread,
-                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, c.threads_t * c.threads_dm);
+                      c.dms_per_thread, code_kind(k) == CK_INTEG ? 1 : c.unroll, c.staging, c.vec_bytes, maxt_bucket(c));
     return b;
 }
 std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, const std::string& name) {
     char b[320];
-    const int maxt = c.threads_t * c.threads_dm;
+    const int maxt = maxt_bucket(c);
     switch (code_kind(k)) {
         case CK_DEDISP_U8:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u8, %d, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
@@ -254,7 +260,7 @@ std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, cons
             break;
         case CK_INTEG:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_INTEG(%s, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
-                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt);
+                          c.samples_per_thread, c.dms_per_thread, 1, c.staging, c.vec_bytes, maxt);
             break;
         default:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_SNR(%s, %d, %d, %d, %d, %d, %d)\n", name.c_str(),

@@ -312,6 +312,7 @@ extern "C" ddp_status ddp_tune_bruteforce(ddp_plan* plan, const ddp_tune_io* io,
     for (int s = 0; s < DDP_NSLOTS; ++s) {
         const ddp_kernel k = ddp_slot_kernel(plan, s);
         if (k == DDP_K_COUNT) continue;
+        if (bp->slots != 0 && !(bp->slots & (1u << s))) continue;
         const std::vector<ddp_kcfg>& V = ddp_valid_set(plan, k);
         size_t n = V.size(), stride = 1;
         if (bp->max_evals_per_kernel > 0 && (int64_t)n > bp->max_evals_per_kernel) {
