@@ -1,0 +1,67 @@
+"""Multi-process plumbing of the bench (N > 1): one process per GPU, each searching its own beams,
+no data-path collective.  Covered here on CPU with
+the gloo backend and world_size 2: the beam partition is exact and the ranks agree on
+(max over ranks of the time, sum over ranks of the units) -- the only two numbers they exchange.
+"""
+import os
+import socket
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist  # noqa: E402
+import torch.multiprocessing as mp  # noqa: E402
+
+from paper_1811_04165_b200.shard import beam_seed, beams_of_rank, combine  # noqa: E402
+
+
+def test_beam_partition_is_exact_and_balanced():
+    for world in (1, 2, 3, 4, 8):
+        for n in (0, 1, 7, 8, 9, 64):
+            owned = [beams_of_rank(n, r, world) for r in range(world)]
+            flat = [b for o in owned for b in o]
+            assert flat == list(range(n))                      # every beam exactly once, in order
+            sizes = [len(o) for o in owned]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        beams_of_rank(4, 2, 2)
+    assert beam_seed(100, 0) == 100 and len({beam_seed(100, b) for b in range(8)}) == 8
+
+
+def test_combine_without_process_group_is_identity():
+    assert combine(3.5, 7.0) == (3.5, 7.0)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        beams = beams_of_rank(world, rank, world)             # bench: one beam per rank (weak scaling)
+        local_ms = 10.0 + 5.0 * rank                          # rank 1 is the slower one
+        local_units = 1000.0 * len(beams)
+        ms, units = combine(local_ms, local_units, torch.device("cpu"))
+        dist.barrier()
+        out[rank] = (beams, ms, units)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world_size_two_gloo_agrees_on_max_time_and_summed_units():
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+    assert out[0][0] == [0] and out[1][0] == [1]
+    for r in range(world):
+        _, ms, units = out[r]
+        assert ms == 15.0                                     # max over ranks, never wall clock of rank 0
+        assert units == 2000.0                                # whole-job units
