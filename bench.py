@@ -38,7 +38,7 @@ ALU_LANES_PER_CLK_PER_SM = 64  # alu pipe: 4 SMSP x 16 lanes/clk (rt_SMSP = 2; B
 TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"cfg1": 260067072}  # profiles/r01_cfg1.md: 91.5 MB read + 168.6 MB written
 
 
 def measured_peaks():
@@ -273,8 +273,10 @@ def run_ours(args):
         e_mid = torch.cuda.Event(enable_timing=True)
         e_mid.record()
         plan.integrate(buf["d_out"], buf["d_integ"])
+        e_int = torch.cuda.Event(enable_timing=True)
+        e_int.record()
         plan.snr(buf["d_out"], buf["d_integ"], buf["d_snr"], buf["d_argmax"])
-        return e_mid
+        return e_mid, e_int
 
     def barrier():
         torch.cuda.synchronize()
@@ -294,12 +296,14 @@ def run_ours(args):
         e0 = torch.cuda.Event(enable_timing=True)
         e1 = torch.cuda.Event(enable_timing=True)
         e0.record()
-        em = step()
+        em, ei = step()
         e1.record()
-        ev.append((e0, em, e1))
+        ev.append((e0, em, ei, e1))
     barrier()
-    step_ms = [a.elapsed_time(c) for a, _, c in ev]
-    dd_ms = [a.elapsed_time(b) for a, b, _ in ev]
+    step_ms = [a.elapsed_time(d) for a, _, _, d in ev]
+    dd_ms = [a.elapsed_time(b) for a, b, _, _ in ev]
+    int_ms = float(np.mean([b.elapsed_time(c) for _, b, c, _ in ev]))
+    snr_ms = float(np.mean([c.elapsed_time(d) for _, _, c, d in ev]))
     local_ms = float(sum(step_ms))
     tot_ms, tot_units = combine(local_ms, units_per_step * args.steps, dev)
     value = tot_units / (tot_ms * 1e-3)
@@ -348,6 +352,15 @@ def run_ours(args):
                         "peak_gbs": peaks["hbm_gbs"], "frac": hbm_bytes / (dd_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                         "peak_source": peak_src}}
 
+    # integrate / snr are HBM bound: read Y (+ planes), write planes
+    y_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
+    pl_bytes = 4.0 * float(info.ndm) * sum(float(info.plane_len[k]) for k in range(info.nwidths) if info.widths[k] > 1)
+    stages = {"dedisperse_ms": dd_avg_ms,
+              "integrate": {"ms": int_ms, "algorithmic_bytes": y_bytes + pl_bytes,
+                            "hbm_frac": (y_bytes + pl_bytes) / (int_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+              "snr": {"ms": snr_ms, "algorithmic_bytes": y_bytes + pl_bytes,
+                      "hbm_frac": (y_bytes + pl_bytes) / (snr_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
     # ---- the oracle timed beside it (rank 0, N = 1 only) + parity of the sampled rows
     cpu = None
     parity = None
@@ -381,7 +394,7 @@ def run_ours(args):
                     "h2d_bytes_per_step": int(h_in.numel()),
                     "d2h_bytes_per_step": int(h_snr.numel() * 4 + h_arg.numel() * 4)},
             "gpu_launches": int(kernels_per_step * args.steps),
-            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "parity": parity}
+            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "parity": parity}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

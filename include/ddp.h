@@ -115,7 +115,9 @@ typedef struct {
  *                       For a subband plan pass NULL (ndm is then n_coarse*n_fine and trial
  *                       a*n_fine+b has DM coarse_first + a*coarse_step + b*fine_step), or the
  *                       identical grid (checked).
- * widths[nwidths]       host, strictly increasing boxcar widths >= 1, nwidths <= DDP_MAX_WIDTHS.
+ * widths[nwidths]       host, strictly increasing boxcar widths, each a power of two (1, 2, 4, ...;
+ *                       INT.3: BJ configs; the paper's own factor list is garbled),
+ *                       nwidths <= DDP_MAX_WIDTHS.
  * nsamp_out             output samples per DM trial (> 0); floor(nsamp_out / max width) >= 2.
  * Delay tables (DD.1-DD.3): delay[i][c] = floor(((4.148808e3*DM[i]) * (f[c]^-2 - f_ref^-2)) / t_samp + 0.5)
  * in float64, f_ref = max_c f[c].  Errors: DDP_E_ARG, DDP_E_SHAPE (nchan % n_subbands),

@@ -10,10 +10,15 @@
 //
 // What is computed (P:n = PAPER.md line n; readings in DESIGN.md):
 //   dedisp   out[g][i][t] = sum_r in[g][r][t + delay[g][i][r]]            P:51, P:63, P:71 fn.4
-//   integ    I_w[i][j]    = sum_{k<w} Y[i][j*w + k], j < floor(ns/w)
+//   integ    I_w[i][j]    = sum_{k<w} Y[i][j*w + k], j < floor(ns/w), w = 2^m
 //   snr      (max - mean)/std per (DM, width), exact integer moments      P:63; BJ:cfg0
 #ifndef DDP_KERNELS_CUH_
 #define DDP_KERNELS_CUH_
+
+// How the packed dedispersion kernel accumulates its two 16-bit lane pairs (see ddp_dedisp_packed_body).
+#ifndef DDP_ACC_MODE
+#define DDP_ACC_MODE 0
+#endif
 
 typedef unsigned char ddp_u8;
 typedef unsigned int ddp_u32;
@@ -108,7 +113,11 @@ __device__ __forceinline__ void ddp_acc_window(const ddp_u8* ptr, ddp_u32 (&acc)
     }
 }
 
-// Same for uint32 elements: vector loads when the window happens to be VEC-aligned, else scalar.
+// Same for uint32 elements.  VEC >= 8: aligned VEC-byte loads from the aligned-down address, covering
+// SPT + VEC/4 elements, then one of VEC/4 statically indexed add sequences selected by the
+// misalignment -- which is the same for all threads that share a (trial, row) delay, i.e. uniform
+// over a warp whenever threads_t >= 32, so the switch does not diverge.  Callers guarantee that
+// SPT + VEC/4 elements from the aligned-down address are readable.
 template <int SPT, int VEC>
 __device__ __forceinline__ void ddp_acc_window(const ddp_u32* ptr, ddp_u32 (&acc)[SPT]) {
     constexpr int VE = VEC / 4;  // elements per vector
@@ -116,16 +125,25 @@ __device__ __forceinline__ void ddp_acc_window(const ddp_u32* ptr, ddp_u32 (&acc
 #pragma unroll
         for (int s = 0; s < SPT; ++s) acc[s] += ptr[s];
     } else {
-        if ((((ddp_u64)ptr) & (ddp_u64)(VEC - 1)) == 0) {
-            typedef typename DdpVec<VEC>::type vec_t;
-            union { vec_t v[SPT / VE]; ddp_u32 w[SPT]; } r;
+        typedef typename DdpVec<VEC>::type vec_t;
+        constexpr int NV = SPT / VE + 1;
+        const ddp_u32 mis = (ddp_u32)(((ddp_u64)ptr) >> 2) & (ddp_u32)(VE - 1);
+        const vec_t* base = (const vec_t*)(ptr - mis);
+        union { vec_t v[NV]; ddp_u32 w[NV * VE]; } r;
 #pragma unroll
-            for (int v = 0; v < SPT / VE; ++v) r.v[v] = ((const vec_t*)ptr)[v];
+        for (int v = 0; v < NV; ++v) r.v[v] = base[v];
+        if (mis == 0u) {
 #pragma unroll
             for (int s = 0; s < SPT; ++s) acc[s] += r.w[s];
+        } else if (mis == 1u) {
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) acc[s] += r.w[s + 1];
+        } else if (VE > 2 && mis == 2u) {
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) acc[s] += r.w[s + (VE > 2 ? 2 : 0)];
         } else {
 #pragma unroll
-            for (int s = 0; s < SPT; ++s) acc[s] += ptr[s];
+            for (int s = 0; s < SPT; ++s) acc[s] += r.w[s + (VE > 2 ? 3 : 0)];
         }
     }
 }
@@ -445,17 +463,68 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     };
 
-    ddp_u32 accE[DPT][K], accO[DPT][K];
-    ddp_u32 tot[WIDE ? DPT : 1][WIDE ? K : 1][4];
+    ddp_u32 accE[DPT][K];
+#if DDP_ACC_MODE == 2
+    ddp_u64 accT[DPT][K];  // exact 64-bit sum of the whole words; bytes 1,3 = (accT - accE) >> 8
+#else
+    ddp_u32 accO[DPT][K];
+#endif
 #pragma unroll
     for (int j = 0; j < DPT; ++j)
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            accE[j][k] = accO[j][k] = 0u;
-            if constexpr (WIDE) tot[j][k][0] = tot[j][k][1] = tot[j][k][2] = tot[j][k][3] = 0u;
+            accE[j][k] = 0u;
+#if DDP_ACC_MODE == 2
+            accT[j][k] = 0ull;
+#else
+            accO[j][k] = 0u;
+#endif
         }
     const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
     const ddp_u32* lanep = (const ddp_u32*)ddp_smem + wb;
+    // Unpacks the 16-bit lanes into the thread's own output words (ADD: on top of what an earlier
+    // flush left there) and clears them.  WIDE reductions flush every FL rows straight into the
+    // output tile -- it is owned by this thread alone and stays L2 resident -- instead of keeping
+    // 4 uint32 totals per word in registers, which frees them for a larger DM block per thread.
+    auto emit = [&](bool add) {
+#pragma unroll
+        for (int j = 0; j < DPT; ++j) {
+            const int dm = tile_dm + ty * DPT + j;
+            if (dm < p.ndm) {
+                ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+#if DDP_ACC_MODE == 2
+                    const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
+#else
+                    const ddp_u32 oo = accO[j][k];
+#endif
+                    ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = oo & 0xffffu, v2 = accE[j][k] >> 16, v3 = oo >> 16;
+                    const int t = tile_t + 4 * (wb + 32 * k);
+                    if (t + 3 < p.ns) {
+                        if (add) {
+                            const uint4 o = *(const uint4*)(orow + t);
+                            v0 += o.x; v1 += o.y; v2 += o.z; v3 += o.w;
+                        }
+                        *(uint4*)(orow + t) = make_uint4(v0, v1, v2, v3);
+                    } else {
+                        if (t < p.ns) orow[t] = add ? orow[t] + v0 : v0;
+                        if (t + 1 < p.ns) orow[t + 1] = add ? orow[t + 1] + v1 : v1;
+                        if (t + 2 < p.ns) orow[t + 2] = add ? orow[t + 2] + v2 : v2;
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                accE[j][k] = 0u;
+#if DDP_ACC_MODE == 2
+                accT[j][k] = 0ull;
+#else
+                accO[j][k] = 0u;
+#endif
+            }
+        }
+    };
 
     if constexpr (STAGING == 2) {
         if (tid == 0) {
@@ -498,76 +567,98 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 w = wp[32 * k];
                     const ddp_u32 e = w & 0x00ff00ffu;
+#if DDP_ACC_MODE == 0  // extraction on the alu pipe, both accumulations as IMAD on the fma pipe
                     const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
                     asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accE[j][k]) : "r"(e), "r"(one));
                     asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
+#elif DDP_ACC_MODE == 1  // plain adds (IADD3)
+                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
+                    accE[j][k] += e;
+                    accO[j][k] += o;
+#elif DDP_ACC_MODE == 3  // even lanes IADD3, odd lanes IMAD
+                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
+                    accE[j][k] += e;
+                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
+#else  // 2: one extraction only; the whole word goes into an exact 64-bit sum (IMAD.WIDE)
+                    accE[j][k] += e;
+                    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(accT[j][k]) : "r"(w), "r"(one));
+#endif
                 }
             }
         }
         if constexpr (WIDE) {
-            if ((r0 + U) % FL == 0) {
-#pragma unroll
-                for (int j = 0; j < DPT; ++j)
-#pragma unroll
-                    for (int k = 0; k < K; ++k) {
-                        tot[j][k][0] += accE[j][k] & 0xffffu;
-                        tot[j][k][1] += accO[j][k] & 0xffffu;
-                        tot[j][k][2] += accE[j][k] >> 16;
-                        tot[j][k][3] += accO[j][k] >> 16;
-                        accE[j][k] = accO[j][k] = 0u;
-                    }
-            }
+            if ((r0 + U) % FL == 0) emit(r0 + U > FL);  // block-uniform
         }
         __syncthreads();
     }
-
-#pragma unroll
-    for (int j = 0; j < DPT; ++j) {
-        const int dm = tile_dm + ty * DPT + j;
-        if (dm >= p.ndm) continue;
-        ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = accO[j][k] & 0xffffu, v2 = accE[j][k] >> 16, v3 = accO[j][k] >> 16;
-            if constexpr (WIDE) {
-                v0 += tot[j][k][0]; v1 += tot[j][k][1]; v2 += tot[j][k][2]; v3 += tot[j][k][3];
-            }
-            const int t = tile_t + 4 * (wb + 32 * k);
-            if (t + 3 < p.ns) {
-                *(uint4*)(orow + t) = make_uint4(v0, v1, v2, v3);
-            } else {
-                if (t < p.ns) orow[t] = v0;
-                if (t + 1 < p.ns) orow[t + 1] = v1;
-                if (t + 2 < p.ns) orow[t + 2] = v2;
-            }
-        }
+    if constexpr (WIDE) {
+        if (p.nred % FL != 0) emit(true);  // WIDE means nred > FL: at least one flush came before
+    } else {
+        emit(false);
     }
 }
 
 // ------------------------------------------------------------------------------------ integration
-// Tile = TT = blockDim.x*SPT consecutive samples of one row; every width divides TT (host rule).
-// Per row: SPT samples per thread (vector loads), thread-local running sums, warp inclusive scan of
-// the thread totals with shuffles, cross-warp offsets through shared memory, the tile's exclusive
-// prefix P[0..TT] written to (bank-padded) shared memory, then I_w[j] = P[(j+1)w] - P[jw] for every
-// width with coalesced stores.  Exact in uint32 because the true sums are < 2^32 (plan check).
-__device__ __forceinline__ int ddp_pad(int i) { return i + (i >> 5); }
+// Widths are powers of two (plan rule, INT.3), so the block sums form a binary tree and no prefix
+// sum is needed: a thread owns SPT consecutive samples of one row and folds them pairwise in
+// registers (widths 2..SPT), the thread totals are folded across lanes with xor shuffles (widths
+// 2*SPT .. SW*SPT, SW = lanes of one row inside a warp) and, for wider boxcars, across warps through
+// a few words of shared memory.  Every level whose width is requested (p.lvl_plane[m] >= 0 for
+// w = 2^m) is stored straight from registers: ~4 instructions per input sample instead of a
+// shared-memory round trip per output, which is what makes the kernel HBM bound.
+template <int N>
+__device__ __forceinline__ void ddp_store_run(ddp_u32* o, int idx, int len, const ddp_u32 (&v)[N]) {
+    // v[0..N) -> o[idx..idx+N), clipped to len; idx is a multiple of N and rows are 16-byte aligned
+    if (idx + N <= len) {
+        if constexpr (N >= 4) {
+#pragma unroll
+            for (int i = 0; i < N; i += 4) *(uint4*)(o + idx + i) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+        } else if constexpr (N == 2) {
+            *(uint2*)(o + idx) = make_uint2(v[0], v[1]);
+        } else {
+            o[idx] = v[0];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            if (idx + i < len) o[idx + i] = v[i];
+    }
+}
 
-template <int SPT, int DPT, int UNROLL, int STAGING, int VEC>
-__device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
+template <int SPT, int M>
+struct DdpIntegFold {  // levels M .. log2(SPT) inside one thread; x holds SPT >> (M-1) partial sums on entry
+    template <int NIN>
+    static __device__ __forceinline__ void run(const DdpIntegParams& p, const ddp_u32 (&x)[NIN], int t0, int dm, bool live,
+                                               ddp_u32& total) {
+        if constexpr (NIN == 1) {
+            total = x[0];
+        } else {
+            ddp_u32 y[NIN / 2];
+#pragma unroll
+            for (int i = 0; i < NIN / 2; ++i) y[i] = x[2 * i] + x[2 * i + 1];
+            const int k = p.lvl_plane[M];
+            if (k >= 0 && live)
+                ddp_store_run<NIN / 2>(p.out + p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k], t0 >> M, p.plane_len[k], y);
+            DdpIntegFold<SPT, M + 1>::template run<NIN / 2>(p, y, t0, dm, live, total);
+        }
+    }
+};
+
+template <int SPT, int DPT, int STAGING, int VEC>
+__device__ __forceinline__ void ddp_integ_tree_body(const DdpIntegParams& p) {
     extern __shared__ __align__(128) unsigned char ddp_smem[];
     constexpr int VE = (VEC >= 4 ? VEC : 4) / 4;  // elements per load
     constexpr int LV = VE < SPT ? VE : SPT;       // elements per load actually usable
+    constexpr int LS = SPT == 16 ? 4 : SPT == 8 ? 3 : SPT == 4 ? 2 : SPT == 2 ? 1 : 0;  // log2(SPT)
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int TT = blockDim.x * SPT;
-    const int SW = blockDim.x < 32 ? blockDim.x : 32;  // shuffle segment: a warp may span several ty rows
+    const int SW = blockDim.x < 32 ? blockDim.x : 32;  // lanes of one row inside a warp
     const int lane = tx & (SW - 1), wx = tx >> 5;
     const int nwx = (blockDim.x + 31) >> 5;
-    const int prow = (ddp_pad(TT) + 2 + 3) & ~3;  // padded prefix row length, multiple of 4 (ddp_smem_bytes)
-    ddp_u32* P = (ddp_u32*)ddp_smem + (size_t)ty * prow;
-    ddp_u32* wtot = (ddp_u32*)ddp_smem + (size_t)blockDim.y * prow + ty * 32;
-    // raw staging area (STAGING 1/2): one tile per ty
-    ddp_u32* raw = (ddp_u32*)ddp_smem + (size_t)blockDim.y * (prow + 32) + (size_t)ty * TT;
-    ddp_u64* mbar = (ddp_u64*)((ddp_u32*)ddp_smem + (size_t)blockDim.y * (prow + 32 + TT));
+    // shared: warp totals [blockDim.y][32], then the raw staging tiles (STAGING 1/2), then the mbarrier
+    ddp_u32* wtot = (ddp_u32*)ddp_smem + ty * 32;
+    ddp_u32* raw = (ddp_u32*)ddp_smem + (size_t)blockDim.y * 32 + (size_t)ty * TT;
+    ddp_u64* mbar = (ddp_u64*)((ddp_u32*)ddp_smem + (size_t)blockDim.y * (32 + TT));
     const int ns4 = (p.ns + 3) & ~3;  // rows are readable up to here (out_stride is a multiple of 4)
     ddp_u32 tma_phase = 0;
     if constexpr (STAGING == 2) {
@@ -577,6 +668,9 @@ __device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
         }
         __syncthreads();
     }
+    int lsw = 0;  // log2(SW)
+    while ((1 << lsw) < SW) ++lsw;
+    const bool cross = nwx > 1 && p.max_lvl > LS + 5;  // some width spans more than one warp
 
     for (int it = 0; it < p.tiles_per_block; ++it) {
         const int tile_t = (blockIdx.x * p.tiles_per_block + it) * TT;
@@ -595,22 +689,23 @@ __device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
                     if (LV > 1 && t + LV <= ns4) {
                         typedef typename DdpVec<LV * 4>::type vec_t;
                         union { vec_t v; ddp_u32 w[LV]; } r;
-                        r.v = *(const vec_t*)(row + t);
+                        r.v = __ldg((const vec_t*)(row + t));
 #pragma unroll
                         for (int e = 0; e < LV; ++e) x[v * LV + e] = r.w[e];
                     } else {
 #pragma unroll
-                        for (int e = 0; e < LV; ++e) x[v * LV + e] = (t + e < p.ns) ? row[t + e] : 0u;
+                        for (int e = 0; e < LV; ++e) x[v * LV + e] = (t + e < p.ns) ? __ldg(row + t + e) : 0u;
                     }
                 }
             } else {
-                // copy the raw tile (clipped to the readable row) to shared memory, then read it back
                 int len = ns4 - tile_t;
                 len = len < TT ? len : TT;
                 if constexpr (STAGING == 1) {
+                    __syncthreads();  // previous tile fully read
                     for (int i = tx * 4; i < len; i += blockDim.x * 4) *(uint4*)(raw + i) = *(const uint4*)(row + tile_t + i);
                     __syncthreads();
                 } else {
+                    __syncthreads();
                     if (tx == 0) {
                         ddp_mbar_expect_tx(mbar, (ddp_u32)(len * 4));
                         ddp_bulk_g2s(raw, row + tile_t, (ddp_u32)(len * 4), mbar);
@@ -624,39 +719,39 @@ __device__ __forceinline__ void ddp_integ_body(const DdpIntegParams& p) {
 #pragma unroll
             for (int s = 0; s < SPT; ++s)
                 if (t0 + s >= p.ns) x[s] = 0u;
-            // thread-local inclusive running sums
-#pragma unroll
-            for (int s = 1; s < SPT; ++s) x[s] += x[s - 1];
-            // warp inclusive scan of the thread totals
-            ddp_u32 incl = x[SPT - 1];
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const ddp_u32 n = __shfl_up_sync(0xffffffffu, incl, d, SW);
-                if (lane >= d) incl += n;
-            }
-            if (lane == SW - 1) wtot[wx] = incl;
-            __syncthreads();
-            ddp_u32 base = incl - x[SPT - 1];  // exclusive within the warp
-            for (int w = 0; w < wx; ++w) base += wtot[w];
-            if (tx == 0) P[0] = 0u;
-#pragma unroll
-            for (int s = 0; s < SPT; ++s) P[ddp_pad(tx * SPT + s + 1)] = base + x[s];
-            __syncthreads();
-            if (live) {
-                for (int k = 0; k < p.nplanes; ++k) {
-                    const int w = p.width[k];
-                    const int nout = TT / w;
-                    const int j0 = tile_t / w;
-                    ddp_u32* o = p.out + p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + j0;
-                    const int nvalid = p.plane_len[k] - j0;
-                    for (int jj = tx; jj < nout && jj < nvalid; jj += blockDim.x)
-                        o[jj] = P[ddp_pad((jj + 1) * w)] - P[ddp_pad(jj * w)];
+            // widths 2 .. SPT in registers
+            ddp_u32 v;
+            DdpIntegFold<SPT, 1>::template run<SPT>(p, x, t0, dm, live, v);
+            // widths 2*SPT .. SW*SPT across the lanes of the row
+            for (int l = 1; l <= lsw; ++l) {
+                v += __shfl_xor_sync(0xffffffffu, v, 1 << (l - 1));
+                const int m = LS + l;
+                const int k = p.lvl_plane[m];
+                if (k >= 0 && live && (lane & ((1 << l) - 1)) == 0) {
+                    const int idx = t0 >> m;
+                    if (idx < p.plane_len[k]) p.out[p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + idx] = v;
                 }
             }
-            __syncthreads();
+            // wider boxcars: warp totals through shared memory
+            if (cross) {
+                __syncthreads();
+                if (lane == 0) wtot[wx] = v;
+                __syncthreads();
+                if (live && tx < nwx) {
+                    for (int l = 1; (1 << l) <= nwx; ++l) {
+                        const int m = LS + 5 + l;
+                        const int k = p.lvl_plane[m];
+                        if (k >= 0 && (tx & ((1 << l) - 1)) == 0) {
+                            ddp_u32 sum = 0u;
+                            for (int q = 0; q < (1 << l); ++q) sum += wtot[tx + q];
+                            const int idx = (tile_t + tx * 32 * SPT) >> m;
+                            if (idx < p.plane_len[k]) p.out[p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + idx] = sum;
+                        }
+                    }
+                }
+            }
         }
     }
-    (void)nwx;
 }
 
 // ------------------------------------------------------------------------------------ S/N
@@ -718,25 +813,38 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
         m.s1 = 0; m.s2 = 0; m.mx = 0; m.ix = 0xffffffffu;
         const int nchunks = (n + CH - 1) / CH;
         if constexpr (STAGING == 0) {
+            // Whole chunks: all of a thread's loads are issued before any is consumed (SPT/LV vector
+            // loads in flight per thread); sums per value, but max / argmax per chunk -- the index is
+            // only resolved when the chunk raises the thread's maximum (rare after the first chunks).
+            const int nfull = n / CH;
 #pragma unroll UNROLL
-            for (int c = 0; c < nchunks; ++c) {
+            for (int c = 0; c < nfull; ++c) {
                 const int t0 = c * CH + tx * SPT;
+                ddp_u32 x[SPT];
 #pragma unroll
                 for (int v = 0; v < SPT / LV; ++v) {
-                    const int t = t0 + v * LV;
-                    if (LV > 1 && t + LV <= n) {
-                        typedef typename DdpVec<LV * 4>::type vec_t;
-                        union { vec_t v; ddp_u32 w[LV]; } r;
-                        r.v = *(const vec_t*)(row + t);
+                    typedef typename DdpVec<LV * 4>::type vec_t;
+                    union { vec_t v; ddp_u32 w[LV]; } r;
+                    r.v = __ldg((const vec_t*)(row + t0 + v * LV));
 #pragma unroll
-                        for (int e = 0; e < LV; ++e) ddp_mom_add(m, r.w[e], (ddp_u32)(t + e));
-                    } else {
+                    for (int e = 0; e < LV; ++e) x[v * LV + e] = r.w[e];
+                }
+                ddp_u32 cm = x[0];
 #pragma unroll
-                        for (int e = 0; e < LV; ++e)
-                            if (t + e < n) ddp_mom_add(m, row[t + e], (ddp_u32)(t + e));
-                    }
+                for (int e = 0; e < SPT; ++e) {
+                    m.s1 += x[e];
+                    m.s2 += (ddp_u64)x[e] * (ddp_u64)x[e];
+                    if (e) cm = x[e] > cm ? x[e] : cm;
+                }
+                if (cm > m.mx) {  // strict: indices are visited in increasing order per thread
+                    m.mx = cm;
+#pragma unroll
+                    for (int e = SPT - 1; e >= 0; --e)
+                        if (x[e] == cm) m.ix = (ddp_u32)(t0 + e);
                 }
             }
+            for (int t = nfull * CH + tx * SPT, e = 0; e < SPT; ++e)  // ragged last chunk
+                if (t + e < n) ddp_mom_add(m, __ldg(row + t + e), (ddp_u32)(t + e));
         } else if constexpr (STAGING == 1) {
             for (int c = 0; c < nchunks; ++c) {
                 int len = n4 - c * CH;
@@ -819,7 +927,7 @@ __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
     }
 #define DDP_DEFINE_INTEG(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpIntegParams p) {                  \
-        ddp_integ_body<SPT, DPT, UNROLL, STAGING, VEC>(p);                                             \
+        ddp_integ_tree_body<SPT, DPT, STAGING, VEC>(p);                                                \
     }
 #define DDP_DEFINE_SNR(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                  \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpSnrParams p) {                    \

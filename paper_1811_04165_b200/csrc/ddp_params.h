@@ -41,6 +41,8 @@ struct DdpIntegParams {
     int ndm;
     int ns;
     int tiles_per_block;         // consecutive time tiles one block walks (gene "unroll")
+    int max_lvl;                 // log2 of the largest width
+    int lvl_plane[DDP_MAXW];     // plane index of width 2^m, -1 if that width is not requested
 };
 
 // S/N (BJ:cfg0): series k of row i = n[k] values at base[k] + i*stride[k].

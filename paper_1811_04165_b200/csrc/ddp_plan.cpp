@@ -85,6 +85,7 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
         if (!(chan_freq_mhz[c] > 0.0) || !std::isfinite(chan_freq_mhz[c])) return DDP_E_ARG;
     for (int k = 0; k < nwidths; ++k) {
         if (widths[k] < 1) return DDP_E_ARG;
+        if ((widths[k] & (widths[k] - 1)) != 0 || widths[k] >= (1 << (DDP_MAXW - 1))) return DDP_E_ARG;  // INT.3
         if (k > 0 && widths[k] <= widths[k - 1]) return DDP_E_ARG;
     }
     if (nsamp_out / widths[nwidths - 1] < 2) return DDP_E_ARG;
@@ -302,8 +303,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             return c.staging == 1 ? row * c.unroll : 2 * row * c.unroll + 16;
         }
         case DDP_K_INTEGRATE: {
-            const int64_t prow = ((TT + (TT >> 5) + 2) + 3) & ~(int64_t)3;
-            size_t b = (size_t)c.threads_dm * (prow + 32) * 4;
+            size_t b = (size_t)c.threads_dm * 32 * 4;  // warp totals [threads_dm][32]
             if (c.staging != 0) b += (size_t)c.threads_dm * TT * 4 + 16;
             return b;
         }

@@ -325,8 +325,22 @@ bool nvrtc_compile(const std::string& name, const std::string& define, const std
         log = std::string("nvrtcCreateProgram: ") + g_api.p_nvrtcGetErrorString(r);
         return false;
     }
-    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "--device-int128"};
-    r = g_api.p_nvrtcCompileProgram(prog, 4, opts);
+    // DDP_NVRTC_DEFINES="NAME=VALUE NAME2=VALUE2": development hook for template experiments
+    std::vector<std::string> extra;
+    if (const char* d = std::getenv("DDP_NVRTC_DEFINES")) {
+        std::string all = d, cur;
+        for (char ch : all + " ") {
+            if (ch == ' ') {
+                if (!cur.empty()) extra.push_back("-D" + cur);
+                cur.clear();
+            } else {
+                cur += ch;
+            }
+        }
+    }
+    std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "--device-int128"};
+    for (const std::string& e : extra) opts.push_back(e.c_str());
+    r = g_api.p_nvrtcCompileProgram(prog, (int)opts.size(), opts.data());
     g_ncompiles.fetch_add(1);
     if (r != NVRTC_SUCCESS) {
         size_t n = 0;
@@ -360,6 +374,8 @@ const std::string& source_tag() {
     static const std::string tag = [] {
         uint64_t h = 1469598103934665603ull;
         for (const char* c = ddp_kernel_source; *c; ++c) h = (h ^ (unsigned char)*c) * 1099511628211ull;
+        if (const char* d = std::getenv("DDP_NVRTC_DEFINES"))
+            for (const char* c = d; *c; ++c) h = (h ^ (unsigned char)*c) * 1099511628211ull;
         char b[24];
         std::snprintf(b, sizeof b, "%016llx", (unsigned long long)h);
         return std::string(b);
@@ -692,6 +708,13 @@ ddp_status launch_integ(const ddp_plan* p, const ddp_kcfg& c, DdpCompiled* K, co
     }
     if (np == 0) return DDP_OK;  // only w = 1: nothing to integrate
     q.nplanes = np;
+    for (int m = 0; m < DDP_MAXW; ++m) q.lvl_plane[m] = -1;
+    for (int k = 0; k < np; ++k) {
+            int m = 0;
+            while ((1 << m) < q.width[k]) ++m;
+        q.lvl_plane[m] = k;
+        if (m > q.max_lvl) q.max_lvl = m;
+    }
     q.ndm = p->ndm;
     q.ns = p->ns;
     q.tiles_per_block = c.unroll;

@@ -162,6 +162,31 @@ def test_direct_plan_kernel_configuration_sweep(kernel):
     g.close()
 
 
+def test_integrate_and_snr_sparse_wide_widths_sweep():
+    """Widths with gaps and boxcars wider than one warp's samples (cross-warp level of the tree),
+    ragged length, every block shape family: integrate and snr against the oracle."""
+    cfg = small_direct(name="wide", nchan=32, nsamp_out=5203, ndm=19, widths=(1, 2, 8, 64, 512, 1024), n_pulses=2)
+    g = GpuSearch(cfg)
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="wide default")
+    for kernel in (ddp.K_INTEGRATE, ddp.K_SNR):
+        V = g.plan.enumerate_kcfgs(kernel)
+        picks = _sample(V, 40, seed=77 + kernel)
+        if kernel == ddp.K_INTEGRATE:  # make sure 16-lane rows and the widest blocks are in
+            picks += [c for c in V if c.threads_t == 16 and c.staging == 0][:3]
+            picks += [c for c in V if c.threads_t == 1024 and c.samples_per_thread == 1][:3]
+        for c in picks:
+            g.plan.set_kcfg(kernel, c)
+            g.buf["d_integ"].fill_(-1)
+            g.buf["d_snr"].fill_(-7.0)
+            g.buf["d_argmax"].fill_(-1)
+            g.integrate()
+            g.snr()
+            compare_all(g, Yo, what="%s %r" % (ddp.KERNEL_NAMES[kernel], c))
+    g.close()
+
+
 @pytest.mark.parametrize("kernel", [ddp.K_SUB1, ddp.K_SUB2])
 def test_subband_plan_kernel_configuration_sweep(kernel):
     cfg = small_subband(name="sweep_sb", nchan=128, nsamp_out=2100, ndm=24 * 8,

@@ -146,6 +146,7 @@ def test_plan_create_rejects_bad_arguments():
     assert status(dm_list=[-1.0, 0.0]) == binding.E_ARG
     assert status(widths=[2, 1]) == binding.E_ARG                   # not strictly increasing
     assert status(widths=[0, 1]) == binding.E_ARG
+    assert status(widths=[1, 3]) == binding.E_ARG                   # not a power of two (INT.3)
     assert status(widths=[1, 64]) == binding.E_ARG                  # floor(ns / w_max) < 2 (INT.2)
     assert status(widths=list(range(1, 18))) == binding.E_ARG       # > DDP_MAX_WIDTHS
     assert status(nsamp_out=0) == binding.E_ARG
