@@ -340,7 +340,7 @@ def run_ours(args):
     achieved = adds / (dd_avg_ms * 1e-3) / 1e12
     in_bytes = float(info.nchan) * float(info.nsamp_in_required)
     out_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
-    sub_bytes = 2.0 * info.n_coarse * info.n_subbands * float(info.nsamp_sub) * 4.0 if info.subband else 0.0
+    sub_bytes = 2.0 * info.n_coarse * info.n_subbands * float(info.nsamp_sub) * info.sub_elem_bytes if info.subband else 0.0
     hbm_bytes = in_bytes + out_bytes + sub_bytes
     roofline = {"bound": "alu", "kernel": "dedisperse (%s)" % ("sub1+sub2" if info.subband else "direct"),
                 "achieved": achieved, "peak": alu_peak, "unit": "Tadd/s", "frac": achieved / alu_peak,

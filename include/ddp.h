@@ -106,6 +106,8 @@ typedef struct {
     int64_t integ_elems;         /* uint32 elements the caller allocates for d_integ                    */
     int64_t workspace_bytes;     /* bytes the caller allocates for ddp_plan_bind_workspace              */
     double adds_dedisp;          /* algorithmic integer adds of one dedisperse call                     */
+    int sub_elem_bytes;          /* subband: bytes per element of the intermediate S: 2 (uint16) when
+                                    255 * channels-per-subband <= 65535 makes that exact, else 4 (SB.4)  */
 } ddp_plan_info;
 
 /* ---- plan -------------------------------------------------------------------------------------
@@ -167,8 +169,9 @@ ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_t in_stride
                            uint32_t* d_out, size_t out_stride, uint32_t* d_integ, float* d_snr,
                            uint32_t* d_argmax, float* h_snr, uint32_t* h_argmax, void* stream);
 /* Debug accessor: device pointer of the subband intermediate S[n_coarse][n_subbands][sub_stride]
- * inside the bound workspace (NULL for a direct plan or before bind). */
-ddp_status ddp_plan_subband_buffer(const ddp_plan* plan, uint32_t** d_sub);
+ * (elements of sub_elem_bytes bytes: uint16 or uint32) inside the bound workspace (NULL for a direct
+ * plan or before bind). */
+ddp_status ddp_plan_subband_buffer(const ddp_plan* plan, void** d_sub);
 
 /* ---- kernel configurations ----------------------------------------------------------------------
  * Validity rules V1-V7 are listed in DESIGN.md (from P:136-152 and the sm_100a limits). */

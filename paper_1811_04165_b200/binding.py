@@ -69,7 +69,8 @@ class PlanInfo(C.Structure):
                 ("nsamp_sub", C.c_int64), ("sub_stride", C.c_int64),
                 ("widths", C.c_int * DDP_MAX_WIDTHS), ("plane_len", C.c_int64 * DDP_MAX_WIDTHS),
                 ("plane_stride", C.c_int64 * DDP_MAX_WIDTHS), ("plane_offset", C.c_int64 * DDP_MAX_WIDTHS),
-                ("integ_elems", C.c_int64), ("workspace_bytes", C.c_int64), ("adds_dedisp", C.c_double)]
+                ("integ_elems", C.c_int64), ("workspace_bytes", C.c_int64), ("adds_dedisp", C.c_double),
+                ("sub_elem_bytes", C.c_int)]
 
 
 FITNESS_FN = C.CFUNCTYPE(C.c_double, C.c_void_p, C.POINTER(Kcfg))

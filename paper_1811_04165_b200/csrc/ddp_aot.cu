@@ -7,12 +7,15 @@
 
 #define DDP_AOT_U8(S, D, U, G, V, T, W) DDP_DEFINE_DEDISP(ddp_dedisp_u8_s##S##_d##D##_u##U##_g##G##_v##V##_t##T##_w##W, ddp_u8, S, D, U, G, V, T, W)
 #define DDP_AOT_U32(S, D, U, G, V, T) DDP_DEFINE_DEDISP(ddp_dedisp_u32_s##S##_d##D##_u##U##_g##G##_v##V##_t##T##_w0, ddp_u32, S, D, U, G, V, T, 0)
+#define DDP_AOT_U16(S, D, U, G, V, T, W) DDP_DEFINE_DEDISP(ddp_dedisp_u16_s##S##_d##D##_u##U##_g##G##_v##V##_t##T##_w##W, ddp_u16, S, D, U, G, V, T, W)
 #define DDP_AOT_INTEG(S, D, U, G, V, T) DDP_DEFINE_INTEG(ddp_integ_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 #define DDP_AOT_SNR(S, D, U, G, V, T) DDP_DEFINE_SNR(ddp_snr_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 
-// plan defaults (ddp_plan.cpp::default_kcfgs)
+// plan defaults (ddp_plan.cpp::default_kcfgs); W = code flags (bit 0 wide flush, bit 1 uint16 result,
+// bits 2-3 log2 lane-sum group of the packed uint16 kernel)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 1)
-DDP_AOT_U8(16, 2, 8, 1, 16, 256, 0)
+DDP_AOT_U8(16, 2, 8, 1, 16, 256, 2)
+DDP_AOT_U16(4, 8, 8, 2, 16, 256, 8)
 DDP_AOT_U32(4, 4, 4, 0, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 0, 16, 256)
 DDP_AOT_SNR(4, 1, 4, 0, 16, 256)
@@ -21,6 +24,8 @@ DDP_AOT_U8(8, 4, 8, 0, 4, 256, 0)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 0)
 DDP_AOT_U8(16, 4, 8, 2, 16, 256, 1)
 DDP_AOT_U8(16, 4, 8, 2, 16, 256, 0)
+DDP_AOT_U16(4, 4, 4, 0, 8, 256, 0)
+DDP_AOT_U16(4, 8, 8, 1, 16, 256, 8)
 DDP_AOT_U32(4, 4, 4, 1, 16, 256)
 DDP_AOT_U32(4, 4, 4, 2, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 1, 16, 256)

@@ -21,6 +21,7 @@
 #endif
 
 typedef unsigned char ddp_u8;
+typedef unsigned short ddp_u16;
 typedef unsigned int ddp_u32;
 typedef unsigned long long ddp_u64;
 typedef long long ddp_i64;
@@ -29,6 +30,12 @@ typedef long long ddp_i64;
 __device__ __forceinline__ ddp_u32 ddp_dp4a(ddp_u32 a, ddp_u32 b, ddp_u32 c) {
     ddp_u32 d;
     asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+// d = c + a.lo16 * b.byte0 + a.hi16 * b.byte1: b = 0x0001 adds the low half of a, b = 0x0100 the high half.
+__device__ __forceinline__ ddp_u32 ddp_dp2a_lo(ddp_u32 a, ddp_u32 b, ddp_u32 c) {
+    ddp_u32 d;
+    asm("dp2a.lo.u32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
 __device__ __forceinline__ ddp_u32 ddp_shf_r(ddp_u32 lo, ddp_u32 hi, ddp_u32 sh) {
@@ -148,11 +155,51 @@ __device__ __forceinline__ void ddp_acc_window(const ddp_u32* ptr, ddp_u32 (&acc
     }
 }
 
+// Same for uint16 elements (the narrow subband intermediate, SB.4): aligned VEC-byte loads from the
+// aligned-down address, word-select stages, a 16-bit funnel shift for an odd element offset, then
+// the two halves of every word are added to their accumulators.  Callers guarantee that
+// SPT*2 + VEC bytes from the aligned-down address are readable.
+template <int SPT, int VEC>
+__device__ __forceinline__ void ddp_acc_window(const ddp_u16* ptr, ddp_u32 (&acc)[SPT]) {
+    if constexpr (VEC < 4 || SPT < 2) {
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) acc[s] += (ddp_u32)ptr[s];
+    } else {
+        constexpr int NW = SPT / 2 + VEC / 4;
+        const ddp_u64 a = (ddp_u64)ptr;
+        const ddp_u32 o = (ddp_u32)(a & (ddp_u64)(VEC - 1));
+        typedef typename DdpVec<VEC>::type vec_t;
+        const vec_t* base = (const vec_t*)(a - o);
+        union { vec_t v[NW * 4 / VEC]; ddp_u32 w[NW]; } r;
+#pragma unroll
+        for (int v = 0; v < NW * 4 / VEC; ++v) r.v[v] = base[v];
+        if constexpr (VEC >= 16) {
+            if (o & 8u) {
+#pragma unroll
+                for (int k = 0; k + 2 < NW; ++k) r.w[k] = r.w[k + 2];
+            }
+        }
+        if constexpr (VEC >= 8) {
+            if (o & 4u) {
+#pragma unroll
+                for (int k = 0; k + 1 < NW; ++k) r.w[k] = r.w[k + 1];
+            }
+        }
+        const ddp_u32 sh = (o & 2u) * 8u;
+#pragma unroll
+        for (int k = 0; k < SPT / 2; ++k) {
+            const ddp_u32 w = ddp_shf_r(r.w[k], r.w[k + 1], sh);
+            acc[2 * k] += w & 0xffffu;
+            acc[2 * k + 1] += w >> 16;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------ dedispersion
 // Block = blockDim.x (time) x blockDim.y (DM) threads; tile = TT = blockDim.x*SPT samples by
 // TD = blockDim.y*DPT trials; grid = (time tiles, DM tiles, groups).  Thread (tx, ty) owns samples
 // tile_t + tx*SPT .. +SPT-1 of trials tile_dm + ty*DPT .. +DPT-1 in SPT*DPT uint32 registers.
-template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC>
+template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, bool OUT16>
 __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
     extern __shared__ __align__(128) unsigned char ddp_smem[];
     constexpr int AL = 16 / (int)sizeof(IN_T);  // elements per 16 bytes
@@ -294,11 +341,24 @@ __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
         }
     }
 
-    // Epilogue: uint32 sums, vector stores where the whole group of samples is in range.
+    // Epilogue: uint32 sums (uint16 for the narrow subband intermediate, exact by the plan's
+    // 255 * channels-per-subband <= 65535 rule), vector stores where the whole group is in range.
 #pragma unroll
     for (int j = 0; j < DPT; ++j) {
         const int dm = tile_dm + ty * DPT + j;
         if (dm >= p.ndm) continue;
+        if constexpr (OUT16) {
+            ddp_u16* o = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride + t0;
+            if (SPT >= 2 && t0 + SPT <= p.ns) {
+#pragma unroll
+                for (int s = 0; s + 1 < SPT; s += 2) *(ddp_u32*)(o + s) = acc[j][s] | (acc[j][s + 1] << 16);
+            } else {
+#pragma unroll
+                for (int s = 0; s < SPT; ++s)
+                    if (t0 + s < p.ns) o[s] = (ddp_u16)acc[j][s];
+            }
+            continue;
+        }
         ddp_u32* o = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride + t0;
         if (SPT >= 4 && t0 + SPT <= p.ns) {
 #pragma unroll
@@ -368,9 +428,10 @@ __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst
     }
 }
 
-template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE>
+template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE, bool OUT16>
 __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p) {
     static_assert(SPT >= 4 && VEC >= 4, "packed staging works on whole 4-sample words");
+    static_assert(!(WIDE && OUT16), "a uint16 result never needs the wide flush");
     extern __shared__ __align__(128) unsigned char ddp_smem[];
     constexpr int K = SPT / 4;   // words per thread
     constexpr int VW = VEC / 4;  // words per staging load
@@ -490,7 +551,27 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
 #pragma unroll
         for (int j = 0; j < DPT; ++j) {
             const int dm = tile_dm + ty * DPT + j;
-            if (dm < p.ndm) {
+            if (OUT16 && dm < p.ndm) {  // the 16-bit lanes are the result: interleave and store
+                ddp_u16* orow = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+#if DDP_ACC_MODE == 2
+                    const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
+#else
+                    const ddp_u32 oo = accO[j][k];
+#endif
+                    const ddp_u32 lo = __byte_perm(accE[j][k], oo, 0x5410u), hi = __byte_perm(accE[j][k], oo, 0x7632u);
+                    const int t = tile_t + 4 * (wb + 32 * k);
+                    if (t + 3 < p.ns) {
+                        *(uint2*)(orow + t) = make_uint2(lo, hi);
+                    } else {
+                        if (t < p.ns) orow[t] = (ddp_u16)lo;
+                        if (t + 1 < p.ns) orow[t + 1] = (ddp_u16)(lo >> 16);
+                        if (t + 2 < p.ns) orow[t + 2] = (ddp_u16)hi;
+                    }
+                }
+            }
+            if (!OUT16 && dm < p.ndm) {
                 ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
@@ -595,6 +676,215 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         if (p.nred % FL != 0) emit(true);  // WIDE means nred > FL: at least one flush came before
     } else {
         emit(false);
+    }
+}
+
+// ------------------------------------------------------------------------------------ packed staged uint16 dedispersion
+// Subband step 2 on the narrow intermediate (uint16 S, SB.4), STAGING 1 or 2.  Step 2 re-reads every
+// staged sample once per fine DM, so it is bound by shared-memory bandwidth: one LDS.32 brings TWO
+// consecutive samples of one (subband, trial) to a thread, 32 consecutive words per warp (conflict
+// free).  Each staged row exists as two copies -- copy 0 as stored, copy 1 shifted by one element --
+// so that a delayed window is word aligned in one of them whatever the delay's parity; with TMA the
+// bulk copy writes copy 0 in place and only copy 1 is made by the block.  The words of G <= 4
+// subbands are first summed as they are (two 16-bit lanes per register, exact while
+// G * 255 * channels-per-subband <= 65535: G comes from the plan), then dp2a splits the lanes into
+// the two uint32 totals of the thread's sample pair: (G loads + G-1 adds + 2 dp2a) per 2G adds.
+// Offsets of all (trial, subband) windows of the tile are tabulated once per block; the ring of
+// NB chunk buffers keeps chunk c+2 in flight (TMA) and chunk c+1 in conversion while chunk c is summed.
+template <int VW, bool GLOBAL>
+__device__ __forceinline__ void ddp_shift16_store(const ddp_u32* src, ddp_u32* dst0, ddp_u32* dst1) {
+    ddp_u32 w[VW + 1];
+    if constexpr (GLOBAL) {
+        if constexpr (VW == 4) {
+            const uint4 v = __ldg((const uint4*)src);
+            w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+        } else if constexpr (VW == 2) {
+            const uint2 v = __ldg((const uint2*)src);
+            w[0] = v.x; w[1] = v.y;
+        } else {
+            w[0] = __ldg(src);
+        }
+        w[VW] = __ldg(src + VW);
+        if constexpr (VW == 4) *(uint4*)dst0 = make_uint4(w[0], w[1], w[2], w[3]);
+        else if constexpr (VW == 2) *(uint2*)dst0 = make_uint2(w[0], w[1]);
+        else dst0[0] = w[0];
+    } else {
+        if constexpr (VW == 4) {
+            const uint4 v = *(const uint4*)src;
+            w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+        } else if constexpr (VW == 2) {
+            const uint2 v = *(const uint2*)src;
+            w[0] = v.x; w[1] = v.y;
+        } else {
+            w[0] = src[0];
+        }
+        w[VW] = src[VW];
+    }
+    ddp_u32 x[VW];
+#pragma unroll
+    for (int i = 0; i < VW; ++i) x[i] = __byte_perm(w[i], w[i + 1], 0x5432u);
+    if constexpr (VW == 4) *(uint4*)dst1 = make_uint4(x[0], x[1], x[2], x[3]);
+    else if constexpr (VW == 2) *(uint2*)dst1 = make_uint2(x[0], x[1]);
+    else dst1[0] = x[0];
+}
+
+template <int SPT, int DPT, int U, int STAGING, int VEC, int GRP>
+__device__ __forceinline__ void ddp_dedisp_packed16_body(const DdpDedispParams& p) {
+    static_assert(SPT >= 2 && VEC >= 4, "packed staging works on whole 2-sample words");
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int K = SPT / 2;               // words per thread
+    constexpr int VW = VEC / 4;              // words per staging load
+    constexpr int NB = STAGING == 2 ? 3 : 2; // chunk buffers
+    constexpr int G = GRP < U ? GRP : U;     // words summed in 16-bit lanes before the split
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int nthreads = blockDim.x * blockDim.y;
+    const int tid = ty * blockDim.x + tx;
+    const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
+    const int TT = blockDim.x * SPT, TD = blockDim.y * DPT;
+    const int g = blockIdx.z;
+    const int tile_t = blockIdx.x * TT;
+    const int tile_dm = blockIdx.y * TD;
+    const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
+    const ddp_u16* in_g = (const ddp_u16*)p.in + (ddp_i64)g * p.in_group_stride;
+    const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
+    const int winw = p.win >> 1;             // words per staged row copy (multiple of 4)
+    const int nredp = (p.nred + 3) & ~3;
+
+    // shared-memory carve-up (ddp_smem_bytes mirrors it)
+    ddp_u32* copies = (ddp_u32*)ddp_smem;                      // [NB][U][2][winw]
+    ddp_u32* offs = copies + (size_t)NB * U * 2 * winw;        // [TD][nredp]  byte offsets inside a chunk buffer
+    ddp_u64* mbar = (ddp_u64*)(offs + (size_t)TD * nredp);     // TMA: [NB]
+    const int nchunks = p.nred / U;
+
+    // staged extent of reduction row r: aligned start (elements from the row start) and words to stage
+    auto row_extent = [&](int r, ddp_i64& a0, int& lenw) {
+        const int dmin = __ldg(dl + r);
+        a0 = ((ddp_i64)tile_t + dmin) & ~(ddp_i64)7;
+        const ddp_i64 l = (p.in_row_len - a0) >> 1;
+        lenw = (int)(l < winw ? (l < 0 ? 0 : l) : winw);
+    };
+    auto tma_issue = [&](int c, int b) {  // warp 0, lane u < U: window of row u of chunk c -> copy 0 of buffer b
+        ddp_i64 a0 = 0;
+        int lenw = 0;
+        if (lane < U) row_extent(c * U + lane, a0, lenw);
+        const ddp_u32 bytes = (ddp_u32)lenw * 4u;
+        ddp_u32 total = bytes;
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
+        if (lane == 0) ddp_mbar_expect_tx(&mbar[b], total);
+        __syncwarp();
+        if (bytes)
+            ddp_bulk_g2s(copies + ((size_t)b * U + lane) * 2 * winw, in_g + (ddp_i64)(c * U + lane) * p.in_row_stride + a0,
+                         bytes, &mbar[b]);
+    };
+    // chunk c in buffer b: copy 1 from copy 0 (TMA), or both copies from global memory
+    const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
+    auto stage = [&](int c, int b) {
+        ddp_u32* cb = copies + (size_t)b * U * 2 * winw;
+        for (int unit = warp; unit < (U << parts_log2); unit += nwarps) {
+            const int u = unit >> parts_log2, part = unit & ((1 << parts_log2) - 1);
+            ddp_i64 a0;
+            int lenw;
+            row_extent(c * U + u, a0, lenw);
+            ddp_u32* d0 = cb + (size_t)u * 2 * winw;
+            const ddp_u32* src;
+            if constexpr (STAGING == 2) src = d0;
+            else src = (const ddp_u32*)(in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0);
+            for (int v = ((part << 5) + lane) * VW; v + VW < lenw; v += (32 << parts_log2) * VW)
+                ddp_shift16_store<VW, STAGING == 1>(src + v, d0 + v, d0 + winw + v);
+        }
+    };
+
+    ddp_u32 accL[DPT][K], accH[DPT][K];
+#pragma unroll
+    for (int j = 0; j < DPT; ++j)
+#pragma unroll
+        for (int k = 0; k < K; ++k) accL[j][k] = accH[j][k] = 0u;
+    const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
+
+    if constexpr (STAGING == 2) {
+        if (tid == 0) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) ddp_mbar_init(&mbar[b], 1);
+            ddp_mbar_fence_init();
+        }
+    }
+    for (int idx = tid; idx < TD * p.nred; idx += nthreads) {
+        const int j = idx / p.nred, r = idx - j * p.nred;
+        const int dmin = __ldg(dl + r);
+        const int dd = __ldg(dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride + r);
+        const int pos = (int)(((ddp_i64)tile_t + dmin) & 7) + (dd - dmin);
+        offs[j * nredp + r] = (ddp_u32)((((r % U) * 2 + (pos & 1)) * winw + (pos >> 1)) * 4);
+    }
+    __syncthreads();
+    if constexpr (STAGING == 2) {
+        if (warp == 0) {
+            tma_issue(0, 0);
+            if (nchunks > 1) tma_issue(1, 1);
+        }
+        ddp_mbar_wait(&mbar[0], 0u);
+    }
+    stage(0, 0);
+    __syncthreads();
+
+    int b = 0;        // buffer of chunk c
+    ddp_u32 use = 0;  // how many times the ring has wrapped for chunk c
+    for (int c = 0; c < nchunks; ++c) {
+        const int b1 = b + 1 < NB ? b + 1 : 0;
+        if (c + 1 < nchunks) {
+            if constexpr (STAGING == 2) {
+                const int b2 = b1 + 1 < NB ? b1 + 1 : 0;  // last read by chunk c - 1
+                if (warp == 0 && c + 2 < nchunks) tma_issue(c + 2, b2);
+                ddp_mbar_wait(&mbar[b1], (b1 == 0 ? use + 1u : use) & 1u);
+            }
+            stage(c + 1, b1);
+        }
+        const ddp_u32* ob = offs + (size_t)(ty * DPT) * nredp + c * U;
+        const unsigned char* base = (const unsigned char*)(copies + (size_t)b * U * 2 * winw + wb);
+#pragma unroll
+        for (int j = 0; j < DPT; ++j) {
+#pragma unroll
+            for (int u = 0; u < U; u += G) {
+                ddp_u32 o[G];
+                if constexpr (G == 4) {
+                    const uint4 v = *(const uint4*)(ob + j * nredp + u);
+                    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+                } else if constexpr (G == 2) {
+                    const uint2 v = *(const uint2*)(ob + j * nredp + u);
+                    o[0] = v.x; o[1] = v.y;
+                } else {
+                    o[0] = ob[j * nredp + u];
+                }
+                ddp_u32 s16[K];
+#pragma unroll
+                for (int q = 0; q < G; ++q) {
+                    const ddp_u32* wp = (const ddp_u32*)(base + o[q]);
+#pragma unroll
+                    for (int k = 0; k < K; ++k) s16[k] = q == 0 ? wp[32 * k] : s16[k] + wp[32 * k];
+                }
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    accL[j][k] = ddp_dp2a_lo(s16[k], 0x0001u, accL[j][k]);
+                    accH[j][k] = ddp_dp2a_lo(s16[k], 0x0100u, accH[j][k]);
+                }
+            }
+        }
+        __syncthreads();
+        b = b1;
+        if (b == 0) ++use;
+    }
+
+#pragma unroll
+    for (int j = 0; j < DPT; ++j) {
+        const int dm = tile_dm + ty * DPT + j;
+        if (dm >= p.ndm) continue;
+        ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const int t = tile_t + 2 * (wb + 32 * k);
+            if (t + 1 < p.ns) *(uint2*)(orow + t) = make_uint2(accL[j][k], accH[j][k]);
+            else if (t < p.ns) orow[t] = accL[j][k];
+        }
     }
 }
 
@@ -913,17 +1203,22 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
 }
 
 // ------------------------------------------------------------------------------------ entry points
-// uint8 input with staging takes the packed kernel; everything else the generic one.
-template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, bool WIDE>
+// uint8 / uint16 input with staging takes the packed kernels; everything else the generic one.
+// FLAGS: bit 0 WIDE (uint8 packed: reduction longer than 256 rows), bit 1 OUT16 (uint16 result: the
+// narrow subband intermediate), bits 2-3 log2 of the uint16 packed kernel's lane-sum group.
+template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, int FLAGS>
 __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
+    constexpr bool WIDE = (FLAGS & 1) != 0, OUT16 = (FLAGS & 2) != 0;
     if constexpr (sizeof(IN_T) == 1 && STAGING != 0)
-        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE>(p);
+        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16>(p);
+    else if constexpr (sizeof(IN_T) == 2 && STAGING != 0)
+        ddp_dedisp_packed16_body<SPT, DPT, UNROLL, STAGING, VEC, 1 << ((FLAGS >> 2) & 3)>(p);
     else
-        ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC>(p);
+        ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC, OUT16>(p);
 }
-#define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT, WIDE)                   \
+#define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT, FLAGS)                  \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpDedispParams p) {                 \
-        ddp_dedisp_entry<IN_T, SPT, DPT, UNROLL, STAGING, VEC, (WIDE) != 0>(p);                        \
+        ddp_dedisp_entry<IN_T, SPT, DPT, UNROLL, STAGING, VEC, (FLAGS)>(p);                            \
     }
 #define DDP_DEFINE_INTEG(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpIntegParams p) {                  \

@@ -178,6 +178,9 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     I.out_stride_min = round_up(nsamp_out, 4);
     I.nsamp_sub = p->subband ? (int64_t)nsamp_out + max_d2 : 0;
     I.sub_stride = p->subband ? round_up(I.nsamp_sub + 32, 32) : 0;
+    // SB.4: the intermediate is stored as uint16 whenever that is exact (255 * channels per subband
+    // fits 16 bits), which halves its HBM and shared-memory traffic; uint32 otherwise.
+    I.sub_elem_bytes = p->subband ? (255 * (int64_t)p->cps <= 65535 ? 2 : 4) : 0;
     int64_t off = 0;
     for (int k = 0; k < nwidths; ++k) {
         I.widths[k] = widths[k];
@@ -194,7 +197,7 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     I.integ_elems = off;
     int64_t tbytes = p->subband ? round_up((int64_t)p->d1.size() * 4, 256) + round_up((int64_t)p->d2.size() * 4, 256)
                                 : round_up((int64_t)p->delay.size() * 4, 256);
-    int64_t sbytes = p->subband ? round_up((int64_t)p->ncoarse * p->nsub * I.sub_stride * 4, 256) : 0;
+    int64_t sbytes = p->subband ? round_up((int64_t)p->ncoarse * p->nsub * I.sub_stride * I.sub_elem_bytes, 256) : 0;
     I.workspace_bytes = tbytes + sbytes + 256;
     I.adds_dedisp = p->subband ? (double)p->ncoarse * nchan * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
                                : (double)p->ndm * nchan * nsamp_out;
@@ -252,7 +255,7 @@ DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k) {
     switch (k) {
         case DDP_K_DIRECT: g = {p->ns, p->ndm, p->nchan, 1}; break;
         case DDP_K_SUB1: g = {(int)p->info.nsamp_sub, p->ncoarse, p->cps, 1}; break;
-        case DDP_K_SUB2: g = {p->ns, p->nfine, p->nsub, 4}; break;
+        case DDP_K_SUB2: g = {p->ns, p->nfine, p->nsub, p->info.sub_elem_bytes}; break;
         default: break;
     }
     return g;
@@ -283,6 +286,8 @@ int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     if (g.in_bytes == 1)  // packed kernel: 16-byte carry + shifted-copy tail, in bytes, multiple of 16
         return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 32, 16);
+    if (g.in_bytes == 2 && c.staging != 0)  // packed uint16 kernel: 8-element carry + 4 spare words, multiple of 8
+        return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 16, 8);
     return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 2 * AL, AL);
 }
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
@@ -299,6 +304,11 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 size_t b = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
                 if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
                 return b;
+            }
+            if (g.in_bytes == 2) {  // ddp_dedisp_packed16_body: copies [NB][U][2][win/2] words, offs [TD][nred4], mbar [NB]
+                const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
+                const size_t nb = c.staging == 2 ? 3 : 2;
+                return nb * c.unroll * 2 * row + TD * (size_t)((g.nred + 3) & ~3) * 4 + nb * 8;
             }
             return c.staging == 1 ? row * c.unroll : 2 * row * c.unroll + 16;
         }
@@ -339,6 +349,11 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
             if (c.vec_bytes < 4) return no("V5: staged uint8 input needs vec_bytes >= 4");
             if (c.threads_t < 32) return no("V1: staged uint8 input needs threads_t >= 32");
         }
+    } else if (geo.in_bytes == 2) {
+        if (c.vec_bytes < 4) return no("V5: uint16 input needs vec_bytes >= 4");
+        if (c.vec_bytes > 2 * c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread*2");
+        if (c.staging != 0 && c.threads_t < 32)  // the packed kernel gives each warp 32 consecutive 2-sample words
+            return no("V1: staged uint16 input needs threads_t >= 32");
     } else {
         if (c.vec_bytes < 4) return no("V5: uint32 input needs vec_bytes >= 4");
         if (c.vec_bytes > 4 * c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread*4");
@@ -453,7 +468,7 @@ static void default_kcfgs(ddp_plan* p) {
     const ddp_kcfg pref[DDP_K_COUNT] = {
         /* direct    */ {64, 4, 16, 4, 8, 1, 16},
         /* sub1      */ {64, 4, 16, 2, 8, 1, 16},
-        /* sub2      */ {128, 2, 4, 4, 4, 0, 16},
+        /* sub2      */ {128, 2, 4, 8, 8, 2, 16},
         /* integrate */ {256, 1, 4, 1, 1, 0, 16},
         /* snr       */ {256, 1, 4, 1, 4, 0, 16},
     };

@@ -211,24 +211,38 @@ std::atomic<int64_t> g_ncompiles{0};
 CUmodule g_aot_mod = nullptr;
 bool g_aot_tried = false;
 
-enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3 };
-CodeKind code_kind(ddp_kernel k) {
+enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3, CK_DEDISP_U16 = 4 };
+CodeKind code_kind(const ddp_plan* p, ddp_kernel k) {
     switch (k) {
         case DDP_K_DIRECT:
         case DDP_K_SUB1: return CK_DEDISP_U8;
-        case DDP_K_SUB2: return CK_DEDISP_U32;
+        case DDP_K_SUB2: return p->info.sub_elem_bytes == 2 ? CK_DEDISP_U16 : CK_DEDISP_U32;
         case DDP_K_INTEGRATE: return CK_INTEG;
         default: return CK_SNR;
     }
 }
+bool is_dedisp(CodeKind ck) { return ck == CK_DEDISP_U8 || ck == CK_DEDISP_U32 || ck == CK_DEDISP_U16; }
 const char* kind_tag(CodeKind ck) {
-    static const char* t[] = {"ddp_dedisp_u8", "ddp_dedisp_u32", "ddp_integ", "ddp_snr"};
+    static const char* t[] = {"ddp_dedisp_u8", "ddp_dedisp_u32", "ddp_integ", "ddp_snr", "ddp_dedisp_u16"};
     return t[ck];
 }
-// WIDE: the packed uint8 kernel keeps uint32 totals beside its 16-bit lanes only when the reduction
-// is longer than 256 rows (direct dedispersion); other code paths ignore the flag (normalised to 0).
-int wide_flag(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
-    return (code_kind(k) == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) ? 1 : 0;
+const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck == CK_DEDISP_U16 ? "ddp_u16" : "ddp_u32"); }
+// Code-shape flags of the dedispersion template (ddp_kernels.cuh, ddp_dedisp_entry):
+//   bit 0  WIDE   the packed uint8 kernel flushes its 16-bit lanes every 256 rows: only when the
+//                 reduction is longer than that (direct dedispersion);
+//   bit 1  OUT16  subband step 1 writes the narrow (uint16) intermediate;
+//   bits 2-3      packed uint16 kernel (step 2): log2 of how many subband words are summed in 16-bit
+//                 lanes before they are split, the largest of {1, 2, 4} that cannot overflow.
+int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    const CodeKind ck = code_kind(p, k);
+    int f = 0;
+    if (ck == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) f |= 1;
+    if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
+    if (ck == CK_DEDISP_U16 && c.staging != 0) {
+        const int64_t room = 65535 / (255 * (int64_t)p->cps);
+        f |= (room >= 4 ? 2 : (room >= 2 ? 1 : 0)) << 2;
+    }
+    return f;
 }
 // threads_t x threads_dm is a launch parameter; the code shape only sees it through
 // __launch_bounds__, whose register cap is the same (255) for every block of <= 256 threads.
@@ -238,25 +252,25 @@ int maxt_bucket(const ddp_kcfg& c) {
 }
 std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     char b[160];
-    if (code_kind(k) == CK_DEDISP_U8 || code_kind(k) == CK_DEDISP_U32)
-        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(code_kind(k)), c.samples_per_thread,
-                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt_bucket(c), wide_flag(p, k, c));
+    const CodeKind ck = code_kind(p, k);
+    if (is_dedisp(ck))
+        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(ck), c.samples_per_thread,
+                      c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt_bucket(c), code_flags(p, k, c));
     else  // integrate reads `unroll` at run time (tiles per block): not part of its code shape
-        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(code_kind(k)), c.samples_per_thread,
-                      c.dms_per_thread, code_kind(k) == CK_INTEG ? 1 : c.unroll, c.staging, c.vec_bytes, maxt_bucket(c));
+        std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(ck), c.samples_per_thread,
+                      c.dms_per_thread, ck == CK_INTEG ? 1 : c.unroll, c.staging, c.vec_bytes, maxt_bucket(c));
     return b;
 }
 std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, const std::string& name) {
     char b[320];
     const int maxt = maxt_bucket(c);
-    switch (code_kind(k)) {
+    const CodeKind ck = code_kind(p, k);
+    switch (ck) {
         case CK_DEDISP_U8:
-            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u8, %d, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
-                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt, wide_flag(p, k, c));
-            break;
+        case CK_DEDISP_U16:
         case CK_DEDISP_U32:
-            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, ddp_u32, %d, %d, %d, %d, %d, %d, 0)\n", name.c_str(),
-                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt);
+            std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, %s, %d, %d, %d, %d, %d, %d, %d)\n", name.c_str(), kind_type(ck),
+                          c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt, code_flags(p, k, c));
             break;
         case CK_INTEG:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_INTEG(%s, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
@@ -585,9 +599,9 @@ extern "C" ddp_status ddp_plan_bind_workspace(ddp_plan* plan, void* d_workspace,
     return DDP_OK;
 }
 
-extern "C" ddp_status ddp_plan_subband_buffer(const ddp_plan* plan, uint32_t** d_sub) {
+extern "C" ddp_status ddp_plan_subband_buffer(const ddp_plan* plan, void** d_sub) {
     if (!plan || !d_sub) return DDP_E_ARG;
-    *d_sub = (plan->subband && plan->ws) ? plan->d_sub : nullptr;
+    *d_sub = (plan->subband && plan->ws) ? (void*)plan->d_sub : nullptr;
     return DDP_OK;
 }
 
@@ -651,7 +665,7 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
             break;
         case DDP_K_SUB1:  // g = subband, i = coarse DM, r = channel of the subband (SB.1)
             q.in = io.d_in;
-            q.out = p->d_sub;
+            q.out = p->d_sub;  // uint16 or uint32 elements (info.sub_elem_bytes); strides below are in elements
             q.delay = p->d_d1;
             q.in_row_stride = (long long)io.in_stride;
             q.in_group_stride = (long long)io.in_stride * p->cps;

@@ -37,6 +37,11 @@ class GpuSearch:
         self.buf["d_in"].copy_(torch.from_numpy(X))
         torch.cuda.synchronize()
 
+    def upload(self):
+        """Re-uploads self.X after the test changed it in place."""
+        self.buf["d_in"].copy_(self.torch.from_numpy(self.X))
+        self.torch.cuda.synchronize()
+
     def dedisperse(self):
         self.plan.dedisperse(self.buf["d_in"], self.buf["d_out"])
         self.torch.cuda.synchronize()
@@ -75,14 +80,13 @@ class GpuSearch:
         import ctypes
         i = self.info
         n = i.n_coarse * i.n_subbands * i.sub_stride
-        host = np.empty(n, dtype=np.uint32)
+        dt = {2: np.uint16, 4: np.uint32}[i.sub_elem_bytes]  # SB.4: narrow storage where exact
         ptr = self.plan.subband_buffer()
         assert ptr
         # the buffer lives inside the torch workspace tensor: find its offset there
         base = self.buf["workspace"].data_ptr()
         off = ptr - base
-        ws = self.buf["workspace"][off: off + n * 4].cpu().numpy().view(np.uint32)
-        host[:] = ws
+        host = self.buf["workspace"][off: off + n * i.sub_elem_bytes].cpu().numpy().view(dt).astype(np.uint32)
         return host.reshape(i.n_coarse, i.n_subbands, i.sub_stride)[:, :, : i.nsamp_sub]
 
     def close(self):

@@ -208,6 +208,42 @@ def test_subband_plan_kernel_configuration_sweep(kernel):
     g.close()
 
 
+def test_subband_wide_subbands_keep_uint32_intermediate():
+    """SB.4: more than 257 channels per subband cannot be stored in 16 bits -> uint32 S, generic step 2."""
+    cfg = small_subband(name="wide_sb", nchan=1040, nsamp_out=1500, ndm=4 * 6,
+                        subband=SubbandPlan(n_subbands=2, n_coarse=4, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=6, fine_step=0.25))
+    g = GpuSearch(cfg)
+    assert g.info.sub_elem_bytes == 4
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    assert np.array_equal(g.subband_intermediate(), So)
+    compare_all(g, Yo, what="wide_sb default")
+    for kernel in (ddp.K_SUB1, ddp.K_SUB2):
+        for c in _sample(g.plan.enumerate_kcfgs(kernel), 12, seed=7 + kernel):
+            g.plan.set_kcfg(kernel, c)
+            g.buf["d_out"].fill_(-1)
+            Y = g.dedisperse()
+            assert np.array_equal(g.subband_intermediate(), So), "S differs for %r" % c
+            assert np.array_equal(Y, Yo), "Y differs for %s %r" % (ddp.KERNEL_NAMES[kernel], c)
+    g.close()
+
+
+def test_subband_saturated_input_fills_the_uint16_intermediate():
+    """255 everywhere: S = 255 * channels-per-subband is the largest value the narrow storage must hold."""
+    cfg = small_subband(name="sat_sb", nchan=8 * 256, nsamp_out=1100, ndm=3 * 4,
+                        subband=SubbandPlan(n_subbands=8, n_coarse=3, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=4, fine_step=0.25))
+    g = GpuSearch(cfg)
+    assert g.info.sub_elem_bytes == 2
+    g.X[:] = 255
+    g.upload()
+    Y = g.dedisperse()
+    assert np.all(g.subband_intermediate() == 255 * 256)
+    assert np.all(Y == 255 * 8 * 256)
+    g.close()
+
+
 # ---------------------------------------------------------------------------------- full-size configs
 def _sampled_rows(ndm, n, seed):
     rng = np.random.default_rng(seed)
