@@ -470,10 +470,15 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     // staged extent of reduction row r: aligned start (elements from the row start) and words to stage
     auto row_extent = [&](int r, ddp_i64& a0, int& lenw) {
         const int s = r / SC;
-        const int dmin = dls[(size_t)(s & 1) * TD * SC + (r - s * SC)];
+        const int* d = dls + (size_t)(s & 1) * TD * SC + (r - s * SC);
+        const int dmin = d[0], dmax = d[(nd - 1) * SC];  // delays do not decrease with the trial index
         a0 = ((ddp_i64)tile_t + dmin) & ~(ddp_i64)15;
+        // words this row's own trials read (p.win bounds it for the worst row of the plan), whole uint4s
+        int need = (((int)((ddp_i64)tile_t + dmin - a0) + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
+        need = (need + 3) & ~3;
+        if (need > winw) need = winw;
         ddp_i64 l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
-        lenw = (int)(l < winw ? (l < 0 ? 0 : l) : winw);
+        lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
     };
     auto tma_issue = [&](int c) {  // warp 0, lane u < U: raw window of row u of chunk c -> raw slot c & 1
         unsigned char* dst = raw + (size_t)(c & 1) * U * (win + 16);
