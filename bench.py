@@ -215,6 +215,46 @@ class ClockSampler:
         return out
 
 
+# ------------------------------------------------------------------------------------ tuner comparison
+CAMPAIGN_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "campaign_b200.json")
+# The paper's own tuning-time figures: ANOTHER machine, ANOTHER workload -- context, never a target.
+PAPER_TUNING_CONTEXT = {
+    "brute_force_hours": "5-24 (about 10 on one GPU)", "ga_hours": "2-5",
+    "hardware": "NVIDIA GeForce GTX Titan X (Maxwell), ARTS cluster node ARTS0; OpenCL kernels",
+    "what_one_evaluation_is": "a whole external pipeline run, 3-minute cap", "cite": "PAPER.md:7, 115, 205, 225",
+}
+
+
+def tuning_report():
+    """GA vs brute force vs random search (BASELINE.json metric, configs[4]).  A campaign takes about
+    half an hour of GPU time, so it is NOT run inside the bench: this quotes the committed summary of
+    the last campaign (campaign.py -> campaign_summary.py) and says so.  None if no campaign is stored."""
+    out = {"measured_in_this_run": False, "paper_context": PAPER_TUNING_CONTEXT, "stored": None}
+    if not os.path.exists(CAMPAIGN_JSON):
+        return out
+    with open(CAMPAIGN_JSON) as fh:
+        c = json.load(fh)
+    def runs(kind):
+        return {s: {"final_ms": r["final_ms"], "evaluations": r["n_fitness_calls"], "kernel_timings": r["n_kernel_timings"],
+                    "compiles": r["n_compiles"], "wall_s": round(r["wall_seconds"], 1), "best_so_far_at": r["best_so_far_at"]}
+                for s, r in c.get(kind, {}).get("runs", {}).items()}
+    bf = c.get("bf", {})
+    out["stored"] = {
+        "source": "paper_1811_04165_b200/campaign_b200.json (python -m paper_1811_04165_b200.campaign --workload cfg2; "
+                  "times are the campaign's interleaved re-timing of each tuner's best joint configuration)",
+        "workload": c.get("workload"), "gpu": c.get("gpu"), "unit": "ms per pipeline pass (sub1+sub2+integrate+snr)",
+        "valid_configurations_per_kernel": c.get("space"), "defaults_ms": c.get("defaults_ms"),
+        "brute_force": {"final_ms": bf.get("final_ms"), "sum_of_isolated_minima_ms": bf.get("sum_isolated_min_ms"),
+                        "evaluations": bf.get("n_fitness_calls"), "wall_s": round(bf.get("wall_seconds", 0.0), 1)},
+        "ga": runs("ga"), "random": runs("random"),
+        "ga_final_ms_median": c.get("ga", {}).get("final_ms_median"),
+        "random_final_ms_median": c.get("random", {}).get("final_ms_median"),
+        "ga_vs_bf": c.get("ga_vs_bf"),
+        "note": "wall_s of seeds after the first is warm: compiled code shapes are memoised within the campaign process",
+    }
+    return out
+
+
 # ------------------------------------------------------------------------------------ our arm
 def apply_tuned(plan, ddp, workload):
     """Loads the committed tuned kernel configurations of the workload (written by the tuners on a
@@ -394,7 +434,8 @@ def run_ours(args):
                     "h2d_bytes_per_step": int(h_in.numel()),
                     "d2h_bytes_per_step": int(h_snr.numel() * 4 + h_arg.numel() * 4)},
             "gpu_launches": int(kernels_per_step * args.steps),
-            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "parity": parity}
+            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "parity": parity,
+            "tuning": tuning_report()}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
