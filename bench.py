@@ -38,7 +38,11 @@ ALU_LANES_PER_CLK_PER_SM = 64  # alu pipe: 4 SMSP x 16 lanes/clk (rt_SMSP = 2; B
 TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
-NCU_TRAFFIC_BYTES = {"cfg1": 260067072}  # profiles/r01_cfg1.md: 91.5 MB read + 168.6 MB written
+# dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) from one `ncu --set full` capture
+# (stored, not measured by the bench; cold-cache, ncu flushes caches between replay passes):
+#   cfg1  profiles/r01_cfg1.md   91.5 MB read + 168.6 MB written
+#   cfg2  profiles/r01_cfg2.md   sub1 49.1 + 47.4 MB, sub2 101.0 + 143.3 MB (capture "after", commit cc0769b)
+NCU_TRAFFIC_BYTES = {"cfg1": 260067072, "cfg2": 340865280}
 
 
 def measured_peaks():
