@@ -40,9 +40,10 @@ TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
 # dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) from one `ncu --set full` capture
 # (stored, not measured by the bench; cold-cache, ncu flushes caches between replay passes):
-#   cfg1  profiles/r01_cfg1.md   91.5 MB read + 168.6 MB written
+#   cfg1  profiles/r01_final.md  228.6 MB read + 172.0 MB written (1.57x algorithmic: read-backs of the wide flush)
 #   cfg2  profiles/r01_cfg2.md   sub1 49.1 + 47.4 MB, sub2 101.0 + 143.3 MB (capture "after", commit cc0769b)
-NCU_TRAFFIC_BYTES = {"cfg1": 260067072, "cfg2": 340865280}
+#   cfg3  profiles/r01_final.md  1154.3 MB read + 318.0 MB written
+NCU_TRAFFIC_BYTES = {"cfg1": 400645376, "cfg2": 340865280, "cfg3": 1472343312}
 
 
 def measured_peaks():
