@@ -75,6 +75,7 @@ bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k);
 int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD);           // dedisp kernels only
 int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // staged row window (elements)
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
+bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // packed uint8 kernel: one copy buffer
 bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::string* why);
 const std::vector<ddp_kcfg>& ddp_valid_set(const ddp_plan* p, ddp_kernel k);
 bool ddp_kcfg_equal(const ddp_kcfg& a, const ddp_kcfg& b);

@@ -428,7 +428,7 @@ __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst
     }
 }
 
-template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE, bool OUT16>
+template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE, bool OUT16, bool SINGLE>
 __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p) {
     static_assert(SPT >= 4 && VEC >= 4, "packed staging works on whole 4-sample words");
     static_assert(!(WIDE && OUT16), "a uint16 result never needs the wide flush");
@@ -437,6 +437,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     constexpr int VW = VEC / 4;  // words per staging load
     constexpr int SC = 64;       // channels per delay superchunk (multiple of every U)
     constexpr int FL = 256;      // channels between flushes of the 16-bit lanes
+    // SINGLE: one buffer of shifted copies instead of two (the host picks it when two do not fit in
+    // 227 KB, so that wide windows can still take several channels per chunk): chunk c is converted and
+    // then summed, two barriers per chunk; the TMA raw slots stay double buffered, so the copy of
+    // chunk c+1 is still in flight while chunk c is processed.
+    constexpr int NBC = SINGLE ? 1 : 2;
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int nthreads = blockDim.x * blockDim.y;
     const int tid = ty * blockDim.x + tx;
@@ -452,9 +457,9 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     const ddp_u32 one = (ddp_u32)p.one;
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it)
-    ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [2][U][4][winw]
-    ddp_u32* offs = copies + (size_t)2 * U * 4 * winw;           // [2][TD][U]   byte offsets into ddp_smem
-    int* dls = (int*)(offs + (((size_t)2 * TD * U + 3) & ~(size_t)3));  // [2][TD][SC], 16-byte aligned
+    ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [NBC][U][4][winw]
+    ddp_u32* offs = copies + (size_t)NBC * U * 4 * winw;         // [NBC][TD][U] byte offsets into ddp_smem
+    int* dls = (int*)(offs + (((size_t)NBC * TD * U + 3) & ~(size_t)3));  // [2][TD][SC], 16-byte aligned
     unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
     ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
     const int nchunks = p.nred / U;
@@ -499,7 +504,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     // Each row is split over `parts` warps (a power of two), so the per-row set-up is done once per warp.
     const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
     auto stage = [&](int c) {
-        ddp_u32* cb = copies + (size_t)(c & 1) * U * 4 * winw;
+        ddp_u32* cb = copies + (size_t)(c & (NBC - 1)) * U * 4 * winw;
         for (int unit = warp; unit < (U << parts_log2); unit += nwarps) {
             const int u = unit >> parts_log2, part = unit & ((1 << parts_log2) - 1);
             ddp_i64 a0;
@@ -516,8 +521,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     };
     auto prep_offs = [&](int c) {
-        ddp_u32* ob = offs + (size_t)(c & 1) * TD * U;
-        const ddp_u32 cbase = (ddp_u32)((size_t)(c & 1) * U * 4 * winw);
+        ddp_u32* ob = offs + (size_t)(c & (NBC - 1)) * TD * U;
+        const ddp_u32 cbase = (ddp_u32)((size_t)(c & (NBC - 1)) * U * 4 * winw);
         const int s = (c * U) / SC;
         const int* d = dls + (size_t)(s & 1) * TD * SC + (c * U - s * SC);
         for (int idx = tid; idx < TD * U; idx += nthreads) {
@@ -624,18 +629,29 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     if constexpr (STAGING == 2) {
         if (warp == 0) {
             tma_issue(0);
-            if (nchunks > 1) tma_issue(1);
+            if (!SINGLE && nchunks > 1) tma_issue(1);
         }
-        ddp_mbar_wait(&mbar[0], 0u);
+        if constexpr (!SINGLE) ddp_mbar_wait(&mbar[0], 0u);
     }
-    stage(0);
-    prep_offs(0);
-    __syncthreads();
+    if constexpr (!SINGLE) {
+        stage(0);
+        prep_offs(0);
+        __syncthreads();
+    }
 
     for (int c = 0; c < nchunks; ++c) {
         const int r0 = c * U;
         if (r0 % SC == 0 && r0 + SC < p.nred) load_dls(r0 / SC + 1);
-        if (c + 1 < nchunks) {
+        if constexpr (SINGLE) {
+            // every thread has left chunk c - 1 (barrier at the end of the last iteration)
+            if constexpr (STAGING == 2) {
+                if (warp == 0 && c + 1 < nchunks) tma_issue(c + 1);  // raw slot (c + 1) & 1 was converted in iteration c - 1
+                ddp_mbar_wait(&mbar[c & 1], (ddp_u32)((c >> 1) & 1));
+            }
+            stage(c);
+            prep_offs(c);
+            __syncthreads();
+        } else if (c + 1 < nchunks) {
             if constexpr (STAGING == 2) {
                 if (warp == 0 && c + 2 < nchunks) tma_issue(c + 2);  // slot c & 1 was converted during iteration c - 1
                 ddp_mbar_wait(&mbar[(c + 1) & 1], (ddp_u32)(((c + 1) >> 1) & 1));
@@ -643,7 +659,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
             stage(c + 1);
             prep_offs(c + 1);
         }
-        const ddp_u32* ob = offs + ((size_t)(c & 1) * TD + ty * DPT) * U;
+        const ddp_u32* ob = offs + ((size_t)(c & (NBC - 1)) * TD + ty * DPT) * U;
 #pragma unroll
         for (int j = 0; j < DPT; ++j) {
 #pragma unroll
@@ -1210,12 +1226,13 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
 // ------------------------------------------------------------------------------------ entry points
 // uint8 / uint16 input with staging takes the packed kernels; everything else the generic one.
 // FLAGS: bit 0 WIDE (uint8 packed: reduction longer than 256 rows), bit 1 OUT16 (uint16 result: the
-// narrow subband intermediate), bits 2-3 log2 of the uint16 packed kernel's lane-sum group.
+// narrow subband intermediate), bits 2-3 log2 of the uint16 packed kernel's lane-sum group, bit 4 SINGLE
+// (uint8 packed: one buffer of shifted copies, chosen by the host when two do not fit).
 template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, int FLAGS>
 __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
-    constexpr bool WIDE = (FLAGS & 1) != 0, OUT16 = (FLAGS & 2) != 0;
+    constexpr bool WIDE = (FLAGS & 1) != 0, OUT16 = (FLAGS & 2) != 0, SINGLE = (FLAGS & 16) != 0;
     if constexpr (sizeof(IN_T) == 1 && STAGING != 0)
-        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16>(p);
+        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16, SINGLE>(p);
     else if constexpr (sizeof(IN_T) == 2 && STAGING != 0)
         ddp_dedisp_packed16_body<SPT, DPT, UNROLL, STAGING, VEC, 1 << ((FLAGS >> 2) & 3)>(p);
     else

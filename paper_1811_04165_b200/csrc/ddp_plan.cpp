@@ -299,11 +299,16 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (c.staging == 0) return 0;
             const DdpKGeom g = ddp_kgeom(p, k);
             const size_t row = (size_t)ddp_dedisp_win(p, k, c) * g.in_bytes;
-            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [2][U][4][win], offs [2][TD][U], dls [2][TD][64], raw, mbar
+            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
-                size_t b = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
-                if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
-                return b;
+                auto layout = [&](size_t nb) {
+                    size_t b = nb * 4 * row * c.unroll + ((nb * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+                    if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
+                    return b;
+                };
+                // two buffers of shifted copies when they fit, else one (ddp_u8_single_buffered)
+                const size_t two = layout(2);
+                return two <= DDP_SMEM_LIMIT ? two : layout(1);
             }
             if (g.in_bytes == 2) {  // ddp_dedisp_packed16_body: copies [NB][U][2][win/2] words, offs [TD][nred4], mbar [NB]
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
@@ -324,6 +329,17 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
         }
         default: return 0;
     }
+}
+
+// The packed uint8 kernel keeps two buffers of shifted copies (chunk c+1 converted while chunk c is
+// summed); a configuration whose two buffers exceed 227 KB runs with one, if that fits.
+bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    if (c.staging == 0 || ddp_kgeom(p, k).in_bytes != 1) return false;
+    const size_t row = (size_t)ddp_dedisp_win(p, k, c);
+    const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
+    size_t two = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+    if (c.staging == 2) two += 2 * (size_t)c.unroll * (row + 16) + 16;
+    return two > DDP_SMEM_LIMIT;
 }
 
 // Validity rules (from Table 3 P:136-152 + sm_100a limits).

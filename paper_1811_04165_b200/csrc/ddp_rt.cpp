@@ -232,12 +232,14 @@ const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck 
 //                 reduction is longer than that (direct dedispersion);
 //   bit 1  OUT16  subband step 1 writes the narrow (uint16) intermediate;
 //   bits 2-3      packed uint16 kernel (step 2): log2 of how many subband words are summed in 16-bit
-//                 lanes before they are split, the largest of {1, 2, 4} that cannot overflow.
+//                 lanes before they are split, the largest of {1, 2, 4} that cannot overflow;
+//   bit 4  SINGLE packed uint8 kernel with one buffer of shifted copies (two do not fit in 227 KB).
 int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const CodeKind ck = code_kind(p, k);
     int f = 0;
     if (ck == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) f |= 1;
     if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
+    if (ck == CK_DEDISP_U8 && ddp_u8_single_buffered(p, k, c)) f |= 16;
     if (ck == CK_DEDISP_U16 && c.staging != 0) {
         const int64_t room = 65535 / (255 * (int64_t)p->cps);
         f |= (room >= 4 ? 2 : (room >= 2 ? 1 : 0)) << 2;

@@ -264,6 +264,11 @@ def test_cfg1_full_size_sampled_rows():
         i = int(round(p.dm / cfg.dm_step))
         lo, hi = max(0, i - 8), min(cfg.ndm, i + 9)
         assert S[lo:hi].max() > 6.0, "pulse %r not detected" % (p,)
+    # a shape whose two buffers of shifted copies exceed 227 KB: single-buffered copies + wide flush
+    Yo = oracle_direct_rows(cfg, g.X, rows)
+    g.plan.set_kcfg(ddp.K_DIRECT, ddp.Kcfg(64, 8, 16, 8, 16, 2, 16))
+    g.buf["d_out"].fill_(-1)
+    assert np.array_equal(g.dedisperse()[rows], Yo), "single-buffered direct kernel differs"
     g.close()
 
 
@@ -283,6 +288,14 @@ def test_cfg2_full_size_sampled_rows_and_identity_rows():
     d = configs.apertif_direct()
     Yd = oracle_direct_rows(d, g.X, coarse * sb.n_fine)
     assert np.array_equal(u32(g.buf["d_out"])[coarse * sb.n_fine, : cfg.nsamp_out], Yd)
+    # step-1 shapes whose two buffers of shifted copies exceed 227 KB run single-buffered (TMA and
+    # cooperative staging): same S, same Y
+    for genes in ([128, 4, 16, 8, 4, 2, 16], [128, 4, 16, 8, 4, 1, 16]):
+        g.plan.set_kcfg(ddp.K_SUB1, ddp.Kcfg(*genes))
+        g.buf["d_out"].fill_(-1)
+        Y = g.dedisperse()
+        assert np.array_equal(g.subband_intermediate()[coarse], So), "S differs for single-buffered %r" % genes
+        assert np.array_equal(Y[rows], Yo), "Y differs for single-buffered %r" % genes
     g.close()
 
 

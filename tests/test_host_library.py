@@ -272,8 +272,12 @@ def test_validity_rules_named_cases():
         assert not plan.check_kcfg(ddp.K_SUB1, c), why
     # V4: 48 channels per subband -> unroll 16 divides, and sub2 (32 subbands) accepts 16 too
     assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 16, 0, 16))
-    # V6: the same shape staged needs 16 rows x 4 shifted copies x 2 buffers of a ~2.5 KB window
-    assert not plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 16, 1, 16))
+    # V6: the same shape staged needs 16 rows x 4 shifted copies of a ~2.5 KB window; two buffers of
+    # them exceed 227 KB, one fits, so the shape is valid and runs single-buffered ...
+    assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 16, 1, 16))
+    # ... while 8 rows of the 7.7 KB windows of a 2048 x 32 tile do not fit even once
+    assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(128, 4, 16, 8, 4, 2, 16))
+    assert not plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(128, 4, 16, 8, 8, 2, 16))
     # uint32-input kernels need vec_bytes >= 4
     assert not plan.check_kcfg(ddp.K_SUB2, ddp.Kcfg(128, 2, 4, 4, 4, 0, 1))
     # the direct kernel is not part of a subband plan
