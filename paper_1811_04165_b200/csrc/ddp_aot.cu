@@ -35,8 +35,11 @@ DDP_AOT_SNR(4, 1, 1, 2, 16, 256)
 // tuned shapes of tuned_b200.json (cfg1 / cfg2 / cfg3 on B200), so that the bench needs no run-time compiler
 DDP_AOT_U8(16, 4, 16, 2, 16, 512, 1)   // cfg1 direct   [64,8,16,4,16,TMA,16]
 DDP_AOT_U8(16, 8, 4, 2, 16, 512, 1)    // cfg3 direct   [64,8,16,8,4,TMA,16]
-DDP_AOT_U8(16, 8, 2, 2, 16, 512, 2)    // cfg2 sub1     [128,4,16,8,2,TMA,16], uint16 result
+DDP_AOT_U8(16, 8, 4, 2, 8, 512, 18)    // cfg2 sub1     [128,4,16,8,4,TMA,8], uint16 result, single-buffered copies
+DDP_AOT_U8(16, 8, 2, 2, 16, 512, 2)    // cfg2 sub1, best double-buffered shape [128,4,16,8,2,TMA,16]
 DDP_AOT_U16(8, 4, 8, 2, 16, 256, 8)    // cfg2 sub2     [32,8,8,4,8,TMA,16], lane-sum group 4
 DDP_AOT_INTEG(16, 2, 1, 0, 16, 256)    // integrate     [16|64,2,16,2,1,direct,16]
 DDP_AOT_SNR(8, 1, 1, 0, 8, 256)        // snr cfg1/cfg2 [64,2,8,1,1,direct,8]
 DDP_AOT_SNR(8, 1, 2, 0, 8, 256)        // snr cfg3      [32,8,8,1,2,direct,8]
+DDP_AOT_INTEG(16, 1, 1, 0, 16, 256)    // integrate cfg2 [16,2,16,1,1,direct,16]
+DDP_AOT_SNR(8, 1, 1, 0, 16, 256)       // snr cfg2      [64,4,8,1,1,direct,16]
