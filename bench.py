@@ -41,9 +41,9 @@ TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) from one `ncu --set full` capture
 # (stored, not measured by the bench; cold-cache, ncu flushes caches between replay passes):
 #   cfg1  profiles/r01_final.md  228.6 MB read + 172.0 MB written (1.57x algorithmic: read-backs of the wide flush)
-#   cfg2  profiles/r01_cfg2.md   sub1 49.1 + 47.4 MB, sub2 101.0 + 143.3 MB (capture "after", commit cc0769b)
+#   cfg2  profiles/r01_cfg2.md   sub1 49.1 + 48.3 MB, sub2 101.0 + 144.7 MB (final capture of round 1)
 #   cfg3  profiles/r01_final.md  1154.3 MB read + 318.0 MB written
-NCU_TRAFFIC_BYTES = {"cfg1": 400645376, "cfg2": 340865280, "cfg3": 1472343312}
+NCU_TRAFFIC_BYTES = {"cfg1": 400645376, "cfg2": 343099392, "cfg3": 1472343312}
 
 
 def measured_peaks():
