@@ -15,9 +15,13 @@
 #ifndef DDP_KERNELS_CUH_
 #define DDP_KERNELS_CUH_
 
-// How the packed dedispersion kernel accumulates its two 16-bit lane pairs (see ddp_dedisp_packed_body).
+// How the packed dedispersion kernel accumulates its two 16-bit lane pairs (see ddp_dedisp_packed_body):
+// 0 both as IMAD, 1 both as IADD3, 2 one lane pair + a 64-bit IMAD.WIDE sum, 3 even lanes IADD3 and odd
+// lanes IMAD.  Measured on B200 with the tuned shapes (dedispersion ms, cfg1 / cfg2 / cfg3):
+// mode 0 4.765 / 0.3746 / 21.41, mode 1 5.014 / 0.3865 / 22.62, mode 2 5.877 / 0.4278 / 29.86,
+// mode 3 4.684 / 0.3749 / 21.12 -- mode 3 spreads the adds over the alu and fma pipes best.
 #ifndef DDP_ACC_MODE
-#define DDP_ACC_MODE 0
+#define DDP_ACC_MODE 3
 #endif
 
 typedef unsigned char ddp_u8;
