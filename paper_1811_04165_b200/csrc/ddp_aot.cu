@@ -36,7 +36,8 @@ DDP_AOT_SNR(4, 1, 1, 2, 16, 256)
 DDP_AOT_U8(16, 4, 16, 2, 16, 512, 1)   // cfg1 direct   [64,8,16,4,16,TMA,16]
 DDP_AOT_U8(16, 8, 8, 2, 16, 512, 17)   // cfg3 direct   [128,4,16,8,8,TMA,16], wide flush, single-buffered copies
 DDP_AOT_U8(16, 8, 4, 2, 16, 512, 1)    // cfg3 direct, best double-buffered shape [64,8,16,8,4,TMA,16]
-DDP_AOT_U8(16, 8, 4, 2, 8, 512, 18)    // cfg2 sub1     [128,4,16,8,4,TMA,8], uint16 result, single-buffered copies
+DDP_AOT_U8(16, 8, 4, 2, 16, 512, 18)   // cfg2 sub1     [128,4,16,8,4,TMA,16], uint16 result, single-buffered copies
+DDP_AOT_U8(16, 8, 4, 2, 8, 512, 18)    // cfg2 sub1, 8-byte staging loads [128,4,16,8,4,TMA,8], uint16 result, single-buffered copies
 DDP_AOT_U8(16, 8, 2, 2, 16, 512, 2)    // cfg2 sub1, best double-buffered shape [128,4,16,8,2,TMA,16]
 DDP_AOT_U16(8, 4, 8, 2, 16, 256, 8)    // cfg2 sub2     [32,8,8,4,8,TMA,16], lane-sum group 4
 DDP_AOT_INTEG(16, 2, 1, 0, 16, 256)    // integrate     [16|64,2,16,2,1,direct,16]
