@@ -40,10 +40,10 @@ TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
 # dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) from one `ncu --set full` capture
 # (stored, not measured by the bench; cold-cache, ncu flushes caches between replay passes):
-#   cfg1  profiles/r01_final.md  228.6 MB read + 172.0 MB written (1.57x algorithmic: read-backs of the wide flush)
-#   cfg2  profiles/r01_cfg2.md   sub1 49.1 + 48.3 MB, sub2 101.0 + 144.7 MB (final capture of round 1)
-#   cfg3  profiles/r01_final.md  1154.3 MB read + 318.0 MB written
-NCU_TRAFFIC_BYTES = {"cfg1": 400645376, "cfg2": 343099392, "cfg3": 1472343312}
+#   cfg1  profiles/r01_final.md  221.2 MB read + 171.2 MB written (1.54x algorithmic, see the profile)
+#   cfg2  profiles/r01_final.md  sub1 49.2 + 48.6 MB, sub2 101.0 + 145.9 MB
+#   cfg3  profiles/r01_final.md  1170.0 MB read + 309.8 MB written
+NCU_TRAFFIC_BYTES = {"cfg1": 392428032, "cfg2": 344683520, "cfg3": 1479793472}
 
 
 def measured_peaks():

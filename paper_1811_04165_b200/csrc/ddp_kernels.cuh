@@ -19,7 +19,9 @@
 // 0 both as IMAD, 1 both as IADD3, 2 one lane pair + a 64-bit IMAD.WIDE sum, 3 even lanes IADD3 and odd
 // lanes IMAD.  Measured on B200 with the tuned shapes (dedispersion ms, cfg1 / cfg2 / cfg3):
 // mode 0 4.765 / 0.3746 / 21.41, mode 1 5.014 / 0.3865 / 22.62, mode 2 5.877 / 0.4278 / 29.86,
-// mode 3 4.684 / 0.3749 / 21.12 -- mode 3 spreads the adds over the alu and fma pipes best.
+// mode 3 4.684 / 0.3749 / 21.12.  Mode 3 wins by issuing less, not by pipe balance: at cfg1 3.72 G warp
+// instructions instead of 4.03 G (1.55 vs 1.68 per add), with the alu pipe at 73 % and fma at 19 %
+// (mode 0: 60 % / 30 %), profiles/r01_final.md.
 #ifndef DDP_ACC_MODE
 #define DDP_ACC_MODE 3
 #endif
