@@ -34,7 +34,13 @@ import numpy as np  # noqa: E402
 METRIC = "dm_trial_samples_per_s"
 UNIT = "DM-trial samples/s"
 SM_COUNT = 148
-ALU_LANES_PER_CLK_PER_SM = 64  # alu pipe: 4 SMSP x 16 lanes/clk (rt_SMSP = 2; B300_MICROARCH "Pipe rates")
+# Scalar int32 add rate of one SM.  MEASURED on B200 with ddp_ubench (profiles/r01_ubench.md): a
+# dependent-free IADD3 stream sustains 126.4-127.4 thread-adds/clk/SM, the issue-port limit of 4 SMSP x 32
+# lanes, i.e. twice the 64/clk of LOP3 / PRMT / IMAD / IDP.4A (63.2-63.9 measured).  Until the end of round 1
+# the roofline used 64 (the B300 guide's alu-pipe width), which overstated every fraction by 2x; the old
+# figure is still reported as roofline.frac_vs_64_lane_pipe for continuity.
+ADD_LANES_PER_CLK_PER_SM = 128
+ALU_LANES_PER_CLK_PER_SM = 64  # LOP3 / PRMT / IMAD pipes: 4 SMSP x 16 lanes/clk (B300_MICROARCH "Pipe rates"; measured 63.7)
 TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
@@ -381,7 +387,8 @@ def run_ours(args):
     peaks, peak_src = measured_peaks()
     dd_avg_ms = float(np.mean(dd_ms))
     adds = float(info.adds_dedisp)
-    alu_peak = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # Tadd/s
+    alu_peak = SM_COUNT * ADD_LANES_PER_CLK_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # Tadd/s
+    pipe64_peak = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
     achieved = adds / (dd_avg_ms * 1e-3) / 1e12
     in_bytes = float(info.nchan) * float(info.nsamp_in_required)
     out_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
@@ -389,8 +396,10 @@ def run_ours(args):
     hbm_bytes = in_bytes + out_bytes + sub_bytes
     roofline = {"bound": "alu", "kernel": "dedisperse (%s)" % ("sub1+sub2" if info.subband else "direct"),
                 "achieved": achieved, "peak": alu_peak, "unit": "Tadd/s", "frac": achieved / alu_peak,
-                "peak_source": "derived: %d SMs x %d int32 adds/clk/SM (alu pipe) x sm_max_mhz %.0f (%s)" % (
-                    SM_COUNT, ALU_LANES_PER_CLK_PER_SM, peaks["sm_max_mhz"], peak_src),
+                "peak_source": "%d SMs x %d int32 adds/clk/SM (IADD3 issue rate, measured 126.4-127.4 with ddp_ubench, "
+                               "profiles/r01_ubench.md) x sm_max_mhz %.0f (%s)" % (
+                    SM_COUNT, ADD_LANES_PER_CLK_PER_SM, peaks["sm_max_mhz"], peak_src),
+                "frac_vs_64_lane_pipe": achieved / pipe64_peak,  # the denominator used until the end of round 1
                 "algorithmic_adds_per_launch": adds, "kernel_ms": dd_avg_ms,
                 "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
                 "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (dd_avg_ms * 1e-3) / 1e9,

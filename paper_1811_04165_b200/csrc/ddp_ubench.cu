@@ -1,9 +1,12 @@
 // Instruction-rate micro-benchmarks behind the dedispersion add roofline (
 // "the per-SM integer-add rate of sm_100 is not in MEASURED_PEAKS.json and must be
 // measured on the box").  Standalone: build.py compiles it with nvcc for sm_100a into `ddp_ubench`;
-// `ddp_ubench` prints one JSON object with, per instruction mix, thread-operations per clock per SM
-// (SM cycles from clock64 inside the kernel, so the figure does not depend on the DVFS state) and
-// the same per second at the observed clock.  Nothing of the search is computed here.
+// `ddp_ubench` prints one JSON object with, per instruction mix, thread-operations per clock per SM:
+// "thread_ops_per_clk_per_sm_wall" = all thread-operations of the launch / CUDA-event time / (SMs x the
+// device's SM clock) -- the figure to use (B200, 1965 MHz: IADD3 126-127, LOP3 / PRMT / IMAD / IDP.4A 63.7) --
+// and "thread_ops_per_clk_per_sm" from clock64 deltas inside the kernel, which on B200 comes out 1.34x
+// higher than the wall-clock figure for every mix (cause not investigated) and is kept only for
+// comparison.  Nothing of the search is computed here.
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -105,6 +108,9 @@ __global__ void __launch_bounds__(512, 2) ubench(unsigned* out, unsigned long lo
     if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(c1 - c0);
 }
 
+static double g_clock_hz = 0.0;  // SM clock used for the wall-clock figure (cudaDeviceProp::clockRate)
+static double g_wall[M_COUNT];
+
 template <int MIX>
 static void run(int nsm, int iters, unsigned* d_out, unsigned long long* d_cyc, double* ops_clk_sm, double* ms_out) {
     const int blocks = 2 * nsm, threads = 512;  // two co-resident blocks per SM: 8 warps per scheduler
@@ -124,6 +130,7 @@ static void run(int nsm, int iters, unsigned* d_out, unsigned long long* d_cyc, 
     for (auto c : cyc) mean += (double)c;
     mean /= blocks;
     *ops_clk_sm = 2.0 * (double)kOpsPerBody[MIX] * iters * threads / mean;  // two blocks share an SM
+    g_wall[MIX] = (double)blocks * threads * (double)kOpsPerBody[MIX] * iters / (ms * 1e-3) / (nsm * g_clock_hz);
     *ms_out = ms;
     CK(cudaEventDestroy(e0));
     CK(cudaEventDestroy(e1));
@@ -134,6 +141,7 @@ int main(int argc, char** argv) {
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, 0));
     const int nsm = prop.multiProcessorCount;
+    g_clock_hz = (double)prop.clockRate * 1e3;
     unsigned* d_out;
     unsigned long long* d_cyc;
     CK(cudaMalloc(&d_out, (size_t)nsm * 1024 * sizeof(unsigned)));
@@ -154,6 +162,8 @@ int main(int argc, char** argv) {
     run<M_T>(nsm, iters, d_out, d_cyc, &r[M_T], &ms[M_T]);
     std::printf("{\"device\": \"%s\", \"sms\": %d, \"iters\": %d, \"thread_ops_per_clk_per_sm\": {", prop.name, nsm, iters);
     for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.2f", m ? ", " : "", kNames[m], r[m]);
+    std::printf("}, \"sm_clock_mhz\": %.0f, \"thread_ops_per_clk_per_sm_wall\": {", g_clock_hz / 1e6);
+    for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.2f", m ? ", " : "", kNames[m], g_wall[m]);
     std::printf("}, \"kernel_ms\": {");
     for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.4f", m ? ", " : "", kNames[m], ms[m]);
     std::printf("}}\n");
