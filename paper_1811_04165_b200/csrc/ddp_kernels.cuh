@@ -17,9 +17,10 @@
 
 // How the packed dedispersion kernel accumulates its two 16-bit lane pairs (see ddp_dedisp_packed_body):
 // 0 both as IMAD, 1 both as IADD3, 2 one lane pair + a 64-bit IMAD.WIDE sum, 3 even lanes IADD3 and odd
-// lanes IMAD.  Measured on B200 with the tuned shapes (dedispersion ms, cfg1 / cfg2 / cfg3):
+// lanes IMAD, 4 even lanes IADD3 and sum(w >> 8) by IMAD.HI.  Measured on B200 with the tuned shapes (dedispersion ms, cfg1 / cfg2 / cfg3):
 // mode 0 4.765 / 0.3746 / 21.41, mode 1 5.014 / 0.3865 / 22.62, mode 2 5.877 / 0.4278 / 29.86,
-// mode 3 4.684 / 0.3749 / 21.12.  Mode 3 wins by issuing less, not by pipe balance: at cfg1 3.72 G warp
+// mode 3 4.684 / 0.3749 / 21.12, mode 4 (one extraction, w >> 8 summed by IMAD.HI; exact, parity green)
+// 5.455 / 0.4177 / 25.42: IMAD.HI takes a 64-bit addend and extra moves.  Mode 3 wins by issuing less, not by pipe balance: at cfg1 3.72 G warp
 // instructions instead of 4.03 G (1.55 vs 1.68 per add), with the alu pipe at 73 % and fma at 19 %
 // (mode 0: 60 % / 30 %), profiles/r01_final.md.
 #ifndef DDP_ACC_MODE
@@ -573,6 +574,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
 #if DDP_ACC_MODE == 2
                     const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
+#elif DDP_ACC_MODE == 4  // accO holds sum(w >> 8) = b1 + 2^8 b2 + 2^16 b3 as one integer; b2 is accE's high lane
+                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);
 #else
                     const ddp_u32 oo = accO[j][k];
 #endif
@@ -593,6 +596,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
 #if DDP_ACC_MODE == 2
                     const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
+#elif DDP_ACC_MODE == 4  // accO holds sum(w >> 8) = b1 + 2^8 b2 + 2^16 b3 as one integer; b2 is accE's high lane
+                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);
 #else
                     const ddp_u32 oo = accO[j][k];
 #endif
@@ -683,6 +688,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                     const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
                     accE[j][k] += e;
                     accO[j][k] += o;
+#elif DDP_ACC_MODE == 4  // ONE extraction: even bytes as 16-bit lanes (IADD3), and w >> 8 summed as a plain
+                         // 32-bit integer by mad.hi(w, 2^24, acc): exact while rows x (2^24 - 1) < 2^32, i.e. for
+                         // the <= 256 rows between flushes; the odd-byte sums are recovered in emit()
+                    accE[j][k] += e;
+                    asm("mad.hi.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(w), "r"(one << 24));
 #elif DDP_ACC_MODE == 3  // even lanes IADD3, odd lanes IMAD
                     const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
                     accE[j][k] += e;
