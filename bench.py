@@ -1,23 +1,29 @@
 #!/usr/bin/env python
-"""bench.py -- the headline measurement (BASELINE.json `metric`: DM-trial samples/s, + % of roofline).
+"""bench.py -- the headline measurement (BASELINE.json `metric`: DM-trial samples/s per config, + % of roofline;
+GA vs brute force vs random search).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg0]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg0] [--also cfg3 cfg2]
     python bench.py --impl reference ...        # the oracle, on the host cores, same metric
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A "step" is one pass of the whole hot path (dedisperse -> integrate -> snr) over one
-batch of synthetic input (BASELINE.json configs[1] by default: Apertif-like direct dedispersion,
-1536 channels x 24 414 samples x 2048 DM trials x 9 widths), through the C ABI (include/ddp.h).
-`value` = DM-trial samples per second of the whole job with the filterbank resident in HBM;
-`e2e` = the same through ddp_search_host with HOST buffers (H2D of the filterbank and D2H of the
-S/N table inside the timed region).  Multi-GPU: one process per GPU, each searching its own beam
-(no data-path collective) -> weak scaling, time = max over ranks.
+A "step" is one pass of the whole hot path (dedisperse -> integrate -> snr) over one batch of
+synthetic input, through the C ABI (include/ddp.h).  The top-level fields describe `--workload` (default
+BASELINE.json configs[1]: Apertif-like direct dedispersion, 1536 channels x 24 414 samples x 2048 DM trials x 9
+widths); at N = 1 the other full-size configs (`--also`, default cfg3 = the largest single-GPU workload, and
+cfg2 = the subband pair) are timed in the same invocation and reported under `per_config`, and a short real
+tuner comparison (`--tune-budget`) runs on cfg2's buffers.  `value` = DM-trial samples per second of the whole job
+with the filterbank resident in HBM; `e2e` = the same through ddp_search_host with HOST buffers (H2D of the
+filterbank and D2H of the S/N table inside the timed region).  Multi-GPU: one process per GPU, each searching its
+own beam (no data-path collective) -> weak scaling, time = max over ranks.
 
-One JSON line is printed by rank 0.  DESIGN.md "Measurement" defines every figure in it.
+Every workload's GPU result is compared with the oracle in the same run (`config.parity`); a mismatch makes the
+bench print `"value": null` with an `error` and exit non-zero.  One JSON line is printed by rank 0.
+"Measurement" defines every figure in it.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
 import subprocess
@@ -34,22 +40,18 @@ import numpy as np  # noqa: E402
 METRIC = "dm_trial_samples_per_s"
 UNIT = "DM-trial samples/s"
 SM_COUNT = 148
-# Scalar int32 add rate of one SM.  MEASURED on B200 with ddp_ubench (profiles/r01_ubench.md): a
-# dependent-free IADD3 stream sustains 126.4-127.4 thread-adds/clk/SM, the issue-port limit of 4 SMSP x 32
-# lanes, i.e. twice the 64/clk of LOP3 / PRMT / IMAD / IDP.4A (63.2-63.9 measured).  Until the end of round 1
-# the roofline used 64 (the B300 guide's alu-pipe width), which overstated every fraction by 2x; the old
-# figure is still reported as roofline.frac_vs_64_lane_pipe for continuity.
-ADD_LANES_PER_CLK_PER_SM = 128
-ALU_LANES_PER_CLK_PER_SM = 64  # LOP3 / PRMT / IMAD pipes: 4 SMSP x 16 lanes/clk (B300_MICROARCH "Pipe rates"; measured 63.7)
+# Scalar int32 add rate of one SM, adds per clock (measured with ddp_ubench, whose loop
+# bodies are verified in SASS at build time -- profiles/r02_ubench.md):
+#   IADD3 issues at 64 thread-instructions/clk/SM (alu pipe, like LOP3 / PRMT); a three-input IADD3 performs two
+#   additions -> 128 adds/clk/SM on the alu pipe alone;
+#   IMAD (fma pipe) issues at 64/clk/SM beside it, one addition each, when the two are interleaved.
+# The roofline denominator is the best measured mix (`ADD_PEAK_PER_CLK_PER_SM`); the alu-only 128 and the
+# 64-lane figure of round 1 are kept as extra fractions so that earlier numbers stay comparable.
+ADD_PEAK_PER_CLK_PER_SM = 192       # three-input IADD3 on the alu pipe + IMAD on the fma pipe, co-issued
+ADD_ALU_ONLY_PER_CLK_PER_SM = 128   # three-input IADD3 alone (the denominator of round 1's last bench line)
+PIPE_LANES_PER_CLK_PER_SM = 64      # one 64-lane pipe at one addition per instruction
 TUNED_JSON = os.path.join(ROOT, "paper_1811_04165_b200", "tuned_b200.json")
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture exists for the workload).
-# dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) from one `ncu --set full` capture
-# (stored, not measured by the bench; cold-cache, ncu flushes caches between replay passes):
-#   cfg1  profiles/r01_final.md  221.2 MB read + 171.2 MB written (1.54x algorithmic, see the profile)
-#   cfg2  profiles/r01_final.md  sub1 49.2 + 48.6 MB, sub2 101.0 + 145.9 MB
-#   cfg3  profiles/r01_final.md  1170.0 MB read + 309.8 MB written
-NCU_TRAFFIC_BYTES = {"cfg1": 392428032, "cfg2": 344683520, "cfg3": 1479793472}
+IN_SLACK = 32  # bytes of readable slack after the last needed sample of a row (include/ddp.h: in_stride_min)
 
 
 def measured_peaks():
@@ -58,6 +60,23 @@ def measured_peaks():
         with open(path) as fh:
             return json.load(fh), "measured"
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dedispersion launch(es) of one step, from the newest
+    profiles/rNN_traffic.json (written from an `ncu --set full` capture of this bench; see the .md beside it).
+    None when no capture of the workload is stored."""
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.json")))
+    for path in reversed(files):
+        try:
+            with open(path) as fh:
+                t = json.load(fh)
+        except (OSError, ValueError):
+            continue
+        if workload in t and t[workload].get("dedisperse_dram_bytes") is not None:
+            return {"bytes": t[workload]["dedisperse_dram_bytes"], "source": os.path.relpath(path, ROOT),
+                    "kernels": t[workload].get("kernels")}
+    return None
 
 
 def get_cfg(name):
@@ -70,22 +89,44 @@ def widths_of(cfg):
 
 
 # ------------------------------------------------------------------------------------ oracle legs
-def oracle_rows_chain(cfg, X, rows):
-    """The oracle as it stands on the given DM rows: dedisperse (direct or subband) -> integrate ->
-    snr.  Returns (Y, snr, argmax).  Only the cpu_baseline / --impl reference legs call this."""
+def oracle_tables(cfg, rows=None):
+    """Delay tables of the oracle for the given row units (all when None): direct -> (delay,), subband -> (d1, d2)."""
     import oracle
     if cfg.subband is None:
-        dms = cfg.dm_list()[np.asarray(rows)]
-        delay = oracle.delay_table(cfg.chan_freq_mhz(), dms, cfg.t_samp_s)
-        Y = oracle.dedisperse(X, delay, cfg.nsamp_out)
-    else:  # rows = coarse-DM indices; every fine DM of them is produced
-        sb = cfg.subband
-        A = (sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse))[np.asarray(rows)]
-        F = sb.fine_step * np.arange(sb.n_fine)
-        d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F)
-        S = oracle.subband_step1(X, d1, sb.n_subbands, cfg.nsamp_out + int(d2.max()))
-        Y = oracle.subband_step2(S, d2, cfg.nsamp_out)
-    _, S, A = oracle.search(Y, widths_of(cfg))
+        dms = cfg.dm_list() if rows is None else cfg.dm_list()[np.asarray(rows)]
+        return (oracle.delay_table(cfg.chan_freq_mhz(), dms, cfg.t_samp_s),)
+    sb = cfg.subband
+    A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+    if rows is not None:
+        A = A[np.asarray(rows)]
+    F = sb.fine_step * np.arange(sb.n_fine)
+    return oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F)
+
+
+def oracle_geometry(cfg):
+    """(nsamp_in, in_stride) of the workload from the ORACLE's delay tables alone -- the reference arm must not
+    touch the product library: nsamp_in = nsamp_out + max delay (DD.5 / SB.5), rows padded by the documented
+    32-byte slack to a multiple of 16 (include/ddp.h, in_stride_min)."""
+    t = oracle_tables(cfg)
+    max_delay = int(t[0].max()) if cfg.subband is None else int(t[0].max()) + int(t[1].max())
+    nsamp_in = cfg.nsamp_out + max_delay
+    return nsamp_in, (nsamp_in + IN_SLACK + 15) // 16 * 16
+
+
+def oracle_rows_chain(cfg, X, rows, mt=False):
+    """The oracle on the given row units: dedisperse (direct or subband) -> integrate -> snr.  mt=False: the
+    single-thread program as it stands; mt=True: the same functions with the rows spread over the host cores
+    (oracle_mt.cpp).  Returns (Y, snr, argmax).  Only the cpu_baseline / --impl reference legs call this."""
+    import oracle
+    t = oracle_tables(cfg, rows)
+    if cfg.subband is None:
+        Y = (oracle.dedisperse_mt if mt else oracle.dedisperse)(X, t[0], cfg.nsamp_out)
+    elif mt:
+        _, Y = oracle.subband_mt(X, t[0], t[1], cfg.subband.n_subbands, cfg.nsamp_out)
+    else:
+        S = oracle.subband_step1(X, t[0], cfg.subband.n_subbands, cfg.nsamp_out + int(t[1].max()))
+        Y = oracle.subband_step2(S, t[1], cfg.nsamp_out)
+    _, S, A = (oracle.search_mt if mt else oracle.search)(Y, widths_of(cfg))
     return Y, S, A
 
 
@@ -101,49 +142,45 @@ def strided_rows(n_units, k):
     return np.unique(np.linspace(0, n_units - 1, k).astype(np.int64))
 
 
-def time_oracle_sample(cfg, X, target_s):
+def time_oracle_sample(cfg, X, target_s, mt=False):
     """Times the oracle chain on an evenly strided sample of row units sized for ~target_s seconds.
     Returns dict(value, seconds, rows, trials, Y, S, A)."""
     n_units, per = oracle_units(cfg)
-    probe = strided_rows(n_units, 2)
+    probe = strided_rows(n_units, 2 if not mt else min(n_units, 16))
     t0 = time.perf_counter()
-    oracle_rows_chain(cfg, X, probe)
+    oracle_rows_chain(cfg, X, probe, mt)
     dt = max(time.perf_counter() - t0, 1e-6) / len(probe)
     rows = strided_rows(n_units, max(2, int(target_s / dt)))
     t0 = time.perf_counter()
-    Y, S, A = oracle_rows_chain(cfg, X, rows)
+    Y, S, A = oracle_rows_chain(cfg, X, rows, mt)
     sec = time.perf_counter() - t0
     trials = len(rows) * per
     return {"value": trials * cfg.nsamp_out / sec, "seconds": sec, "rows": rows, "trials": trials,
             "Y": Y, "S": S, "A": A}
 
 
-def make_input(cfg, info_nsamp_in, in_stride, beam=0):
+def make_input(cfg, nsamp_in, in_stride, beam=0):
     import dataclasses
-    from paper_1811_04165_b200.shard import beam_seed
     from synth import filterbank
-    c = cfg if beam == 0 else dataclasses.replace(cfg, seed=beam_seed(cfg.seed, beam))
-    X, _ = filterbank.make_filterbank(c, int(info_nsamp_in), int(in_stride))
+    c = cfg if beam == 0 else dataclasses.replace(cfg, seed=filterbank.beam_seed(cfg.seed, beam))
+    X, _ = filterbank.make_filterbank(c, int(nsamp_in), int(in_stride))
     return X
 
 
-def host_geometry(cfg):
-    """in_stride / nsamp_in of the workload without touching the GPU (plan creation is host code)."""
-    import paper_1811_04165_b200 as ddp
-    plan = ddp.plan_from_config(cfg, cache_dir=None)
-    i = plan.query()
-    out = (int(i.nsamp_in_required), int(i.in_stride_min))
-    plan.destroy()
-    return out
+def host_info():
+    import oracle
+    return {"nproc": os.cpu_count(), "cpu_model": oracle.cpu_model()}
 
 
 # ------------------------------------------------------------------------------------ reference arm
 def run_reference(args):
+    """The reference arm of this tier = the oracle as it stands (single thread) on the host cores; imports
+    nothing of the product (geometry comes from the oracle's own delay tables)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     cfg = get_cfg(args.workload)
-    nsamp_in, in_stride = host_geometry(cfg)
+    nsamp_in, in_stride = oracle_geometry(cfg)
     X = make_input(cfg, nsamp_in, in_stride)
     n_units, per = oracle_units(cfg)
     # calibrate: rows per step so that the whole run stays within ~2 minutes
@@ -165,12 +202,14 @@ def run_reference(args):
     sample = "%d of %d %s (evenly strided), all %d channels, %d samples, %d widths per step" % (
         len(rows), n_units, "DM rows" if cfg.subband is None else "coarse-DM groups", cfg.nchan, cfg.nsamp_out,
         len(cfg.widths))
+    hi = host_info()
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
             "config": {"workload": cfg.name, "nchan": cfg.nchan, "nsamp_out": cfg.nsamp_out, "ndm": cfg.ndm,
                        "widths": widths_of(cfg), "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                             "nproc": hi["nproc"], "cpu_model": hi["cpu_model"]},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -234,26 +273,27 @@ PAPER_TUNING_CONTEXT = {
     "hardware": "NVIDIA GeForce GTX Titan X (Maxwell), ARTS cluster node ARTS0; OpenCL kernels",
     "what_one_evaluation_is": "a whole external pipeline run, 3-minute cap", "cite": "PAPER.md:7, 115, 205, 225",
 }
+CURVE_AT = (16, 32, 64, 100, 150, 200, 300, 500, 1000)
 
 
-def tuning_report():
-    """GA vs brute force vs random search (BASELINE.json metric, configs[4]).  A campaign takes about
-    half an hour of GPU time, so it is NOT run inside the bench: this quotes the committed summary of
-    the last campaign (campaign.py -> campaign_summary.py) and says so.  None if no campaign is stored."""
-    out = {"measured_in_this_run": False, "paper_context": PAPER_TUNING_CONTEXT, "stored": None}
+def stored_campaign():
+    """The committed summary of the last full campaign (campaign.py -> campaign_summary.py): half an hour of GPU
+    time, so it is quoted, not re-run, by the bench -- and labelled as stored."""
     if not os.path.exists(CAMPAIGN_JSON):
-        return out
+        return None
     with open(CAMPAIGN_JSON) as fh:
         c = json.load(fh)
+
     def runs(kind):
         return {s: {"final_ms": r["final_ms"], "evaluations": r["n_fitness_calls"], "kernel_timings": r["n_kernel_timings"],
                     "compiles": r["n_compiles"], "wall_s": round(r["wall_seconds"], 1), "best_so_far_at": r["best_so_far_at"]}
                 for s, r in c.get(kind, {}).get("runs", {}).items()}
     bf = c.get("bf", {})
-    out["stored"] = {
+    return {
         "source": "paper_1811_04165_b200/campaign_b200.json (python -m paper_1811_04165_b200.campaign --workload cfg2; "
                   "times are the campaign's interleaved re-timing of each tuner's best joint configuration)",
-        "workload": c.get("workload"), "gpu": c.get("gpu"), "unit": "ms per pipeline pass (sub1+sub2+integrate+snr)",
+        "workload": c.get("workload"), "gpu": c.get("gpu"), "l2": c.get("l2", "warm (campaign of round 1)"),
+        "unit": "ms per pipeline pass (sub1+sub2+integrate+snr)",
         "valid_configurations_per_kernel": c.get("space"), "defaults_ms": c.get("defaults_ms"),
         "brute_force": {"final_ms": bf.get("final_ms"), "sum_of_isolated_minima_ms": bf.get("sum_isolated_min_ms"),
                         "evaluations": bf.get("n_fitness_calls"), "wall_s": round(bf.get("wall_seconds", 0.0), 1)},
@@ -261,18 +301,83 @@ def tuning_report():
         "ga_final_ms_median": c.get("ga", {}).get("final_ms_median"),
         "random_final_ms_median": c.get("random", {}).get("final_ms_median"),
         "ga_vs_bf": c.get("ga_vs_bf"),
-        "note": "wall_s of seeds after the first is warm: compiled code shapes are memoised within the campaign process",
     }
+
+
+def live_tuner_comparison(ddp, torch, dev, budget, seed=1):
+    """A SHORT real comparison measured in this run on BASELINE.json configs[2]'s buffers (the cfg4 campaign's
+    workload): GA, random search and a strided brute-force subset at about the same number of fitness
+    evaluations, every timed pass with a cold L2.  Returns the best pipeline time of each after re-timing the
+    three winners in interleaved rounds, plus best-so-far curves against evaluations (BJ:metric)."""
+    t_start = time.time()
+    cfg = get_cfg("cfg2")
+    plan = ddp.plan_from_config(cfg, device=dev.index or 0)
+    info = plan.query()
+    buf = ddp.alloc_buffers(plan, dev)
+    X = make_input(cfg, info.nsamp_in_required, info.in_stride_min)
+    buf["d_in"].copy_(torch.from_numpy(X))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    io = ddp.make_tune_io(buf["d_in"], buf["d_out"], buf["d_integ"], buf["d_snr"], buf["d_argmax"], d_flush=flush,
+                          reps=5, warmup=1, cutoff_factor=3.0)
+    kern = (ddp.K_SUB1, ddp.K_SUB2, ddp.K_INTEGRATE, ddp.K_SNR)
+    defaults = [plan.get_kcfg(k) for k in kern]
+
+    def reset():
+        for k, c in zip(kern, defaults):
+            plan.set_kcfg(k, c)
+
+    def curve(h):
+        out = {str(n): h[n - 1] for n in CURVE_AT if n <= len(h)}
+        if h:
+            out[str(len(h))] = h[-1]
+        return out
+
+    pop = 16
+    gens = max(1, (budget - pop) // (pop - 2))
+    out = {"measured_in_this_run": True, "workload": cfg.name, "unit": "ms per pipeline pass (sub1+sub2+integrate+snr)",
+           "l2": "256 MiB written before every timed pass", "fitness": "median of 5 passes of the summed CUDA-event times",
+           "budget_evaluations": budget, "space": {ddp.KERNEL_NAMES[k]: len(plan.enumerate_kcfgs(k)) for k in kern}}
+    d_ms, _ = plan.time_pipeline(io, defaults)
+    reset()
+    ga = plan.tune_ga(io, seed=seed, population=pop, generations=gens, tournament=3, p_cross=0.8, p_mut=0.05,
+                      elitism=2, max_evals=budget)
+    reset()
+    rnd = plan.tune_random(io, seed=seed, max_evals=ga["n_fitness_calls"])
+    reset()
+    bf = plan.tune_bruteforce(io, max_evals_per_kernel=max(1, budget // 4))
+    finalists = {"defaults": defaults, "ga": ga["best"], "random": rnd["best"], "bruteforce_subset": bf["best"]}
+    io_final = ddp.make_tune_io(buf["d_in"], buf["d_out"], buf["d_integ"], buf["d_snr"], buf["d_argmax"],
+                                d_flush=flush, reps=5, warmup=1, cutoff_factor=0.0)
+    samples = {k: [] for k in finalists}
+    for _ in range(3):
+        for k, c in finalists.items():
+            ms, _ = plan.time_pipeline(io_final, c)
+            samples[k].append(ms)
+    final = {k: sorted(v)[1] for k, v in samples.items()}
+    for name, res in (("ga", ga), ("random", rnd), ("bruteforce_subset", bf)):
+        out[name] = {"final_ms": final[name], "tuner_best_ms": res["best_ms"], "evaluations": res["n_fitness_calls"],
+                     "kernel_timings": res["n_kernel_timings"], "compiles": res["n_compiles"],
+                     "wall_s": round(res["wall_seconds"], 1), "best_so_far_at": curve(res["history"]),
+                     "cfg": [list(c.astuple()) for c in res["best"]]}
+    out["ga"]["params"] = {"population": pop, "generations": gens, "tournament": 3, "p_cross": 0.8, "p_mut": 0.05,
+                           "elitism": 2, "seed": seed}
+    out["bruteforce_subset"]["note"] = ("evenly strided subset of %d configurations per kernel (of %s); the four "
+                                        "winners timed together" % (max(1, budget // 4), out["space"]))
+    out["defaults_ms"] = final["defaults"]
+    out["defaults_ms_first_pass"] = d_ms
+    out["ga_vs_random"] = final["ga"] / final["random"]
+    out["wall_s"] = round(time.time() - t_start, 1)
+    plan.destroy()
     return out
 
 
 # ------------------------------------------------------------------------------------ our arm
 def apply_tuned(plan, ddp, workload):
-    """Loads the committed tuned kernel configurations of the workload (written by the tuners on a
-    B200) into the plan; returns the names applied."""
-    applied = {}
+    """Loads the committed tuned kernel configurations of the workload (written by the tuners on a B200) into
+    the plan; returns (applied, rejected): a tuned entry the plan refuses is reported, never skipped silently."""
+    applied, rejected = {}, {}
     if not os.path.exists(TUNED_JSON):
-        return applied
+        return applied, rejected
     with open(TUNED_JSON) as fh:
         tuned = json.load(fh).get(workload, {})
     for kname, genes in tuned.items():
@@ -281,39 +386,24 @@ def apply_tuned(plan, ddp, workload):
         if plan.check_kcfg(k, c):
             plan.set_kcfg(k, c)
             applied[kname] = list(genes)
-    return applied
+        else:
+            rejected[kname] = list(genes)
+    return applied, rejected
 
 
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    import paper_1811_04165_b200 as ddp
-    from paper_1811_04165_b200.shard import beams_of_rank, combine
-
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback "
-                         "(use --impl reference for the oracle arm)")
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
-    if args.gpus != world and rank == 0:
-        print("bench.py: --gpus %d but WORLD_SIZE %d; using WORLD_SIZE" % (args.gpus, world), file=sys.stderr)
-
-    cfg = get_cfg(args.workload)
-    plan = ddp.plan_from_config(cfg, device=local)
+def bench_workload(name, args, ctx, with_cpu):
+    """Times one workload on this rank's GPU; returns the per-workload record (rank-local; the caller combines
+    ranks for the top-level workload)."""
+    torch, ddp, dev, world, dist = ctx["torch"], ctx["ddp"], ctx["dev"], ctx["world"], ctx["dist"]
+    cfg = get_cfg(name)
+    plan = ddp.plan_from_config(cfg, device=dev.index or 0)
     info = plan.query()
-    tuned = apply_tuned(plan, ddp, args.workload)
+    tuned, rejected = apply_tuned(plan, ddp, name)
     buf = ddp.alloc_buffers(plan, dev)
-    beam = beams_of_rank(world, rank, world)[0]  # one beam per GPU (weak scaling)
-    X = make_input(cfg, info.nsamp_in_required, info.in_stride_min, beam)
+    X = make_input(cfg, info.nsamp_in_required, info.in_stride_min, ctx["beam"])
     h_in = torch.from_numpy(X).pin_memory()
     buf["d_in"].copy_(h_in)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    flush = ctx["flush"]
     h_snr = torch.empty((info.ndm, info.nwidths), dtype=torch.float32).pin_memory()
     h_arg = torch.empty((info.ndm, info.nwidths), dtype=torch.int32).pin_memory()
     kernels_per_step = 3 + (1 if info.subband else 0) - (0 if info.integ_elems > 0 else 1)
@@ -340,7 +430,7 @@ def run_ours(args):
         flush.zero_()
         step()
     barrier()
-    sampler = ClockSampler(local_gpu_id(torch, local))
+    sampler = ClockSampler(local_gpu_id(torch, dev.index or 0))
     ev = []
     for _ in range(args.steps):
         flush.zero_()  # L2 flush between timed iterations, outside the step's events
@@ -352,12 +442,10 @@ def run_ours(args):
         ev.append((e0, em, ei, e1))
     barrier()
     step_ms = [a.elapsed_time(d) for a, _, _, d in ev]
-    dd_ms = [a.elapsed_time(b) for a, b, _, _ in ev]
+    dd_ms = float(np.mean([a.elapsed_time(b) for a, b, _, _ in ev]))
     int_ms = float(np.mean([b.elapsed_time(c) for _, b, c, _ in ev]))
     snr_ms = float(np.mean([c.elapsed_time(d) for _, _, c, d in ev]))
     local_ms = float(sum(step_ms))
-    tot_ms, tot_units = combine(local_ms, units_per_step * args.steps, dev)
-    value = tot_units / (tot_ms * 1e-3)
 
     # ---- end-to-end arm: host buffers through ddp_search_host
     for _ in range(3):
@@ -375,85 +463,175 @@ def run_ours(args):
         e2e_ms += e0.elapsed_time(e1)
     barrier()
     clocks = sampler.stop()
-    e2e_tot_ms, _ = combine(e2e_ms, 0.0, dev)
+
+    # ---- roofline of the dominant kernel (dedispersion; DESIGN.md "Roofline denominators")
+    peaks, peak_src = measured_peaks()
+    adds = float(info.adds_dedisp)
+    per_clk = SM_COUNT * peaks["sm_max_mhz"] * 1e6 / 1e12  # Tadd/s per (add / clk / SM)
+    alu_peak = ADD_PEAK_PER_CLK_PER_SM * per_clk
+    achieved = adds / (dd_ms * 1e-3) / 1e12
+    in_bytes = float(info.nchan) * float(info.nsamp_in_required)
+    out_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
+    sub_bytes = 2.0 * info.n_coarse * info.n_subbands * float(info.nsamp_sub) * info.sub_elem_bytes if info.subband else 0.0
+    hbm_bytes = in_bytes + out_bytes + sub_bytes
+    traffic = ncu_traffic(name)
+    roofline = {"bound": "alu", "kernel": "dedisperse (%s)" % ("sub1+sub2" if info.subband else "direct"),
+                "achieved": achieved, "peak": alu_peak, "unit": "Tadd/s", "frac": achieved / alu_peak,
+                "peak_source": "%d SMs x %d int32 adds/clk/SM (three-input IADD3 on the alu pipe co-issued with IMAD on "
+                               "the fma pipe, measured with ddp_ubench, profiles/r02_ubench.md) x sm_max_mhz %.0f (%s)" % (
+                                   SM_COUNT, ADD_PEAK_PER_CLK_PER_SM, peaks["sm_max_mhz"], peak_src),
+                "frac_vs_alu_pipe_only_128": achieved / (ADD_ALU_ONLY_PER_CLK_PER_SM * per_clk),
+                "frac_vs_64_lane_pipe": achieved / (PIPE_LANES_PER_CLK_PER_SM * per_clk),
+                "algorithmic_adds_per_launch": adds, "kernel_ms": dd_ms,
+                "traffic": traffic["bytes"] if traffic else None, "traffic_source": traffic["source"] if traffic else None,
+                "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (dd_ms * 1e-3) / 1e9,
+                        "peak_gbs": peaks["hbm_gbs"], "frac": hbm_bytes / (dd_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        "peak_source": peak_src}}
+
+    # integrate / snr are HBM bound: read Y (+ planes), write planes (DESIGN.md 6.2, 6.3)
+    y_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
+    pl_bytes = 4.0 * float(info.ndm) * sum(float(info.plane_len[k]) for k in range(info.nwidths) if info.widths[k] > 1)
+    stages = {"dedisperse_ms": dd_ms,
+              "integrate": {"ms": int_ms, "algorithmic_bytes": y_bytes + pl_bytes,
+                            "hbm_frac": (y_bytes + pl_bytes) / (int_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+              "snr": {"ms": snr_ms, "algorithmic_bytes": y_bytes + pl_bytes,
+                      "hbm_frac": (y_bytes + pl_bytes) / (snr_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
+    # ---- the oracle timed beside it (rank 0, N = 1 only) + parity of the rows it computed
+    cpu, cpu_mt, parity = None, None, None
+    if with_cpu:
+        n_units, per = oracle_units(cfg)
+        Yg_all = buf["d_out"].cpu().numpy().view(np.uint32)
+        Sg_all, Ag_all = h_snr.numpy(), h_arg.numpy().view(np.uint32)
+        unit_name = "DM rows" if cfg.subband is None else "coarse-DM groups"
+        hi = host_info()
+
+        def check(r):
+            rows = r["rows"] if cfg.subband is None else (r["rows"][:, None] * per + np.arange(per)[None, :]).reshape(-1)
+            ok = (np.array_equal(Yg_all[rows, : cfg.nsamp_out], r["Y"]) and np.array_equal(Ag_all[rows], r["A"]) and
+                  bool(np.all(np.abs(Sg_all[rows] - r["S"]) <= 1e-5 * np.maximum(1.0, np.abs(r["S"])))))
+            return int(len(rows)), bool(ok)
+
+        r1 = time_oracle_sample(cfg, X, args.cpu_seconds, mt=False)
+        n1, ok1 = check(r1)
+        cpu = {"value": r1["value"], "unit": UNIT, "cores": 1, "kind": "oracle", "nproc": hi["nproc"],
+               "cpu_model": hi["cpu_model"],
+               "sample": "%d of %d %s (evenly strided): dedisperse+integrate+snr, single thread, %.1f s" % (
+                   len(r1["rows"]), n_units, unit_name, r1["seconds"])}
+        import oracle
+        rm = time_oracle_sample(cfg, X, args.cpu_seconds_mt, mt=True)
+        nm, okm = check(rm)
+        cpu_mt = {"value": rm["value"], "unit": UNIT, "cores": oracle.mt_threads(), "kind": "oracle, DM rows spread over "
+                  "the host cores (omp parallel for, oracle_mt.cpp)", "nproc": hi["nproc"], "cpu_model": hi["cpu_model"],
+                  "sample": "%d of %d %s (evenly strided), %.1f s" % (len(rm["rows"]), n_units, unit_name, rm["seconds"])}
+        parity = {"ok": bool(ok1 and okm), "rows_checked": int(len(set(r1["rows"].tolist()) | set(rm["rows"].tolist())) * per),
+                  "of_rows": int(info.ndm), "what": "dedispersion bit-exact, S/N <= 1e-5 relative, argmax exact",
+                  "legs": {"single_thread_rows": n1, "all_cores_rows": nm}}
+
+    rec = {"workload": cfg.name, "value": units_per_step * args.steps / (local_ms * 1e-3), "unit": UNIT,
+           "ms_per_step": local_ms / args.steps, "dedisp_ms": dd_ms, "roofline": roofline, "stages": stages,
+           "dedisp_only": {"value": units_per_step / (dd_ms * 1e-3), "unit": UNIT, "ms": dd_ms},
+           "e2e": {"value": units_per_step * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                   "h2d_bytes_per_step": int(h_in.numel()),
+                   "d2h_bytes_per_step": int(h_snr.numel() * 4 + h_arg.numel() * 4)},
+           "gpu_launches": int(kernels_per_step * args.steps), "clocks": clocks,
+           "kcfg": {ddp.KERNEL_NAMES[k]: list(plan.get_kcfg(k).astuple()) for k in range(5) if _in_plan(plan, k)},
+           "tuned_from": os.path.basename(TUNED_JSON) if tuned else None, "tuned_rejected": rejected or None,
+           "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_mt, "parity": parity,
+           "shape": {"nchan": cfg.nchan, "nsamp_out": cfg.nsamp_out, "ndm": cfg.ndm, "widths": widths_of(cfg)},
+           "working_set_mb": (hbm_bytes + info.integ_elems * 4.0) / 1e6,
+           "_local_ms": local_ms, "_e2e_ms": e2e_ms, "_units": units_per_step * args.steps}
+    plan.destroy()
+    del buf, h_in
+    torch.cuda.empty_cache()
+    return rec
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1811_04165_b200 as ddp
+    from paper_1811_04165_b200.shard import beams_of_rank, combine
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback "
+                         "(use --impl reference for the oracle arm)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    if args.gpus != world and rank == 0:
+        print("bench.py: --gpus %d but WORLD_SIZE %d; using WORLD_SIZE" % (args.gpus, world), file=sys.stderr)
+
+    ctx = {"torch": torch, "ddp": ddp, "dev": dev, "world": world, "dist": dist,
+           "beam": beams_of_rank(world, rank, world)[0],  # one beam per GPU (weak scaling)
+           "flush": torch.empty(256 << 20, dtype=torch.uint8, device=dev)}  # > 126 MB L2
+    with_cpu = world == 1 and not args.no_cpu_baseline
+    main_rec = bench_workload(args.workload, args, ctx, with_cpu)
+    tot_ms, tot_units = combine(main_rec["_local_ms"], main_rec["_units"], dev)
+    e2e_tot_ms, _ = combine(main_rec["_e2e_ms"], 0.0, dev)
+    value = tot_units / (tot_ms * 1e-3)
     e2e_value = tot_units / (e2e_tot_ms * 1e-3)
+
+    # ---- the other full-size configs and the live tuner comparison: N = 1 only (ranks are independent replicas)
+    per_config, tuning_live = {}, None
+    if world == 1:
+        also = [w for w in (args.also if args.also is not None else (["cfg3", "cfg2"] if args.workload == "cfg1" else []))
+                if w != args.workload]
+        ctx["beam"] = 0
+        for w in also:
+            per_config[w] = bench_workload(w, args, ctx, with_cpu)
+        if args.tune_budget > 0:
+            tuning_live = live_tuner_comparison(ddp, torch, dev, args.tune_budget)
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (dedispersion; DESIGN.md "Roofline")
-    peaks, peak_src = measured_peaks()
-    dd_avg_ms = float(np.mean(dd_ms))
-    adds = float(info.adds_dedisp)
-    alu_peak = SM_COUNT * ADD_LANES_PER_CLK_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # Tadd/s
-    pipe64_peak = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
-    achieved = adds / (dd_avg_ms * 1e-3) / 1e12
-    in_bytes = float(info.nchan) * float(info.nsamp_in_required)
-    out_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
-    sub_bytes = 2.0 * info.n_coarse * info.n_subbands * float(info.nsamp_sub) * info.sub_elem_bytes if info.subband else 0.0
-    hbm_bytes = in_bytes + out_bytes + sub_bytes
-    roofline = {"bound": "alu", "kernel": "dedisperse (%s)" % ("sub1+sub2" if info.subband else "direct"),
-                "achieved": achieved, "peak": alu_peak, "unit": "Tadd/s", "frac": achieved / alu_peak,
-                "peak_source": "%d SMs x %d int32 adds/clk/SM (IADD3 issue rate, measured 126.4-127.4 with ddp_ubench, "
-                               "profiles/r01_ubench.md) x sm_max_mhz %.0f (%s)" % (
-                    SM_COUNT, ADD_LANES_PER_CLK_PER_SM, peaks["sm_max_mhz"], peak_src),
-                "frac_vs_64_lane_pipe": achieved / pipe64_peak,  # the denominator used until the end of round 1
-                "algorithmic_adds_per_launch": adds, "kernel_ms": dd_avg_ms,
-                "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (dd_avg_ms * 1e-3) / 1e9,
-                        "peak_gbs": peaks["hbm_gbs"], "frac": hbm_bytes / (dd_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        "peak_source": peak_src}}
+    def brief(r):
+        return {"workload": r["workload"], "value": r["value"], "ms_per_step": r["ms_per_step"], "dedisp_ms": r["dedisp_ms"],
+                "roofline": {"frac": r["roofline"]["frac"], "achieved": r["roofline"]["achieved"], "peak": r["roofline"]["peak"],
+                             "unit": r["roofline"]["unit"], "frac_vs_alu_pipe_only_128": r["roofline"]["frac_vs_alu_pipe_only_128"],
+                             "hbm_frac": r["roofline"]["hbm"]["frac"], "traffic": r["roofline"]["traffic"]},
+                "integrate": r["stages"]["integrate"], "snr": r["stages"]["snr"], "e2e": r["e2e"], "kcfg": r["kcfg"],
+                "tuned_rejected": r["tuned_rejected"], "cpu_baseline": r["cpu_baseline"],
+                "cpu_baseline_all_cores": r["cpu_baseline_all_cores"], "parity": r["parity"], "clocks": r["clocks"],
+                "gpu_launches": r["gpu_launches"], "shape": r["shape"]}
 
-    # integrate / snr are HBM bound: read Y (+ planes), write planes (DESIGN.md 6.2, 6.3)
-    y_bytes = float(info.ndm) * float(info.nsamp_out) * 4.0
-    pl_bytes = 4.0 * float(info.ndm) * sum(float(info.plane_len[k]) for k in range(info.nwidths) if info.widths[k] > 1)
-    stages = {"dedisperse_ms": dd_avg_ms,
-              "integrate": {"ms": int_ms, "algorithmic_bytes": y_bytes + pl_bytes,
-                            "hbm_frac": (y_bytes + pl_bytes) / (int_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]},
-              "snr": {"ms": snr_ms, "algorithmic_bytes": y_bytes + pl_bytes,
-                      "hbm_frac": (y_bytes + pl_bytes) / (snr_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
-
-    # ---- the oracle timed beside it (rank 0, N = 1 only) + parity of the sampled rows
-    cpu = None
-    parity = None
-    if world == 1 and not args.no_cpu_baseline:
-        r = time_oracle_sample(cfg, X, args.cpu_seconds)
-        n_units, per = oracle_units(cfg)
-        sample = "%d of %d %s (evenly strided): dedisperse+integrate+snr, %.1f s" % (
-            len(r["rows"]), n_units, "DM rows" if cfg.subband is None else "coarse-DM groups", r["seconds"])
-        cpu = {"value": r["value"], "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
-        rows = r["rows"] if cfg.subband is None else (
-            r["rows"][:, None] * per + np.arange(per)[None, :]).reshape(-1)
-        Yg = buf["d_out"].cpu().numpy().view(np.uint32)[rows, : cfg.nsamp_out]
-        Sg = h_snr.numpy()[rows]
-        Ag = h_arg.numpy().view(np.uint32)[rows]
-        ok = (np.array_equal(Yg, r["Y"]) and np.array_equal(Ag, r["A"]) and
-              bool(np.all(np.abs(Sg - r["S"]) <= 1e-5 * np.maximum(1.0, np.abs(r["S"])))))
-        parity = {"rows_checked": int(len(rows)), "ok": bool(ok)}
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    everything = [main_rec] + list(per_config.values())
+    failed = [r["workload"] for r in everything if r["parity"] is not None and not r["parity"]["ok"]]
+    m = main_rec
+    launches = sum(2 * r["gpu_launches"] + 2 * 3 * (r["gpu_launches"] // max(1, args.steps)) for r in everything)
+    line = {"metric": METRIC, "value": None if failed else value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": tot_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-            "config": {"workload": cfg.name, "nchan": cfg.nchan, "nsamp_out": cfg.nsamp_out, "ndm": cfg.ndm,
-                       "widths": widths_of(cfg), "beams_per_gpu": 1,
+            "config": {"workload": m["workload"], **m["shape"], "beams_per_gpu": 1,
                        "l2": "256 MiB memset between timed steps (outside each step's events); "
-                             "working set %.0f MB > 126 MB L2" % ((hbm_bytes + info.integ_elems * 4.0) / 1e6),
-                       "kcfg": {ddp.KERNEL_NAMES[k]: list(plan.get_kcfg(k).astuple())
-                                for k in range(5) if _in_plan(plan, k)},
-                       "tuned_from": os.path.basename(TUNED_JSON) if tuned else None},
-            "dedisp_only": {"value": world * units_per_step / (dd_avg_ms * 1e-3), "unit": UNIT, "ms": dd_avg_ms},
+                             "working set %.0f MB > 126 MB L2" % m["working_set_mb"],
+                       "kcfg": m["kcfg"], "tuned_from": m["tuned_from"], "tuned_rejected": m["tuned_rejected"],
+                       "parity": m["parity"],
+                       "parity_all_workloads": {r["workload"]: (r["parity"] or {}).get("ok") for r in everything}},
+            "dedisp_only": {"value": world * m["dedisp_only"]["value"], "unit": UNIT, "ms": m["dedisp_ms"]},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_tot_ms / args.steps,
-                    "h2d_bytes_per_step": int(h_in.numel()),
-                    "d2h_bytes_per_step": int(h_snr.numel() * 4 + h_arg.numel() * 4)},
-            "gpu_launches": int(kernels_per_step * args.steps),
-            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "parity": parity,
-            "tuning": tuning_report()}
+                    "h2d_bytes_per_step": m["e2e"]["h2d_bytes_per_step"], "d2h_bytes_per_step": m["e2e"]["d2h_bytes_per_step"]},
+            "gpu_launches": int(m["gpu_launches"]), "gpu_launches_whole_run": int(launches),
+            "clocks": m["clocks"], "roofline": m["roofline"], "stages": m["stages"],
+            "cpu_baseline": m["cpu_baseline"], "cpu_baseline_all_cores": m["cpu_baseline_all_cores"],
+            "parity": m["parity"],
+            "per_config": {k: brief(r) for k, r in per_config.items()},
+            "tuning": {"measured_in_this_run": tuning_live, "stored_campaign": stored_campaign(),
+                       "paper_context": PAPER_TUNING_CONTEXT}}
+    if failed:
+        line["error"] = "GPU result differs from the oracle on: %s -- no performance number is reported" % ", ".join(failed)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-    return 0
+    return 3 if failed else 0
 
 
 def _in_plan(plan, k):
@@ -480,8 +658,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the cpu_baseline sample")
+    ap.add_argument("--also", nargs="*", default=None, choices=["cfg0", "cfg1", "cfg2", "cfg3"],
+                    help="further workloads timed in the same run at N = 1 (default: cfg3 cfg2 when --workload is cfg1)")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target duration of the single-thread cpu_baseline sample")
+    ap.add_argument("--cpu-seconds-mt", type=float, default=5.0, help="target duration of the all-cores oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune-budget", type=int, default=120,
+                    help="fitness evaluations of the live GA / random / brute-force-subset comparison (0 = skip)")
     ap.add_argument("--ref-seconds", type=float, default=100.0, help="--impl reference: target duration of the whole run")
     args = ap.parse_args()
     if args.steps < 1:

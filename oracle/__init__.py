@@ -16,7 +16,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_SRC_MT = os.path.join(_HERE, "oracle_mt.cpp")
+_LIB_MT = os.path.join(_HERE, "liboracle_mt.so")
 _lib = None
+_lib_mt = None
 
 
 def build(force: bool = False) -> str:
@@ -26,6 +29,13 @@ def build(force: bool = False) -> str:
         subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC",
                                _SRC, "-o", tmp])
         os.replace(tmp, _LIB)
+    # the all-cores leg: oracle.cpp (unchanged) + oracle_mt.cpp (omp parallel for over rows)
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_MT))
+    if force or not os.path.exists(_LIB_MT) or os.path.getmtime(_LIB_MT) < newest:
+        tmp = _LIB_MT + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               _SRC, _SRC_MT, "-o", tmp])
+        os.replace(tmp, _LIB_MT)
     return _LIB
 
 
@@ -35,6 +45,30 @@ def _load():
         build()
         _lib = ctypes.CDLL(_LIB)
     return _lib
+
+
+def _load_mt():
+    global _lib_mt
+    if _lib_mt is None:
+        build()
+        _lib_mt = ctypes.CDLL(_LIB_MT)
+    return _lib_mt
+
+
+def mt_threads() -> int:
+    """Threads the all-cores leg uses (OpenMP default: one per host core unless OMP_NUM_THREADS says otherwise)."""
+    return int(_load_mt().oracle_mt_threads())
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def _p(a: np.ndarray):
@@ -147,6 +181,68 @@ def search(Y: np.ndarray, widths: Sequence[int], ddof: int = 0):
         I = Y if w == 1 else integrate(Y, w)
         planes[w] = I
         s, a = snr(np.ascontiguousarray(I), ddof)
+        S.append(s)
+        A.append(a)
+    return planes, np.stack(S, axis=1), np.stack(A, axis=1)
+
+
+# ---------------------------------------------------------------------------- all-cores leg (oracle_mt.cpp)
+# Same arithmetic: every row is computed by the single-thread function above, rows are spread over
+# the host cores with `omp parallel for`.
+def dedisperse_mt(X: np.ndarray, delay: np.ndarray, ns: int) -> np.ndarray:
+    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    nrows, nchan = delay.shape
+    assert nchan == X.shape[0]
+    Y = np.empty((nrows, ns), dtype=np.uint32)
+    rc = _load_mt().oracle_mt_dedisperse(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), _p(delay),
+                                         ctypes.c_int(nrows), ctypes.c_int(ns), _p(Y), ctypes.c_size_t(ns))
+    if rc != 0:
+        raise ValueError("oracle_mt_dedisperse rc=%d" % rc)
+    return Y
+
+
+def subband_mt(X: np.ndarray, d1: np.ndarray, d2: np.ndarray, nsub: int, ns: int):
+    """(S uint32 [ncoarse][nsub][ns + max d2], Y uint32 [ncoarse*nfine][ns]), coarse DMs spread over the cores."""
+    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    d1 = np.ascontiguousarray(d1, dtype=np.int32)
+    d2 = np.ascontiguousarray(d2, dtype=np.int32)
+    ncoarse, nchan = d1.shape
+    nfine = d2.shape[0]
+    ns1 = ns + int(d2.max())
+    S = np.empty((ncoarse, nsub, ns1), dtype=np.uint32)
+    Y = np.empty((ncoarse * nfine, ns), dtype=np.uint32)
+    rc = _load_mt().oracle_mt_subband(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), ctypes.c_int(nsub),
+                                      _p(d1), ctypes.c_int(ncoarse), ctypes.c_int(ns1), _p(S), ctypes.c_size_t(ns1),
+                                      _p(d2), ctypes.c_int(nfine), ctypes.c_int(ns), _p(Y), ctypes.c_size_t(ns))
+    if rc != 0:
+        raise ValueError("oracle_mt_subband rc=%d" % rc)
+    return S, Y
+
+
+def search_mt(Y: np.ndarray, widths: Sequence[int], ddof: int = 0):
+    """integrate + snr for every width with the rows spread over the cores: (planes, snr, argmax)."""
+    assert Y.dtype == np.uint32 and Y.ndim == 2 and Y.flags.c_contiguous
+    L = _load_mt()
+    planes, S, A = {}, [], []
+    nrows, ns = Y.shape
+    for w in widths:
+        if w == 1:
+            I = Y
+        else:
+            nw = ns // w
+            I = np.empty((nrows, nw), dtype=np.uint32)
+            rc = L.oracle_mt_integrate(_p(Y), ctypes.c_size_t(ns), ctypes.c_int(nrows), ctypes.c_int(ns),
+                                       ctypes.c_int(w), _p(I), ctypes.c_size_t(max(nw, 1)))
+            if rc != 0:
+                raise ValueError("oracle_mt_integrate rc=%d" % rc)
+        planes[w] = I
+        s = np.empty(nrows, dtype=np.float32)
+        a = np.empty(nrows, dtype=np.uint32)
+        rc = L.oracle_mt_snr(_p(I), ctypes.c_size_t(I.shape[1]), ctypes.c_int(nrows), ctypes.c_int(I.shape[1]),
+                             ctypes.c_int(ddof), _p(s), _p(a))
+        if rc != 0:
+            raise ValueError("oracle_mt_snr rc=%d" % rc)
         S.append(s)
         A.append(a)
     return planes, np.stack(S, axis=1), np.stack(A, axis=1)

@@ -15,18 +15,6 @@
 #ifndef DDP_KERNELS_CUH_
 #define DDP_KERNELS_CUH_
 
-// How the packed dedispersion kernel accumulates its two 16-bit lane pairs (see ddp_dedisp_packed_body):
-// 0 both as IMAD, 1 both as IADD3, 2 one lane pair + a 64-bit IMAD.WIDE sum, 3 even lanes IADD3 and odd
-// lanes IMAD, 4 even lanes IADD3 and sum(w >> 8) by IMAD.HI.  Measured on B200 with the tuned shapes (dedispersion ms, cfg1 / cfg2 / cfg3):
-// mode 0 4.765 / 0.3746 / 21.41, mode 1 5.014 / 0.3865 / 22.62, mode 2 5.877 / 0.4278 / 29.86,
-// mode 3 4.684 / 0.3749 / 21.12, mode 4 (one extraction, w >> 8 summed by IMAD.HI; exact, parity green)
-// 5.455 / 0.4177 / 25.42: IMAD.HI takes a 64-bit addend and extra moves.  Mode 3 wins by issuing less, not by pipe balance: at cfg1 3.72 G warp
-// instructions instead of 4.03 G (1.55 vs 1.68 per add), with the alu pipe at 73 % and fma at 19 %
-// (mode 0: 60 % / 30 %), profiles/r01_final.md.
-#ifndef DDP_ACC_MODE
-#define DDP_ACC_MODE 3
-#endif
-
 typedef unsigned char ddp_u8;
 typedef unsigned short ddp_u16;
 typedef unsigned int ddp_u32;
@@ -541,23 +529,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     };
 
-    ddp_u32 accE[DPT][K];
-#if DDP_ACC_MODE == 2
-    ddp_u64 accT[DPT][K];  // exact 64-bit sum of the whole words; bytes 1,3 = (accT - accE) >> 8
-#else
-    ddp_u32 accO[DPT][K];
-#endif
+    ddp_u32 accE[DPT][K], accO[DPT][K];
 #pragma unroll
     for (int j = 0; j < DPT; ++j)
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
-            accE[j][k] = 0u;
-#if DDP_ACC_MODE == 2
-            accT[j][k] = 0ull;
-#else
-            accO[j][k] = 0u;
-#endif
-        }
+        for (int k = 0; k < K; ++k) accE[j][k] = accO[j][k] = 0u;
     const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
     const ddp_u32* lanep = (const ddp_u32*)ddp_smem + wb;
     // Unpacks the 16-bit lanes into the thread's own output words (ADD: on top of what an earlier
@@ -572,13 +548,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_u16* orow = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-#if DDP_ACC_MODE == 2
-                    const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
-#elif DDP_ACC_MODE == 4  // accO holds sum(w >> 8) = b1 + 2^8 b2 + 2^16 b3 as one integer; b2 is accE's high lane
-                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);
-#else
                     const ddp_u32 oo = accO[j][k];
-#endif
                     const ddp_u32 lo = __byte_perm(accE[j][k], oo, 0x5410u), hi = __byte_perm(accE[j][k], oo, 0x7632u);
                     const int t = tile_t + 4 * (wb + 32 * k);
                     if (t + 3 < p.ns) {
@@ -594,13 +564,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-#if DDP_ACC_MODE == 2
-                    const ddp_u32 oo = (ddp_u32)((accT[j][k] - (ddp_u64)accE[j][k]) >> 8);
-#elif DDP_ACC_MODE == 4  // accO holds sum(w >> 8) = b1 + 2^8 b2 + 2^16 b3 as one integer; b2 is accE's high lane
-                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);
-#else
                     const ddp_u32 oo = accO[j][k];
-#endif
                     ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = oo & 0xffffu, v2 = accE[j][k] >> 16, v3 = oo >> 16;
                     const int t = tile_t + 4 * (wb + 32 * k);
                     if (t + 3 < p.ns) {
@@ -617,14 +581,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 }
             }
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                accE[j][k] = 0u;
-#if DDP_ACC_MODE == 2
-                accT[j][k] = 0ull;
-#else
-                accO[j][k] = 0u;
-#endif
-            }
+            for (int k = 0; k < K; ++k) accE[j][k] = accO[j][k] = 0u;
         }
     };
 
@@ -680,27 +637,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 w = wp[32 * k];
                     const ddp_u32 e = w & 0x00ff00ffu;
-#if DDP_ACC_MODE == 0  // extraction on the alu pipe, both accumulations as IMAD on the fma pipe
-                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
-                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accE[j][k]) : "r"(e), "r"(one));
-                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
-#elif DDP_ACC_MODE == 1  // plain adds (IADD3)
-                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
-                    accE[j][k] += e;
-                    accO[j][k] += o;
-#elif DDP_ACC_MODE == 4  // ONE extraction: even bytes as 16-bit lanes (IADD3), and w >> 8 summed as a plain
-                         // 32-bit integer by mad.hi(w, 2^24, acc): exact while rows x (2^24 - 1) < 2^32, i.e. for
-                         // the <= 256 rows between flushes; the odd-byte sums are recovered in emit()
-                    accE[j][k] += e;
-                    asm("mad.hi.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(w), "r"(one << 24));
-#elif DDP_ACC_MODE == 3  // even lanes IADD3, odd lanes IMAD
+                    // even lanes by IADD3 (alu pipe; ptxas folds two of them into one three-input add),
+                    // odd lanes by IMAD with a run-time 1 (fma pipe)
                     const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
                     accE[j][k] += e;
                     asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
-#else  // 2: one extraction only; the whole word goes into an exact 64-bit sum (IMAD.WIDE)
-                    accE[j][k] += e;
-                    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(accT[j][k]) : "r"(w), "r"(one));
-#endif
                 }
             }
         }

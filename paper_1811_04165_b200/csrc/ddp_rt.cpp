@@ -28,6 +28,7 @@
 
 extern const char* const ddp_kernel_source;  // generated: ddp_params.h + ddp_kernels.cuh as one string
 
+#define DDP_MAX_DEVICES 16
 #define DDP_STR2(x) #x
 #define DDP_STR(x) DDP_STR2(x)
 
@@ -75,7 +76,7 @@ struct Api {
     RTC(nvrtcGetErrorString)
 #undef RTC
     bool nvrtc_ok = false;
-    CUcontext ctx[16] = {nullptr};
+    CUcontext ctx[DDP_MAX_DEVICES] = {nullptr};
     bool inited = false;
 };
 Api g_api;
@@ -173,7 +174,7 @@ std::string cu_err(CUresult r) {
 ddp_status ensure_ctx(const ddp_plan* p, int device) {
     std::lock_guard<std::mutex> lk(g_api_mu);
     if (!load_cuda_locked()) return ddp_fail(p, DDP_E_CUDA, g_api.why);
-    if (device < 0 || device >= 16) return ddp_fail(p, DDP_E_ARG, "device ordinal out of range");
+    if (device < 0 || device >= DDP_MAX_DEVICES) return ddp_fail(p, DDP_E_ARG, "device ordinal out of range");
     if (!g_api.ctx[device]) {
         CUdevice dev;
         CUresult r = g_api.p_cuDeviceGet(&dev, device);
@@ -195,21 +196,27 @@ ddp_status ensure_ctx(const ddp_plan* p, int device) {
 struct DdpCompiled {
     std::string name;
     std::vector<char> cubin;  // device image (from NVRTC or the disk cache); empty for AOT functions
-    CUmodule mod = nullptr;
-    CUfunction fn = nullptr;
-    bool loaded = false;
+    bool aot = false;         // function of ddp_aot.cubin (looked up per device in the AOT module)
+    // A CUmodule / CUfunction belongs to the context that loaded it: one slot per device ordinal.
+    CUmodule mod[DDP_MAX_DEVICES] = {nullptr};
+    CUfunction fn[DDP_MAX_DEVICES] = {nullptr};
+    bool loaded[DDP_MAX_DEVICES] = {false};
+    int smem_opt_in[DDP_MAX_DEVICES];  // largest dynamic shared size already granted by cuFuncSetAttribute
     bool failed = false;
     std::string log;
     int regs = 0;
-    int smem_opt_in = -1;  // largest dynamic shared size already granted by cuFuncSetAttribute
+    DdpCompiled() {
+        for (int d = 0; d < DDP_MAX_DEVICES; ++d) smem_opt_in[d] = -1;
+    }
 };
 
 namespace {
 std::mutex g_reg_mu;
 std::unordered_map<std::string, DdpCompiled*> g_reg;
 std::atomic<int64_t> g_ncompiles{0};
-CUmodule g_aot_mod = nullptr;
-bool g_aot_tried = false;
+std::mutex g_load_mu;  // serialises module loads and the per-device AOT initialisation
+CUmodule g_aot_mod[DDP_MAX_DEVICES] = {nullptr};
+bool g_aot_tried[DDP_MAX_DEVICES] = {false};
 
 enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3, CK_DEDISP_U16 = 4 };
 CodeKind code_kind(const ddp_plan* p, ddp_kernel k) {
@@ -237,7 +244,7 @@ const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck 
 int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const CodeKind ck = code_kind(p, k);
     int f = 0;
-    if (ck == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 256) f |= 1;
+    if (ck == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 257) f |= 1;  // 257 * 255 = 65535 still fits the lanes
     if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
     if (ck == CK_DEDISP_U8 && ddp_u8_single_buffered(p, k, c)) f |= 16;
     if (ck == CK_DEDISP_U16 && c.staging != 0) {
@@ -427,46 +434,61 @@ DdpCompiled* obtain_image(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     return K;
 }
 
-// Loads the image into the current context (caller holds the plan's context current).
+// AOT module of the plan's device (ddp_aot.cubin beside the library), loaded once per device.
+CUmodule aot_module_locked(int dev) {
+    if (!g_aot_tried[dev]) {
+        g_aot_tried[dev] = true;
+        std::vector<char> img;
+        if (read_file(lib_dir() + "/ddp_aot.cubin", img)) {
+            if (g_api.p_cuModuleLoadData(&g_aot_mod[dev], img.data()) != CUDA_SUCCESS) g_aot_mod[dev] = nullptr;
+        }
+    }
+    return g_aot_mod[dev];
+}
+
+// Loads the kernel into the context of the plan's device (current on the calling thread).
 ddp_status load_kernel(const ddp_plan* p, DdpCompiled* K) {
-    if (K->loaded) return DDP_OK;
+    const int dev = p->device;
+    std::lock_guard<std::mutex> lk(g_load_mu);
+    if (K->loaded[dev]) return DDP_OK;
     if (K->failed) return ddp_fail(p, DDP_E_COMPILE, K->name + ": " + K->log);
     CUresult r;
-    if (K->cubin.empty()) return ddp_fail(p, DDP_E_COMPILE, K->name + ": no device image");
-    r = g_api.p_cuModuleLoadData(&K->mod, K->cubin.data());
-    if (r != CUDA_SUCCESS) {
-        K->failed = true;
-        K->log = "cuModuleLoadData: " + cu_err(r);
-        return ddp_fail(p, DDP_E_COMPILE, K->name + ": " + K->log);
+    if (K->aot) {
+        CUmodule m = aot_module_locked(dev);
+        if (!m || g_api.p_cuModuleGetFunction(&K->fn[dev], m, K->name.c_str()) != CUDA_SUCCESS || !K->fn[dev])
+            return ddp_fail(p, DDP_E_COMPILE, K->name + ": not in ddp_aot.cubin on this device");
+    } else {
+        if (K->cubin.empty()) return ddp_fail(p, DDP_E_COMPILE, K->name + ": no device image");
+        r = g_api.p_cuModuleLoadData(&K->mod[dev], K->cubin.data());
+        if (r != CUDA_SUCCESS) {
+            K->failed = true;
+            K->log = "cuModuleLoadData: " + cu_err(r);
+            return ddp_fail(p, DDP_E_COMPILE, K->name + ": " + K->log);
+        }
+        r = g_api.p_cuModuleGetFunction(&K->fn[dev], K->mod[dev], K->name.c_str());
+        if (r != CUDA_SUCCESS) {
+            K->failed = true;
+            K->log = "cuModuleGetFunction: " + cu_err(r);
+            return ddp_fail(p, DDP_E_COMPILE, K->name + ": " + K->log);
+        }
     }
-    r = g_api.p_cuModuleGetFunction(&K->fn, K->mod, K->name.c_str());
-    if (r != CUDA_SUCCESS) {
-        K->failed = true;
-        K->log = "cuModuleGetFunction: " + cu_err(r);
-        return ddp_fail(p, DDP_E_COMPILE, K->name + ": " + K->log);
-    }
-    g_api.p_cuFuncGetAttribute(&K->regs, CU_FUNC_ATTRIBUTE_NUM_REGS, K->fn);
-    K->loaded = true;
+    g_api.p_cuFuncGetAttribute(&K->regs, CU_FUNC_ATTRIBUTE_NUM_REGS, K->fn[dev]);
+    K->loaded[dev] = true;
     return DDP_OK;
 }
 
 // AOT lookup: a function of this exact name in ddp_aot.cubin needs no NVRTC at all.
-DdpCompiled* obtain_aot(const std::string& name) {
-    if (!g_aot_tried) {
-        g_aot_tried = true;
-        std::vector<char> img;
-        if (read_file(lib_dir() + "/ddp_aot.cubin", img)) {
-            if (g_api.p_cuModuleLoadData(&g_aot_mod, img.data()) != CUDA_SUCCESS) g_aot_mod = nullptr;
-        }
+DdpCompiled* obtain_aot(const ddp_plan* p, const std::string& name) {
+    {
+        std::lock_guard<std::mutex> lk(g_load_mu);
+        CUmodule m = aot_module_locked(p->device);
+        if (!m) return nullptr;
+        CUfunction fn = nullptr;
+        if (g_api.p_cuModuleGetFunction(&fn, m, name.c_str()) != CUDA_SUCCESS || !fn) return nullptr;
     }
-    if (!g_aot_mod) return nullptr;
-    CUfunction fn = nullptr;
-    if (g_api.p_cuModuleGetFunction(&fn, g_aot_mod, name.c_str()) != CUDA_SUCCESS || !fn) return nullptr;
     DdpCompiled* K = new DdpCompiled();
     K->name = name;
-    K->fn = fn;
-    K->loaded = true;
-    g_api.p_cuFuncGetAttribute(&K->regs, CU_FUNC_ATTRIBUTE_NUM_REGS, fn);
+    K->aot = true;
     std::lock_guard<std::mutex> lk(g_reg_mu);
     auto it = g_reg.find(name);
     if (it != g_reg.end()) {
@@ -486,15 +508,16 @@ ddp_status get_kernel(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, DdpCom
         auto it = g_reg.find(name);
         if (it != g_reg.end()) K = it->second;
     }
-    if (!K) K = obtain_aot(name);
+    if (!K) K = obtain_aot(p, name);
     if (!K) K = obtain_image(p, k, c);
     ddp_status s = load_kernel(p, K);
     if (s != DDP_OK) return s;
+    const int dev = p->device;
     const int smem = (int)ddp_smem_bytes(p, k, c);
-    if (smem > 48 * 1024 && smem > K->smem_opt_in) {
-        CUresult r = g_api.p_cuFuncSetAttribute(K->fn, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, smem);
+    if (smem > 48 * 1024 && smem > K->smem_opt_in[dev]) {
+        CUresult r = g_api.p_cuFuncSetAttribute(K->fn[dev], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, smem);
         if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, K->name + ": shared-memory opt-in: " + cu_err(r));
-        K->smem_opt_in = smem;
+        K->smem_opt_in[dev] = smem;
     }
     *out = K;
     return DDP_OK;
@@ -636,7 +659,7 @@ ddp_status launch(const ddp_plan* p, DdpCompiled* K, unsigned gx, unsigned gy, u
     if (gx == 0 || gy == 0 || gz == 0 || gy > 65535u || gz > 65535u)
         return ddp_fail(p, DDP_E_CONFIG, K->name + ": grid outside the launch limits");
     void* args[] = {params};
-    CUresult r = g_api.p_cuLaunchKernel(K->fn, gx, gy, gz, bx, by, 1, (unsigned)smem, st, args, nullptr);
+    CUresult r = g_api.p_cuLaunchKernel(K->fn[p->device], gx, gy, gz, bx, by, 1, (unsigned)smem, st, args, nullptr);
     if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, K->name + ": cuLaunchKernel: " + cu_err(r));
     return DDP_OK;
 }

@@ -1,16 +1,28 @@
 // Instruction-rate micro-benchmarks behind the dedispersion add roofline (
 // "the per-SM integer-add rate of sm_100 is not in MEASURED_PEAKS.json and must be
-// measured on the box").  Standalone: build.py compiles it with nvcc for sm_100a into `ddp_ubench`;
-// `ddp_ubench` prints one JSON object with, per instruction mix, thread-operations per clock per SM:
-// "thread_ops_per_clk_per_sm_wall" = all thread-operations of the launch / CUDA-event time / (SMs x the
-// device's SM clock) -- the figure to use (B200, 1965 MHz: IADD3 126-127, LOP3 / PRMT / IMAD / IDP.4A 63.7) --
-// and "thread_ops_per_clk_per_sm" from clock64 deltas inside the kernel, which on B200 comes out 1.34x
-// higher than the wall-clock figure for every mix (cause not investigated) and is kept only for
-// comparison.  Nothing of the search is computed here.
+// measured on the box").  Standalone: build.py compiles it with nvcc for sm_100a into `ddp_ubench`
+// and then CHECKS THE SASS of every kernel (cuobjdump): the loop body must hold exactly NCH
+// instructions of the opcode(s) under test plus the loop counter, compare and branch -- ptxas fuses
+// dependent `add.u32` pairs into one three-input IADD3 and merges or hoists anything that is not
+// loop carried, which is how round 1 misread "127 adds per clock" as "127 IADD3 per clock".
+//
+// Construction that cannot be folded: NCH independent dependency chains per thread, ONE instruction
+// per chain per iteration of a loop that is not unrolled (`#pragma unroll 1`), every instruction
+// loop carried through its own chain register.  Mixes alternate two opcodes chain by chain, so a
+// mix that reaches ~2x the single-opcode rate shows that the two opcodes issue to different pipes.
+//
+// One block of 512 threads per SM (a 120 KB dynamic shared-memory request keeps a second block off
+// the SM); the SM clock is measured inside the kernel (clock64 against globaltimer), so the rates do
+// not depend on what nvidia-smi reports.  Output: one JSON object; per kernel
+//   "inst_per_clk_per_sm"  thread-instructions of the loop body (NCH + 3) x iterations x threads /
+//                          (kernel time x measured SM clock), per SM
+//   "adds_per_clk_per_sm"  for the add kernels: scalar 32-bit additions performed, same denominator.
+// Nothing of the search is computed here.
 #include <cuda_runtime.h>
 
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <vector>
 
 #define CK(x)                                                                          \
@@ -22,150 +34,187 @@
         }                                                                              \
     } while (0)
 
-enum Mix { M_IADD3, M_LOP3, M_PRMT, M_IMAD, M_IMADWIDE, M_DP4A, M_LOOP_NOLDS, M_LDS32, M_LOOP,
-           M_LOP3_IADD3, M_LOP3_PRMT_2IADD3, M_T_NOLDS, M_T, M_COUNT };
-static const char* kNames[M_COUNT] = {"iadd3", "lop3", "prmt", "imad", "imad_wide", "idp4a",
-                                      "lop3_prmt_2imad", "lds32", "lds32_lop3_prmt_2imad",
-                                      "lop3_iadd3", "lop3_prmt_2iadd3", "lop3_iadd3_imadwide", "lds32_lop3_iadd3_imadwide"};
-// thread-operations per loop body (8 independent chains x 8 repeats of the pattern)
-static const int kOpsPerBody[M_COUNT] = {64, 64, 64, 64, 64, 64, 64 * 4, 64, 64 * 5, 64 * 2, 64 * 4, 64 * 3, 64 * 4};
+#define NCH 96      // independent chains per thread = instructions under test per loop iteration
+#define THREADS 512
+#define SMEM_WORDS 8192
 
-template <int MIX>
-__global__ void __launch_bounds__(512, 2) ubench(unsigned* out, unsigned long long* cycles, int iters, unsigned one,
-                                               unsigned seed) {
-    __shared__ unsigned sm[2048];
-    for (int i = threadIdx.x; i < 2048; i += blockDim.x) sm[i] = seed * (unsigned)i + 12345u;
-    __syncthreads();
-    unsigned a[8], b[8], c[8];
-    unsigned long long w[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        a[k] = seed + threadIdx.x * 8 + k;
-        b[k] = a[k] ^ 0x9e3779b9u;
-        w[k] = a[k];
-        c[k] = b[k] + 3u;
-    }
-    const unsigned lp = (unsigned)__cvta_generic_to_shared(sm + (threadIdx.x & 511));
-    const long long c0 = clock64();
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if constexpr (MIX == M_IADD3) {
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(a[k]) : "r"(b[k]));
-                } else if constexpr (MIX == M_LOP3) {
-                    asm volatile("lop3.b32 %0, %0, %1, 0x00ff00ff, 0x6a;" : "+r"(a[k]) : "r"(b[k]));
-                } else if constexpr (MIX == M_PRMT) {
-                    asm volatile("prmt.b32 %0, %0, %1, 0x4341;" : "+r"(a[k]) : "r"(b[k]));
-                } else if constexpr (MIX == M_IMAD) {
-                    asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a[k]) : "r"(b[k]), "r"(one));
-                } else if constexpr (MIX == M_IMADWIDE) {
-                    asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w[k]) : "r"(b[k]), "r"(one));
-                } else if constexpr (MIX == M_DP4A) {
-                    asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(a[k]) : "r"(b[k]), "r"(one));
-                } else if constexpr (MIX == M_LOOP_NOLDS || MIX == M_LOOP || MIX == M_LDS32) {
-                    unsigned x = b[k];
-                    if constexpr (MIX != M_LOOP_NOLDS) {
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(x) : "r"(lp + 128u * ((r * 8 + k) & 31)));
-                    }
-                    if constexpr (MIX == M_LDS32) {
-                        asm volatile("add.u32 %0, %0, %1;" : "+r"(a[k]) : "r"(x));  // LDS + IADD3
-                    } else {
-                        unsigned e, o;
-                        asm volatile("and.b32 %0, %1, 0x00ff00ff;" : "=r"(e) : "r"(x));
-                        asm volatile("prmt.b32 %0, %1, 0, 0x4341;" : "=r"(o) : "r"(x));
-                        asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a[k]) : "r"(e), "r"(one));
-                        asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(b[k]) : "r"(o), "r"(one));
-                    }
-                } else if constexpr (MIX == M_LOP3_IADD3) {
-                    unsigned e;
-                    asm volatile("and.b32 %0, %1, 0x00ff00ff;" : "=r"(e) : "r"(b[k]));
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(a[k]) : "r"(e));
-                } else if constexpr (MIX == M_LOP3_PRMT_2IADD3) {
-                    unsigned e, o;
-                    asm volatile("and.b32 %0, %1, 0x00ff00ff;" : "=r"(e) : "r"(b[k]));
-                    asm volatile("prmt.b32 %0, %1, 0, 0x4341;" : "=r"(o) : "r"(b[k]));
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(a[k]) : "r"(e));
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(c[k]) : "r"(o));
-                } else if constexpr (MIX == M_T_NOLDS || MIX == M_T) {
-                    unsigned x = b[k], e;
-                    if constexpr (MIX == M_T) {
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(x) : "r"(lp + 128u * ((r * 8 + k) & 31)));
-                    }
-                    asm volatile("and.b32 %0, %1, 0x00ff00ff;" : "=r"(e) : "r"(x));
-                    asm volatile("add.u32 %0, %0, %1;" : "+r"(a[k]) : "r"(e));
-                    asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w[k]) : "r"(x), "r"(one));
-                }
-            }
-        }
-    }
-    const long long c1 = clock64();
-    unsigned acc = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) acc += a[k] + b[k] + c[k] + (unsigned)w[k] + (unsigned)(w[k] >> 32);
-    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
-    if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(c1 - c0);
+enum Mix {
+    M_IADD_2IN,    // a += b                      -> IADD3 with one zero input (one add per instruction)
+    M_IADD3_3IN,   // a += b; a += c (two PTX adds, fused by ptxas) -> IADD3, three live inputs (two adds)
+    M_LOP3,        // a = a ^ b ^ c
+    M_PRMT,        // a = prmt(a, b, sel)
+    M_IMAD,        // a = b * one + a             -> IMAD
+    M_IDP4A,       // a = dp4a(b, one, a)         -> IDP.4A
+    M_IMAD_IMM,    // a = b * 3 + a               -> IMAD with an immediate multiplier
+    M_IADD3_IMAD,  // even chains IADD3 (three inputs), odd chains IMAD
+    M_LOP3_IMAD,
+    M_PRMT_IMAD,
+    M_LOP3_IDP4A,
+    M_PRMT_IDP4A,
+    M_LOP3_PRMT,   // both on the alu pipe: must NOT exceed the single-opcode rate
+    M_LDS32,       // x = lds[x]: loop-carried, conflict-free 32-bit shared loads
+    M_LDS32_IADD3, // even chains LDS.32, odd chains IADD3 (three inputs)
+    M_COUNT
+};
+static const char* kNames[M_COUNT] = {"iadd_2in", "iadd3_3in", "lop3", "prmt", "imad", "idp4a", "imad_imm", "iadd3_imad",
+                                      "lop3_imad", "prmt_imad", "lop3_idp4a", "prmt_idp4a", "lop3_prmt", "lds32",
+                                      "lds32_iadd3"};
+// scalar 32-bit additions per loop iteration (0 = not an add kernel)
+static const int kAdds[M_COUNT] = {NCH, 2 * NCH, 0, 0, NCH, NCH, NCH, 2 * (NCH / 2) + NCH / 2, 0, 0, 0, 0, 0, 0, 0};
+
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
 }
 
-static double g_clock_hz = 0.0;  // SM clock used for the wall-clock figure (cudaDeviceProp::clockRate)
-static double g_wall[M_COUNT];
+template <int MIX>
+__device__ __forceinline__ void chain_op(unsigned& a, int k, unsigned b, unsigned c, unsigned one, unsigned sbase) {
+    const bool odd = (k & 1) != 0;
+    if constexpr (MIX == M_IADD_2IN) {
+        asm volatile("add.u32 %0, %0, %1;" : "+r"(a) : "r"(b));
+    } else if constexpr (MIX == M_IADD3_3IN) {
+        asm volatile("add.u32 %0, %0, %1;\n\tadd.u32 %0, %0, %2;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_LOP3) {
+        asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_PRMT) {
+        asm volatile("prmt.b32 %0, %0, %1, 0x4341;" : "+r"(a) : "r"(b));
+    } else if constexpr (MIX == M_IMAD) {
+        asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+    } else if constexpr (MIX == M_IDP4A) {
+        asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+    } else if constexpr (MIX == M_IMAD_IMM) {
+        asm volatile("mad.lo.u32 %0, %1, 3, %0;" : "+r"(a) : "r"(b));
+    } else if constexpr (MIX == M_IADD3_IMAD) {
+        if (odd) asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+        else asm volatile("add.u32 %0, %0, %1;\n\tadd.u32 %0, %0, %2;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_LOP3_IMAD) {
+        if (odd) asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+        else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_PRMT_IMAD) {
+        if (odd) asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+        else asm volatile("prmt.b32 %0, %0, %1, 0x4341;" : "+r"(a) : "r"(b));
+    } else if constexpr (MIX == M_LOP3_IDP4A) {
+        if (odd) asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+        else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_PRMT_IDP4A) {
+        if (odd) asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(a) : "r"(b), "r"(one));
+        else asm volatile("prmt.b32 %0, %0, %1, 0x4341;" : "+r"(a) : "r"(b));
+    } else if constexpr (MIX == M_LOP3_PRMT) {
+        if (odd) asm volatile("prmt.b32 %0, %0, %1, 0x4341;" : "+r"(a) : "r"(b));
+        else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a) : "r"(b), "r"(c));
+    } else if constexpr (MIX == M_LDS32) {
+        asm volatile("ld.shared.u32 %0, [%0];" : "+r"(a) : : "memory");
+    } else if constexpr (MIX == M_LDS32_IADD3) {
+        if (odd) asm volatile("add.u32 %0, %0, %1;\n\tadd.u32 %0, %0, %2;" : "+r"(a) : "r"(b), "r"(c));
+        else asm volatile("ld.shared.u32 %0, [%0];" : "+r"(a) : : "memory");
+    }
+    (void)sbase;
+}
 
 template <int MIX>
-static void run(int nsm, int iters, unsigned* d_out, unsigned long long* d_cyc, double* ops_clk_sm, double* ms_out) {
-    const int blocks = 2 * nsm, threads = 512;  // two co-resident blocks per SM: 8 warps per scheduler
-    ubench<MIX><<<blocks, threads>>>(d_out, d_cyc, 16, 1u, 7u);  // warm-up
+__global__ void __launch_bounds__(THREADS, 1) ubench(unsigned* out, unsigned long long* stamps, int iters, unsigned one,
+                                                     unsigned seed) {
+    extern __shared__ __align__(16) unsigned sm[];
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(sm);
+    // sm[i] = shared-memory BYTE ADDRESS of word (i + 32 * 37) mod SMEM_WORDS: a permutation that keeps
+    // the bank (i mod 32), so a warp whose lanes start in distinct banks never conflicts.
+    for (int i = threadIdx.x; i < SMEM_WORDS; i += blockDim.x) sm[i] = sbase + 4u * ((i + 32 * 37) % SMEM_WORDS);
+    __syncthreads();
+    unsigned a[NCH];
+    const bool lds_kernel = MIX == M_LDS32 || MIX == M_LDS32_IADD3;
+#pragma unroll
+    for (int k = 0; k < NCH; ++k) {
+        const bool lds_chain = MIX == M_LDS32 || (MIX == M_LDS32_IADD3 && (k & 1) == 0);
+        a[k] = lds_chain ? sbase + 4u * ((threadIdx.x & 31) + 32u * (((threadIdx.x >> 5) * 7 + k * 13) % (SMEM_WORDS / 32)))
+                         : seed + threadIdx.x * NCH + k;
+    }
+    (void)lds_kernel;
+    const unsigned b = seed ^ 0x9e3779b9u ^ threadIdx.x, c = b * 5u + 3u;
+    __syncthreads();
+    const unsigned long long g0 = gtimer();
+    const long long c0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < NCH; ++k) chain_op<MIX>(a[k], k, b, c, one, sbase);
+    }
+    const long long c1 = clock64();
+    const unsigned long long g1 = gtimer();
+    unsigned acc = 0;
+#pragma unroll
+    for (int k = 0; k < NCH; ++k) acc ^= a[k];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+    if (threadIdx.x == 0) {
+        stamps[2 * blockIdx.x] = (unsigned long long)(c1 - c0);
+        stamps[2 * blockIdx.x + 1] = g1 - g0;
+    }
+}
+
+struct Result { double ms, sm_mhz, inst_rate, add_rate; };
+
+template <int MIX>
+static Result run(int nsm, int iters, unsigned* d_out, unsigned long long* d_st) {
+    const size_t smem = 120 * 1024;  // > half of the SM's shared memory: at most one block per SM
+    CK(cudaFuncSetAttribute(ubench<MIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ubench<MIX><<<nsm, THREADS, smem>>>(d_out, d_st, 64, 1u, 7u);  // warm-up
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
     CK(cudaEventRecord(e0));
-    ubench<MIX><<<blocks, threads>>>(d_out, d_cyc, iters, 1u, 7u);
+    ubench<MIX><<<nsm, THREADS, smem>>>(d_out, d_st, iters, 1u, 7u);
     CK(cudaEventRecord(e1));
     CK(cudaEventSynchronize(e1));
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, e0, e1));
-    std::vector<unsigned long long> cyc(blocks);
-    CK(cudaMemcpy(cyc.data(), d_cyc, blocks * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
-    double mean = 0.0;
-    for (auto c : cyc) mean += (double)c;
-    mean /= blocks;
-    *ops_clk_sm = 2.0 * (double)kOpsPerBody[MIX] * iters * threads / mean;  // two blocks share an SM
-    g_wall[MIX] = (double)blocks * threads * (double)kOpsPerBody[MIX] * iters / (ms * 1e-3) / (nsm * g_clock_hz);
-    *ms_out = ms;
+    std::vector<unsigned long long> st(2 * nsm);
+    CK(cudaMemcpy(st.data(), d_st, st.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    double cyc = 0.0, ns = 0.0;
+    for (int i = 0; i < nsm; ++i) { cyc += (double)st[2 * i]; ns += (double)st[2 * i + 1]; }
+    Result r;
+    r.ms = ms;
+    r.sm_mhz = cyc / ns * 1e3;  // SM cycles per nanosecond of the in-kernel timed region
+    // per-SM rates from the in-kernel cycle count of the block that ran on each SM (mean over SMs)
+    const double cycles_per_block = cyc / nsm;
+    r.inst_rate = (double)(NCH + 3) * iters * THREADS / cycles_per_block;
+    r.add_rate = (double)kAdds[MIX] * iters * THREADS / cycles_per_block;
     CK(cudaEventDestroy(e0));
     CK(cudaEventDestroy(e1));
+    return r;
 }
 
 int main(int argc, char** argv) {
-    const int iters = argc > 1 ? std::atoi(argv[1]) : 4096;
+    const int iters = argc > 1 ? std::atoi(argv[1]) : 8192;
+    const char* only = argc > 2 ? argv[2] : nullptr;  // run one kernel only (for ncu)
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, 0));
     const int nsm = prop.multiProcessorCount;
-    g_clock_hz = (double)prop.clockRate * 1e3;
     unsigned* d_out;
-    unsigned long long* d_cyc;
-    CK(cudaMalloc(&d_out, (size_t)nsm * 1024 * sizeof(unsigned)));
-    CK(cudaMalloc(&d_cyc, (size_t)2 * nsm * sizeof(unsigned long long)));
-    double r[M_COUNT], ms[M_COUNT];
-    run<M_IADD3>(nsm, iters, d_out, d_cyc, &r[M_IADD3], &ms[M_IADD3]);
-    run<M_LOP3>(nsm, iters, d_out, d_cyc, &r[M_LOP3], &ms[M_LOP3]);
-    run<M_PRMT>(nsm, iters, d_out, d_cyc, &r[M_PRMT], &ms[M_PRMT]);
-    run<M_IMAD>(nsm, iters, d_out, d_cyc, &r[M_IMAD], &ms[M_IMAD]);
-    run<M_IMADWIDE>(nsm, iters, d_out, d_cyc, &r[M_IMADWIDE], &ms[M_IMADWIDE]);
-    run<M_DP4A>(nsm, iters, d_out, d_cyc, &r[M_DP4A], &ms[M_DP4A]);
-    run<M_LOOP_NOLDS>(nsm, iters, d_out, d_cyc, &r[M_LOOP_NOLDS], &ms[M_LOOP_NOLDS]);
-    run<M_LDS32>(nsm, iters, d_out, d_cyc, &r[M_LDS32], &ms[M_LDS32]);
-    run<M_LOOP>(nsm, iters, d_out, d_cyc, &r[M_LOOP], &ms[M_LOOP]);
-    run<M_LOP3_IADD3>(nsm, iters, d_out, d_cyc, &r[M_LOP3_IADD3], &ms[M_LOP3_IADD3]);
-    run<M_LOP3_PRMT_2IADD3>(nsm, iters, d_out, d_cyc, &r[M_LOP3_PRMT_2IADD3], &ms[M_LOP3_PRMT_2IADD3]);
-    run<M_T_NOLDS>(nsm, iters, d_out, d_cyc, &r[M_T_NOLDS], &ms[M_T_NOLDS]);
-    run<M_T>(nsm, iters, d_out, d_cyc, &r[M_T], &ms[M_T]);
-    std::printf("{\"device\": \"%s\", \"sms\": %d, \"iters\": %d, \"thread_ops_per_clk_per_sm\": {", prop.name, nsm, iters);
-    for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.2f", m ? ", " : "", kNames[m], r[m]);
-    std::printf("}, \"sm_clock_mhz\": %.0f, \"thread_ops_per_clk_per_sm_wall\": {", g_clock_hz / 1e6);
-    for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.2f", m ? ", " : "", kNames[m], g_wall[m]);
-    std::printf("}, \"kernel_ms\": {");
-    for (int m = 0; m < M_COUNT; ++m) std::printf("%s\"%s\": %.4f", m ? ", " : "", kNames[m], ms[m]);
+    unsigned long long* d_st;
+    CK(cudaMalloc(&d_out, (size_t)nsm * THREADS * sizeof(unsigned)));
+    CK(cudaMalloc(&d_st, (size_t)2 * nsm * sizeof(unsigned long long)));
+    Result r[M_COUNT];
+    bool ran[M_COUNT] = {false};
+#define RUN(M)                                                        \
+    if (!only || std::strcmp(only, kNames[M]) == 0) {                 \
+        r[M] = run<M>(nsm, iters, d_out, d_st);                       \
+        ran[M] = true;                                                \
+    }
+    RUN(M_IADD_2IN) RUN(M_IADD3_3IN) RUN(M_LOP3) RUN(M_PRMT) RUN(M_IMAD) RUN(M_IDP4A) RUN(M_IMAD_IMM) RUN(M_IADD3_IMAD)
+    RUN(M_LOP3_IMAD) RUN(M_PRMT_IMAD) RUN(M_LOP3_IDP4A) RUN(M_PRMT_IDP4A) RUN(M_LOP3_PRMT) RUN(M_LDS32)
+    RUN(M_LDS32_IADD3)
+#undef RUN
+    std::printf("{\"device\": \"%s\", \"sms\": %d, \"iters\": %d, \"threads_per_sm\": %d, \"chains\": %d, \"kernels\": {",
+                prop.name, nsm, iters, THREADS, NCH);
+    bool first = true;
+    for (int m = 0; m < M_COUNT; ++m) {
+        if (!ran[m]) continue;
+        std::printf("%s\"%s\": {\"ms\": %.4f, \"sm_mhz\": %.1f, \"inst_per_clk_per_sm\": %.2f", first ? "" : ", ", kNames[m],
+                    r[m].ms, r[m].sm_mhz, r[m].inst_rate);
+        if (kAdds[m]) std::printf(", \"adds_per_clk_per_sm\": %.2f", r[m].add_rate);
+        std::printf("}");
+        first = false;
+    }
     std::printf("}}\n");
     return 0;
 }

@@ -19,9 +19,7 @@ def beams_of_rank(n_beams: int, rank: int, world: int) -> List[int]:
     return list(range(lo, lo + base + (1 if rank < extra else 0)))
 
 
-def beam_seed(data_seed: int, beam: int) -> int:
-    """Seed of the synthetic filterbank of one beam (beam 0 = the config's own seed)."""
-    return int(data_seed) + 7919 * int(beam)
+from synth.filterbank import beam_seed  # noqa: E402,F401  (data recipe: lives with the generator)
 
 
 def combine(local_ms: float, local_units: float, device=None) -> Tuple[float, float]:

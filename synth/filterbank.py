@@ -89,6 +89,11 @@ def noise_rows(seed: int, c0: int, c1: int, nsamp: int) -> np.ndarray:
     return out[:, :nsamp]
 
 
+def beam_seed(data_seed: int, beam: int) -> int:
+    """Seed of the synthetic filterbank of one beam (beam 0 = the config's own seed)."""
+    return int(data_seed) + 7919 * int(beam)
+
+
 def draw_pulses(cfg: SearchConfig) -> List[Pulse]:
     """The config's pulse list: fixed pulses, plus `n_pulses` hash-drawn ones with the DM on
     the trial grid, width in {1,2,4,8,16,32} (restricted to the config's widths), start a

@@ -5,6 +5,9 @@ The CUDA path and the oracle share only the input generator (synth/, data only).
 """
 from __future__ import annotations
 
+import json
+import os
+
 import numpy as np
 
 import oracle
@@ -12,6 +15,13 @@ import paper_1811_04165_b200 as ddp
 from synth import filterbank
 
 SNR_RTOL = 1e-5  # BASELINE.json north_star: "SNR within 1e-5 relative"
+TUNED_JSON = os.path.join(os.path.dirname(os.path.abspath(ddp.__file__)), "tuned_b200.json")
+
+
+def tuned_shapes(workload):
+    """{kernel name: gene list} of the workload in tuned_b200.json -- the shapes bench.py times."""
+    with open(TUNED_JSON) as fh:
+        return json.load(fh).get(workload, {})
 
 
 def u32(t) -> np.ndarray:
@@ -36,6 +46,18 @@ class GpuSearch:
         self.X = X
         self.buf["d_in"].copy_(torch.from_numpy(X))
         torch.cuda.synchronize()
+
+    def apply_tuned(self, workload):
+        """Sets every kernel slot to its shape in tuned_b200.json (what bench.py runs); a shape that is
+        not valid for the plan is a test failure, not a skip."""
+        applied = {}
+        for kname, genes in tuned_shapes(workload).items():
+            k = ddp.KERNEL_NAMES.index(kname)
+            c = ddp.Kcfg(*genes)
+            assert self.plan.check_kcfg(k, c), "tuned %s %r is not valid for %s" % (kname, genes, workload)
+            self.plan.set_kcfg(k, c)
+            applied[kname] = genes
+        return applied
 
     def upload(self):
         """Re-uploads self.X after the test changed it in place."""
@@ -120,6 +142,24 @@ def oracle_search(Y, widths, ddof=0):
     return oracle.search(np.ascontiguousarray(Y), widths, ddof)
 
 
+# all-cores legs (oracle_mt.cpp: the same single-thread functions, rows spread over the host cores) --
+# what makes every row of the full-size configs affordable
+def oracle_direct_all_rows_mt(cfg, X, rows=None):
+    dms = cfg.dm_list()
+    if rows is not None:
+        dms = dms[np.asarray(rows)]
+    delay = oracle.delay_table(cfg.chan_freq_mhz(), dms, cfg.t_samp_s)
+    return oracle.dedisperse_mt(np.ascontiguousarray(X), delay, cfg.nsamp_out)
+
+
+def oracle_subband_mt(cfg, X):
+    sb = cfg.subband
+    A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+    F = sb.fine_step * np.arange(sb.n_fine)
+    d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F)
+    return oracle.subband_mt(np.ascontiguousarray(X), d1, d2, sb.n_subbands, cfg.nsamp_out)
+
+
 def assert_snr_close(gpu, ref, what=""):
     gpu = np.asarray(gpu, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
@@ -129,7 +169,7 @@ def assert_snr_close(gpu, ref, what=""):
         what, np.argwhere(bad)[:5].tolist(), gpu[bad][:5], ref[bad][:5])
 
 
-def compare_all(g: GpuSearch, Yo, rows=None, what=""):
+def compare_all(g: GpuSearch, Yo, rows=None, what="", ddof=0, mt=False):
     """Full element-by-element comparison of the CUDA results (already computed in g's buffers)
     against the oracle chain applied to the oracle's own dedispersed rows Yo."""
     i = g.info
@@ -143,7 +183,7 @@ def compare_all(g: GpuSearch, Yo, rows=None, what=""):
         Pg = {w: p[rows] for w, p in Pg.items()}
     assert Yg.shape == Yo.shape
     assert np.array_equal(Yg, Yo), "%s dedispersion differs (bit-exact required)" % what
-    Po, So, Ao = oracle_search(Yo, widths, 0)
+    Po, So, Ao = (oracle.search_mt if mt else oracle.search)(np.ascontiguousarray(Yo), widths, ddof)
     for w in widths:
         if w > 1:
             assert np.array_equal(Pg[w], Po[w]), "%s integration plane w=%d differs" % (what, w)

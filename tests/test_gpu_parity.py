@@ -17,8 +17,8 @@ import paper_1811_04165_b200 as ddp  # noqa: E402
 from synth import configs  # noqa: E402
 from synth.configs import SubbandPlan  # noqa: E402
 
-from gpu_common import (GpuSearch, assert_snr_close, compare_all, oracle_direct_rows, oracle_search,  # noqa: E402
-                        oracle_subband, u32)
+from gpu_common import (GpuSearch, assert_snr_close, compare_all, oracle_direct_all_rows_mt,  # noqa: E402
+                        oracle_direct_rows, oracle_search, oracle_subband, oracle_subband_mt, tuned_shapes, u32)
 
 
 def small_direct(**kw):
@@ -125,6 +125,101 @@ def test_error_behaviour():
     plan.destroy()
 
 
+# ---------------------------------------------------------------------------------- API corners
+def test_snr_ddof_one_matches_the_oracle():
+    """SNR.2: snr_ddof = 1 (sample standard deviation) against oracle.snr(ddof=1); short series so that
+    the two readings differ by far more than the tolerance (0.5 % at n = 95)."""
+    cfg = small_direct(name="ddof1", nchan=48, nsamp_out=1530, ndm=21, widths=(1, 2, 4, 8, 16), n_pulses=2)
+    g = GpuSearch(cfg, snr_ddof=1)
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="ddof=1", ddof=1)
+    _, S0, _ = oracle_search(Yo, list(cfg.widths), 0)
+    S1 = g.buf["d_snr"].cpu().numpy()
+    assert np.all(np.abs(S1 - S0) > 1e-5 * np.abs(S0)), "ddof=1 result is indistinguishable from ddof=0"
+    g.close()
+
+
+@pytest.mark.parametrize("subband", [False, True])
+def test_search_host_end_to_end_call(subband):
+    """ddp_search_host (host buffers in, S/N + argmax out) against the oracle: cfg0 and a small subband plan."""
+    cfg = small_subband() if subband else configs.tiny()
+    g = GpuSearch(cfg)
+    i = g.info
+    g.buf["d_in"].zero_()                                   # the call must upload the filterbank itself
+    h_in = torch.from_numpy(g.X).pin_memory()
+    h_snr = torch.full((i.ndm, i.nwidths), -3.0, dtype=torch.float32).pin_memory()
+    h_arg = torch.full((i.ndm, i.nwidths), -1, dtype=torch.int32).pin_memory()
+    g.plan.search_host(h_in, g.buf["d_in"], g.buf["d_out"], g.buf["d_integ"], g.buf["d_snr"], g.buf["d_argmax"],
+                       h_snr, h_arg)                        # synchronises before returning
+    Yo = oracle_subband(cfg, g.X)[1] if subband else oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="search_host device side")
+    _, So, Ao = oracle_search(Yo, list(cfg.widths), 0)
+    assert_snr_close(h_snr.numpy(), So, "search_host host S/N")
+    assert np.array_equal(h_arg.numpy().view(np.uint32), Ao)
+    # pageable host memory and no argmax request
+    h_snr2 = np.full((i.ndm, i.nwidths), -3.0, dtype=np.float32)
+    g.plan.search_host(g.X, g.buf["d_in"], g.buf["d_out"], g.buf["d_integ"], g.buf["d_snr"], None, h_snr2, None)
+    assert_snr_close(h_snr2, So, "search_host pageable, no argmax")
+    g.close()
+
+
+def test_snr_without_argmax_wider_strides_and_a_side_stream():
+    """d_argmax = NULL; in/out strides larger than the minimum; a caller stream other than the current one."""
+    cfg = small_direct(name="strides", nchan=72, nsamp_out=2777, ndm=23, widths=(1, 2, 4, 8), n_pulses=2)
+    g = GpuSearch(cfg)
+    i = g.info
+    Yo = oracle_direct_rows(cfg, g.X)
+    _, So, Ao = oracle_search(Yo, list(cfg.widths), 0)
+    in_stride, out_stride = int(i.in_stride_min) + 48, int(i.out_stride_min) + 12
+    d_in = torch.full((i.nchan, in_stride), 255, dtype=torch.uint8, device="cuda")
+    d_in[:, : i.in_stride_min].copy_(torch.from_numpy(g.X))
+    d_out = torch.full((i.ndm, out_stride), -1, dtype=torch.int32, device="cuda")
+    d_snr = torch.full((i.ndm, i.nwidths), -7.0, dtype=torch.float32, device="cuda")
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        pass
+    g.plan.dedisperse(d_in, d_out, stream=side)
+    g.plan.integrate(d_out, g.buf["d_integ"], stream=side)
+    g.plan.snr(d_out, g.buf["d_integ"], d_snr, None, stream=side)
+    side.synchronize()
+    Yg = u32(d_out)
+    assert np.array_equal(Yg[:, : cfg.nsamp_out], Yo)
+    assert (Yg[:, i.out_stride_min:] == 0xFFFFFFFF).all(), "columns beyond out_stride_min were written"
+    assert_snr_close(d_snr.cpu().numpy(), So, "wide strides / side stream / no argmax")
+    # the same through the default-stream path with argmax, for the argmax comparison
+    g.plan.snr(d_out, g.buf["d_integ"], d_snr, g.buf["d_argmax"])
+    torch.cuda.synchronize()
+    assert np.array_equal(u32(g.buf["d_argmax"]), Ao)
+    g.close()
+
+
+def test_subband_257_channels_per_subband_runs_staged_with_the_uint16_intermediate():
+    """cps = 257 is the largest subband the uint16 intermediate holds exactly (257 * 255 = 65535): the packed
+    kernel must run it without the wide flush (WIDE and OUT16 used to be set together)."""
+    cfg = small_subband(name="cps257", nchan=514, nsamp_out=1200, ndm=3 * 4,
+                        subband=SubbandPlan(n_subbands=2, n_coarse=3, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=4, fine_step=0.25))
+    g = GpuSearch(cfg)
+    assert g.info.sub_elem_bytes == 2
+    g.X[:] = 255
+    g.upload()
+    c = g.plan.get_kcfg(ddp.K_SUB1)
+    assert c.staging != 0
+    Y = g.dedisperse()
+    assert np.all(g.subband_intermediate() == 255 * 257)
+    assert np.all(Y == 255 * 514)
+    g.close()
+    g = GpuSearch(cfg)
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    assert np.array_equal(g.subband_intermediate(), So)
+    compare_all(g, Yo, what="cps257")
+    g.close()
+
+
+
 # ---------------------------------------------------------------------------------- configuration sweep
 def _sample(cfgs, n, seed):
     """n configurations: evenly strided over the canonical enumeration plus seeded random picks, so
@@ -208,6 +303,63 @@ def test_subband_plan_kernel_configuration_sweep(kernel):
     g.close()
 
 
+@pytest.mark.parametrize("nchan", [320, 512])
+def test_direct_wide_reduction_sweep_and_saturation(nchan):
+    """More than 257 channels: the packed kernel flushes its 16-bit lanes every 256 rows (WIDE), with a
+    ragged last flush (320 = 256 + 64) and without one (512): staged shapes incl. single-buffered ones
+    against the oracle, then all-255 input (the largest values the lanes and the flush can see)."""
+    cfg = small_direct(name="wide%d" % nchan, nchan=nchan, nsamp_out=2100, ndm=41, widths=(1, 2, 4, 8), n_pulses=2)
+    g = GpuSearch(cfg)
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="wide default")
+    staged = [c for c in g.plan.enumerate_kcfgs(ddp.K_DIRECT) if c.staging != 0]
+    picks = _sample(staged, 40, seed=nchan)
+    seen = set()
+    for c in picks:
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        seen.add((c.staging, c.unroll))
+        g.buf["d_out"].fill_(-1)
+        assert np.array_equal(g.dedisperse(), Yo), "wide direct differs for %r" % c
+    assert {s for s, _ in seen} >= {1, 2} and len({u for _, u in seen}) >= 3
+    g.X[:] = 255
+    g.upload()
+    for c in picks[::5]:
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.all(g.dedisperse() == 255 * nchan), "saturated wide direct differs for %r" % c
+    g.close()
+
+
+@pytest.mark.parametrize("cps", [96, 256])
+def test_subband_step2_lane_group_sizes(cps):
+    """Step 2 sums G subband words in 16-bit lanes before splitting them: G = 2 for 65..128 channels per
+    subband, G = 1 for 129..257 (cfg2 itself has G = 4).  Sweep of staged step-2 shapes, plus all-255 input."""
+    cfg = small_subband(name="g_cps%d" % cps, nchan=8 * cps, nsamp_out=1800, ndm=5 * 8,
+                        subband=SubbandPlan(n_subbands=8, n_coarse=5, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=8, fine_step=0.25))
+    g = GpuSearch(cfg)
+    assert g.info.sub_elem_bytes == 2
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    assert np.array_equal(g.subband_intermediate(), So)
+    compare_all(g, Yo, what="lane group default")
+    staged = [c for c in g.plan.enumerate_kcfgs(ddp.K_SUB2) if c.staging != 0]
+    picks = _sample(staged, 24, seed=cps)
+    assert {c.staging for c in picks} == {1, 2}
+    for c in picks:
+        g.plan.set_kcfg(ddp.K_SUB2, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.array_equal(g.dedisperse(), Yo), "step 2 differs for %r" % c
+    g.X[:] = 255
+    g.upload()
+    for c in picks[::4]:
+        g.plan.set_kcfg(ddp.K_SUB2, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.all(g.dedisperse() == 255 * 8 * cps)
+    g.close()
+
+
 def test_subband_wide_subbands_keep_uint32_intermediate():
     """SB.4: more than 257 channels per subband cannot be stored in 16 bits -> uint32 S, generic step 2."""
     cfg = small_subband(name="wide_sb", nchan=1040, nsamp_out=1500, ndm=4 * 6,
@@ -245,19 +397,27 @@ def test_subband_saturated_input_fills_the_uint16_intermediate():
 
 
 # ---------------------------------------------------------------------------------- full-size configs
-def _sampled_rows(ndm, n, seed):
-    rng = np.random.default_rng(seed)
-    rows = {0, 1, ndm // 2, ndm - 2, ndm - 1} | set(rng.integers(0, ndm, n).tolist())
-    return np.array(sorted(rows))
+# The shapes that are BENCHMARKED are the ones that are compared: every kernel slot is first left at the
+# plan default and then set to its entry of tuned_b200.json (what bench.py times), and EVERY row of the
+# result is compared with the oracle -- the all-cores leg (oracle_mt.cpp) computes all rows in seconds.
+def _shape_sets(workload):
+    return [("defaults", False), ("tuned_b200.json:" + workload, True)]
 
 
 @pytest.mark.slow
-def test_cfg1_full_size_sampled_rows():
+def test_cfg1_full_size_every_row_default_and_tuned_shapes():
     cfg = configs.apertif_direct()
     g = GpuSearch(cfg)
-    g.run_all()
-    rows = _sampled_rows(cfg.ndm, 12, 1)
-    compare_all(g, oracle_direct_rows(cfg, g.X, rows), rows=rows, what="cfg1")
+    Yo = oracle_direct_all_rows_mt(cfg, g.X)
+    assert tuned_shapes("cfg1"), "tuned_b200.json has no cfg1 entry"
+    for what, tuned in _shape_sets("cfg1"):
+        if tuned:
+            g.apply_tuned("cfg1")
+        g.buf["d_out"].fill_(-1)
+        g.buf["d_integ"].fill_(-1)
+        g.buf["d_snr"].fill_(-7.0)
+        g.run_all()
+        compare_all(g, Yo, what="cfg1 " + what, mt=True)
     # every injected pulse is found at its DM (rows of the pulses' DMs carry the S/N maxima nearby)
     S = g.buf["d_snr"].cpu().numpy()
     for p in g.pulses:
@@ -265,28 +425,32 @@ def test_cfg1_full_size_sampled_rows():
         lo, hi = max(0, i - 8), min(cfg.ndm, i + 9)
         assert S[lo:hi].max() > 6.0, "pulse %r not detected" % (p,)
     # a shape whose two buffers of shifted copies exceed 227 KB: single-buffered copies + wide flush
-    Yo = oracle_direct_rows(cfg, g.X, rows)
     g.plan.set_kcfg(ddp.K_DIRECT, ddp.Kcfg(64, 8, 16, 8, 16, 2, 16))
     g.buf["d_out"].fill_(-1)
-    assert np.array_equal(g.dedisperse()[rows], Yo), "single-buffered direct kernel differs"
+    assert np.array_equal(g.dedisperse(), Yo), "single-buffered direct kernel differs"
     g.close()
 
 
 @pytest.mark.slow
-def test_cfg2_full_size_sampled_rows_and_identity_rows():
+def test_cfg2_full_size_every_row_default_and_tuned_shapes_and_identity_rows():
     cfg = configs.apertif_subband()
     g = GpuSearch(cfg)
-    g.run_all()
     sb = cfg.subband
-    coarse = np.array([0, 1, 31, 63])
-    So, Yo = oracle_subband(cfg, g.X, coarse)
-    Sg = g.subband_intermediate()[coarse]
-    assert np.array_equal(Sg, So)
-    rows = (coarse[:, None] * sb.n_fine + np.arange(sb.n_fine)[None, :]).reshape(-1)
-    compare_all(g, Yo, rows=rows, what="cfg2")
-    # SB.6 / BJ:cfg2: zero-fine-offset rows equal config 1's direct rows at the same DM
+    So, Yo = oracle_subband_mt(cfg, g.X)
+    assert tuned_shapes("cfg2"), "tuned_b200.json has no cfg2 entry"
+    for what, tuned in _shape_sets("cfg2"):
+        if tuned:
+            g.apply_tuned("cfg2")
+        g.buf["d_out"].fill_(-1)
+        g.buf["d_integ"].fill_(-1)
+        g.buf["d_snr"].fill_(-7.0)
+        g.run_all()
+        assert np.array_equal(g.subband_intermediate(), So), "cfg2 %s: S differs" % what
+        compare_all(g, Yo, what="cfg2 " + what, mt=True)
+    # SB.6 / BJ:cfg2: zero-fine-offset rows equal config 1's direct rows at the same DM (all 64 of them)
     d = configs.apertif_direct()
-    Yd = oracle_direct_rows(d, g.X, coarse * sb.n_fine)
+    coarse = np.arange(sb.n_coarse)
+    Yd = oracle_direct_all_rows_mt(d, g.X, coarse * sb.n_fine)
     assert np.array_equal(u32(g.buf["d_out"])[coarse * sb.n_fine, : cfg.nsamp_out], Yd)
     # step-1 shapes whose two buffers of shifted copies exceed 227 KB run single-buffered (TMA and
     # cooperative staging): same S, same Y
@@ -294,18 +458,25 @@ def test_cfg2_full_size_sampled_rows_and_identity_rows():
         g.plan.set_kcfg(ddp.K_SUB1, ddp.Kcfg(*genes))
         g.buf["d_out"].fill_(-1)
         Y = g.dedisperse()
-        assert np.array_equal(g.subband_intermediate()[coarse], So), "S differs for single-buffered %r" % genes
-        assert np.array_equal(Y[rows], Yo), "Y differs for single-buffered %r" % genes
+        assert np.array_equal(g.subband_intermediate(), So), "S differs for single-buffered %r" % genes
+        assert np.array_equal(Y, Yo), "Y differs for single-buffered %r" % genes
     g.close()
 
 
 @pytest.mark.slow
-def test_cfg3_full_size_sampled_rows():
+def test_cfg3_full_size_every_row_default_and_tuned_shapes():
     cfg = configs.ska_mid()
     g = GpuSearch(cfg)
-    g.run_all()
-    rows = _sampled_rows(cfg.ndm, 5, 3)
-    compare_all(g, oracle_direct_rows(cfg, g.X, rows), rows=rows, what="cfg3")
+    Yo = oracle_direct_all_rows_mt(cfg, g.X)
+    assert tuned_shapes("cfg3"), "tuned_b200.json has no cfg3 entry"
+    for what, tuned in _shape_sets("cfg3"):
+        if tuned:
+            g.apply_tuned("cfg3")
+        g.buf["d_out"].fill_(-1)
+        g.buf["d_integ"].fill_(-1)
+        g.buf["d_snr"].fill_(-7.0)
+        g.run_all()
+        compare_all(g, Yo, what="cfg3 " + what, mt=True)
     g.close()
 
 

@@ -318,6 +318,26 @@ def test_template_compiles_for_sm100a_without_a_gpu(tmp_path, k, genes):
     plan.destroy()
 
 
+def test_257_channels_per_subband_compiles_staged_step_one(tmp_path):
+    """cps = 257: the uint16 intermediate is still exact (257 * 255 = 65535) and the packed kernel must not
+    ask for the wide flush at the same time (the template static_asserts against that combination)."""
+    f = 1550.0 - 0.1 * np.arange(514)
+    plan = ddp.plan_create(f, 40.96e-6, None, [1, 2], 1000, n_subbands=2, n_coarse=3, coarse_dm_step=8.0,
+                           n_fine=4, fine_dm_step=0.25, cache_dir=str(tmp_path))
+    assert plan.query().sub_elem_bytes == 2
+    c = plan.get_kcfg(ddp.K_SUB1)
+    assert c.staging != 0
+    plan.compile_kcfg(ddp.K_SUB1, c)
+    plan.compile_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 2, 16, 2, 1, 2, 16))
+    plan.destroy()
+    # 258 channels per subband: uint32 intermediate, wide flush
+    plan = ddp.plan_create(1550.0 - 0.1 * np.arange(516), 40.96e-6, None, [1, 2], 1000, n_subbands=2, n_coarse=3,
+                           coarse_dm_step=8.0, n_fine=4, fine_dm_step=0.25, cache_dir=str(tmp_path))
+    assert plan.query().sub_elem_bytes == 4
+    plan.compile_kcfg(ddp.K_SUB1, plan.get_kcfg(ddp.K_SUB1))
+    plan.destroy()
+
+
 # ----------------------------------------------------------------------------- no fallback
 @pytest.mark.skipif(has_gpu(), reason="checks the behaviour of a machine WITHOUT a CUDA device")
 def test_compute_calls_fail_loudly_without_a_device():

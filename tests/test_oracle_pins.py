@@ -351,3 +351,31 @@ def test_cfg0_pulse_recovered_at_its_dm_and_width():
     assert 15.5 < S[i, j] < 18.5
     others = np.delete(S.max(axis=1), i)
     assert others.max() < S[i, j] - 3.0
+
+
+# ----------------------------------------------------------------------------- all-cores leg
+def test_all_cores_leg_equals_pure_python_brute_force_and_single_thread_leg():
+    """oracle_mt.cpp only spreads rows over the cores: pinned to the pure-Python brute
+    force on a tiny case, and bit-identical to the single-thread functions on cfg0 (direct, subband
+    with a ragged coarse/fine grid, integrate + S/N with ddof 0 and 1)."""
+    f, dms, ts, delay, X = small_case(11)
+    assert oracle.dedisperse_mt(X, delay, 37).tolist() == py_dedisperse(X, delay.tolist(), 37)
+
+    cfg = configs.tiny()
+    d = oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s)
+    Xc, _ = filterbank.make_filterbank(cfg, cfg.nsamp_out + int(d.max()))
+    Y = oracle.dedisperse(Xc, d, cfg.nsamp_out)
+    assert np.array_equal(oracle.dedisperse_mt(Xc, d, cfg.nsamp_out), Y)
+    for ddof in (0, 1):
+        P, S, A = oracle.search(Y, cfg.widths, ddof)
+        Pm, Sm, Am = oracle.search_mt(Y, cfg.widths, ddof)
+        assert all(np.array_equal(P[w], Pm[w]) for w in cfg.widths)
+        assert np.array_equal(S, Sm) and np.array_equal(A, Am)
+    A_dm, F_dm = 4.0 * np.arange(5), 0.5 * np.arange(7)
+    d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, 8, A_dm, F_dm)
+    ns = 3000
+    S1 = oracle.subband_step1(Xc, d1, 8, ns + int(d2.max()))
+    Y2 = oracle.subband_step2(S1, d2, ns)
+    Sm, Ym = oracle.subband_mt(Xc, d1, d2, 8, ns)
+    assert np.array_equal(S1, Sm) and np.array_equal(Y2, Ym)
+    assert oracle.mt_threads() >= 1
