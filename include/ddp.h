@@ -65,14 +65,17 @@ typedef enum {
  *   dms_per_thread     {1,2,4,8,16}                                   (nrDMsPerThread)
  *   unroll      reduction-loop unroll / rows per staging chunk {1,2,4,8,16}   (unroll)
  *   staging     how the delayed input window reaches the threads: 0 direct global loads,
- *               1 cooperative copy to shared memory, 2 TMA bulk copy to shared memory  (localMem)
+ *               1 cooperative copy to shared memory, 2 TMA bulk copy to shared memory  (localMem);
+ *               uint8 dedispersion kernels only: 3 / 4 = TMA bulk copy, then 2 / 4 adjacent channels are
+ *               pre-summed EXACTLY in shared memory for every distinct tuple of their relative delays in
+ *               the tile, and the trials add those partial sums (same integers as the plain sum)
  *   vec_bytes   width in bytes of one input load instruction {1,4,8,16}
  * All genes are powers of two. */
 typedef struct {
     int threads_t, threads_dm, samples_per_thread, dms_per_thread, unroll, staging, vec_bytes;
 } ddp_kcfg;
 
-enum { DDP_STAGE_DIRECT = 0, DDP_STAGE_SMEM = 1, DDP_STAGE_TMA = 2 };
+enum { DDP_STAGE_DIRECT = 0, DDP_STAGE_SMEM = 1, DDP_STAGE_TMA = 2, DDP_STAGE_TMA_MERGE2 = 3, DDP_STAGE_TMA_MERGE4 = 4 };
 
 /* Options of ddp_plan_create; zero-initialise for a direct plan with defaults. */
 typedef struct {

@@ -19,7 +19,7 @@ static const int DDP_CAND_THREADS_DM[] = {1, 2, 4, 8, 16, 32};
 static const int DDP_CAND_SPT[] = {1, 2, 4, 8, 16};
 static const int DDP_CAND_DPT[] = {1, 2, 4, 8, 16};
 static const int DDP_CAND_UNROLL[] = {1, 2, 4, 8, 16};
-static const int DDP_CAND_STAGING[] = {0, 1, 2};
+static const int DDP_CAND_STAGING[] = {0, 1, 2, 3, 4};
 static const int DDP_CAND_VEC[] = {1, 4, 8, 16};
 #define DDP_NGENES 7
 struct DdpGeneDomain { const int* v; int n; };
@@ -40,6 +40,20 @@ struct DdpKGeom {
 
 struct DdpCompiled;  // runtime kernel handle (ddp_rt.cpp)
 
+// Merged staging (staging genes 3 / 4): per DM tile of TD trials and per group of G adjacent reduction rows,
+// the distinct tuples of relative delays ("variants") and which variant every trial uses.  Depends on the
+// delay table, TD and G only, so it is built once on the host and kept in the workspace, instead of being
+// rediscovered by every block.  blob layout (all per tile t < ntiles, global group gg < ngg = rows / G):
+//   nvar  int32 [ntiles][ngg]                     at byte 0
+//   vdesc int32 [ntiles][ngg][vmax][2 + G]        at byte off_vdesc   {min delta, max delta, tau[0..G)}
+//   vid   uint8 [ntiles][ngg][TD]                 at byte off_vid     variant of every trial
+// delta = d[j][r0] - d[first trial][r0]; tau[m] = (d[j][r0+m] - d[j][r0]) - (same for the tile's first trial).
+struct DdpMergeTable {
+    int vmax = 0, ntiles = 0, ngg = 0;
+    int64_t off_vdesc = 0, off_vid = 0;
+    std::vector<unsigned char> blob;
+};
+
 struct ddp_plan {
     // problem
     int nchan = 0, ndm = 0, nwidths = 0, ns = 0;
@@ -57,6 +71,11 @@ struct ddp_plan {
     // configurations + validity caches
     ddp_kcfg kcfg[DDP_K_COUNT];
     mutable std::map<int, int> spread_cache[3];              // dedisp kernel -> (TD -> max window spread)
+    mutable std::map<std::pair<int, int>, int> vmax_cache[3]; // dedisp kernel -> ((TD, G) -> max variants per group)
+    mutable std::map<std::pair<int, int>, DdpMergeTable> merge_tables[3];  // host copies, built on first use
+    int64_t merge_capacity = 0;                               // bytes of the workspace region for the resident table
+    unsigned char* d_merge = nullptr;                         // device: resident merge table (one (kernel, TD, G) at a time)
+    int merge_resident[3] = {-1, 0, 0};                       // (which, TD, G) of the table at d_merge
     mutable std::vector<ddp_kcfg> valid[DDP_K_COUNT];
     mutable bool valid_built[DDP_K_COUNT] = {false, false, false, false, false};
     // device side (ddp_rt.cpp)
@@ -76,6 +95,14 @@ int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD);           // dedisp
 int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // staged row window (elements)
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // packed uint8 kernel: one copy buffer
+// Merged staging (staging genes 3 / 4: G = 2 / 4 adjacent rows pre-summed exactly; uint8 dedispersion only).
+inline int ddp_merge_group(const ddp_kcfg& c) { return c.staging == 3 ? 2 : (c.staging == 4 ? 4 : 0); }
+int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G);  // largest number of distinct relative-shift tuples
+struct DdpMergeGeom { int vmax, lw, le; };
+int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G, int vmax);
+const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, int G);
+DdpMergeGeom ddp_merge_geom(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
+#define DDP_MERGE_VMAX_LIMIT 32                 // half of the kernel's 64 hash slots per group
 bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::string* why);
 const std::vector<ddp_kcfg>& ddp_valid_set(const ddp_plan* p, ddp_kernel k);
 bool ddp_kcfg_equal(const ddp_kcfg& a, const ddp_kcfg& b);

@@ -26,6 +26,14 @@ struct DdpDedispParams {
     int ns;                      // output samples per row
     int win;                     // staged modes: elements of one staged row window in shared memory
     int one;                     // the value 1, unknown to the compiler (packed kernel: adds issued as IMAD)
+    int vmax;                    // merged staging: rows reserved per group = largest variant count of the plan
+    int lw;                      // merged staging: words per variant row  (TT/2 + largest window spread, padded)
+    int le;                      // merged staging: words per expanded channel row
+    const unsigned char* meta;   // merged staging: resident DdpMergeTable blob (device)
+    long long meta_vdesc_off;    //   byte offsets of its vdesc and vid arrays
+    long long meta_vid_off;
+    int meta_ngg;                //   groups per DM tile in the table (all subbands)
+    int meta_gg0_stride;         //   table groups between consecutive kernel groups g (subband step 1: cps / G; direct: 0)
 };
 
 // Integration: plane k holds I_w[i][j] = sum_{m<w} in[i][j*w+m] for w = width[k] > 1.

@@ -14,7 +14,7 @@
 // ------------------------------------------------------------------------------------ genes
 static const DdpGeneDomain kDomains[DDP_NGENES] = {
     {DDP_CAND_THREADS_T, 7}, {DDP_CAND_THREADS_DM, 6}, {DDP_CAND_SPT, 5}, {DDP_CAND_DPT, 5},
-    {DDP_CAND_UNROLL, 5},    {DDP_CAND_STAGING, 3},    {DDP_CAND_VEC, 4}};
+    {DDP_CAND_UNROLL, 5},    {DDP_CAND_STAGING, 5},    {DDP_CAND_VEC, 4}};
 const DdpGeneDomain* ddp_gene_domains() { return kDomains; }
 int* ddp_gene_ptr(ddp_kcfg* c, int gene) {
     switch (gene) {
@@ -198,7 +198,9 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     int64_t tbytes = p->subband ? round_up((int64_t)p->d1.size() * 4, 256) + round_up((int64_t)p->d2.size() * 4, 256)
                                 : round_up((int64_t)p->delay.size() * 4, 256);
     int64_t sbytes = p->subband ? round_up((int64_t)p->ncoarse * p->nsub * I.sub_stride * I.sub_elem_bytes, 256) : 0;
-    I.workspace_bytes = tbytes + sbytes + 256;
+    // region for the resident merged-staging table (one (kernel, TD, G) at a time; DdpMergeTable)
+    p->merge_capacity = round_up(2 * (int64_t)(p->subband ? p->d1.size() : p->delay.size()) * 4 + (1 << 20), 256);
+    I.workspace_bytes = tbytes + sbytes + p->merge_capacity + 256;
     I.adds_dedisp = p->subband ? (double)p->ncoarse * nchan * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
                                : (double)p->ndm * nchan * nsamp_out;
     default_kcfgs(p);
@@ -279,6 +281,123 @@ int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD) {
     p->spread_cache[which][TD] = mx;
     return mx;
 }
+// Merged staging: the largest number of distinct tuples (d[j][r0+m] - d[j][r0])_{m<G} over the TD trials of
+// any DM tile and any group of G adjacent reduction rows -- the rows per group the kernel reserves.
+int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G) {
+    const int which = k == DDP_K_DIRECT ? 0 : (k == DDP_K_SUB1 ? 1 : 2);
+    auto key = std::make_pair(TD, G);
+    auto it = p->vmax_cache[which].find(key);
+    if (it != p->vmax_cache[which].end()) return it->second;
+    const std::vector<int32_t>& t = which == 0 ? p->delay : (which == 1 ? p->d1 : p->d2);
+    const int ni = which == 0 ? p->ndm : (which == 1 ? p->ncoarse : p->nfine);
+    const int nc = which == 2 ? p->nsub : p->nchan;
+    const int nred = ddp_kgeom(p, k).nred;  // groups never straddle a subband: nred % G == 0 is a validity rule
+    int vmax = 0;
+    std::vector<int32_t> found;  // distinct tuples of the current (tile, group), G - 1 ints each
+    for (int lo = 0; lo < ni && vmax <= DDP_MERGE_VMAX_LIMIT; lo += TD) {
+        const int hi = std::min(lo + TD, ni);
+        for (int r0 = 0; r0 + G <= nc; r0 += G) {
+            if (nred % G != 0) continue;
+            found.clear();
+            int nv = 0;
+            for (int j = lo; j < hi; ++j) {
+                const int32_t* d = &t[(size_t)j * nc + r0];
+                int v = 0;
+                for (; v < nv; ++v) {
+                    bool same = true;
+                    for (int m = 1; m < G; ++m) same = same && found[(size_t)v * (G - 1) + m - 1] == d[m] - d[0];
+                    if (same) break;
+                }
+                if (v == nv) {
+                    for (int m = 1; m < G; ++m) found.push_back(d[m] - d[0]);
+                    ++nv;
+                }
+            }
+            vmax = std::max(vmax, nv);
+        }
+    }
+    p->vmax_cache[which][key] = vmax;
+    return vmax;
+}
+static void merge_dims(const ddp_plan* p, ddp_kernel k, int TD, int G, int* ni, int* nc) {
+    *ni = k == DDP_K_DIRECT ? p->ndm : p->ncoarse;
+    *nc = p->nchan;
+    (void)TD; (void)G;
+}
+int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G, int vmax) {
+    int ni, nc;
+    merge_dims(p, k, TD, G, &ni, &nc);
+    const int64_t ntiles = (ni + TD - 1) / TD, ngg = nc / G;
+    return round_up(ntiles * ngg * 4, 16) + round_up(ntiles * ngg * vmax * (2 + G) * 4, 16) + round_up(ntiles * ngg * TD, 16);
+}
+// The full table (see DdpMergeTable).  Trials beyond the last one of a ragged tile repeat the last trial.
+const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, int G) {
+    const int which = k == DDP_K_DIRECT ? 0 : 1;
+    auto key = std::make_pair(TD, G);
+    auto it = p->merge_tables[which].find(key);
+    if (it != p->merge_tables[which].end()) return it->second;
+    DdpMergeTable& T = p->merge_tables[which][key];
+    const std::vector<int32_t>& t = which == 0 ? p->delay : p->d1;
+    int ni, nc;
+    merge_dims(p, k, TD, G, &ni, &nc);
+    T.vmax = ddp_merge_vmax(p, k, TD, G);
+    T.ntiles = (ni + TD - 1) / TD;
+    T.ngg = nc / G;
+    const int64_t n = (int64_t)T.ntiles * T.ngg;
+    T.off_vdesc = round_up(n * 4, 16);
+    T.off_vid = T.off_vdesc + round_up(n * T.vmax * (2 + G) * 4, 16);
+    T.blob.assign((size_t)(T.off_vid + round_up(n * TD, 16)), 0);
+    int32_t* nvar = (int32_t*)T.blob.data();
+    int32_t* vdesc = (int32_t*)(T.blob.data() + T.off_vdesc);
+    unsigned char* vid = T.blob.data() + T.off_vid;
+    const int W = 2 + G;
+    for (int ti = 0; ti < T.ntiles; ++ti) {
+        const int lo = ti * TD, nd = std::min(TD, ni - lo);
+        for (int gg = 0; gg < T.ngg; ++gg) {
+            const int r0 = gg * G;
+            const int32_t* d0 = &t[(size_t)lo * nc + r0];
+            int32_t* vd = vdesc + ((size_t)ti * T.ngg + gg) * T.vmax * W;
+            unsigned char* vi = vid + ((size_t)ti * T.ngg + gg) * TD;
+            int nv = 0;
+            for (int j = 0; j < TD; ++j) {
+                const int32_t* d = &t[(size_t)(lo + std::min(j, nd - 1)) * nc + r0];
+                const int delta = d[0] - d0[0];
+                int v = 0;
+                for (; v < nv; ++v) {
+                    bool same = true;
+                    for (int m = 1; m < G; ++m) same = same && vd[v * W + 2 + m] == (d[m] - d[0]) - (d0[m] - d0[0]);
+                    if (same) break;
+                }
+                if (v == nv) {
+                    vd[v * W] = delta;
+                    vd[v * W + 1] = delta;
+                    vd[v * W + 2] = 0;
+                    for (int m = 1; m < G; ++m) vd[v * W + 2 + m] = (d[m] - d[0]) - (d0[m] - d0[0]);
+                    ++nv;
+                } else {
+                    vd[v * W] = std::min(vd[v * W], delta);
+                    vd[v * W + 1] = std::max(vd[v * W + 1], delta);
+                }
+                vi[j] = (unsigned char)v;
+            }
+            nvar[(size_t)ti * T.ngg + gg] = nv;
+        }
+    }
+    return T;
+}
+DdpMergeGeom ddp_merge_geom(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
+    const int G = ddp_merge_group(c);
+    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
+    const int TD = c.threads_dm * c.dms_per_thread;
+    const int spread = ddp_spread_max(p, k, TD);
+    DdpMergeGeom g;
+    g.vmax = ddp_merge_vmax(p, k, TD, G);
+    // both carry 32 words of slack: the variant rows are built in whole 32-word blocks
+    g.lw = (int)round_up(TT / 2 + spread + 4 + 32, 4);   // variant row: y < TT/2 + spread
+    g.le = (int)round_up(TT / 2 + spread + 20 + 32, 4);  // expanded row: z < 16 + spread + TT/2, whole uint4 stores
+    return g;
+}
+
 int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const DdpKGeom g = ddp_kgeom(p, k);
     const int AL = 16 / g.in_bytes;
@@ -299,6 +418,23 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (c.staging == 0) return 0;
             const DdpKGeom g = ddp_kgeom(p, k);
             const size_t row = (size_t)ddp_dedisp_win(p, k, c) * g.in_bytes;
+            if (g.in_bytes == 1 && ddp_merge_group(c)) {  // ddp_dedisp_merge_body (same carve-up, same order)
+                const size_t G = (size_t)ddp_merge_group(c), U = (size_t)c.unroll, NG = U / G, NGS = 64 / G;
+                const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
+                const DdpMergeGeom mg = ddp_merge_geom(p, k, c);
+                size_t b = 2 * NG * mg.vmax * mg.lw * 4;              // pw
+                b += U * (size_t)mg.le * 4;                           // ebuf
+                b += 2 * TD * NGS * 4;                                // dbase
+                b += 2 * 2 * 64 * 4;                                  // dmm
+                b += ((2 * TD * NG + 3) & ~(size_t)3) * 4;            // offs
+                b += NG * mg.vmax * 8 * 4;                            // rowd
+                b += 2 * NGS * mg.vmax * (2 + G) * 4;                 // vdesc
+                b += 2 * NGS * 4;                                     // nvar
+                b += 2 * NGS * TD;                                    // vid
+                b = (b + 15) & ~(size_t)15;
+                b += 2 * U * (row + 16) + 16;                         // raw, mbar
+                return b;
+            }
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
                 auto layout = [&](size_t nb) {
@@ -334,7 +470,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
 // The packed uint8 kernel keeps two buffers of shifted copies (chunk c+1 converted while chunk c is
 // summed); a configuration whose two buffers exceed 227 KB runs with one, if that fits.
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
-    if (c.staging == 0 || ddp_kgeom(p, k).in_bytes != 1) return false;
+    if (c.staging == 0 || ddp_merge_group(c) || ddp_kgeom(p, k).in_bytes != 1) return false;
     const size_t row = (size_t)ddp_dedisp_win(p, k, c);
     const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
     size_t two = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
@@ -357,8 +493,20 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     // V7: a gene the kernel does not read is pinned (snr reads `unroll` only with direct loads)
     if (k == DDP_K_SNR && c.staging != 0 && c.unroll != 1) return no("V7: snr ignores unroll when staged; must be 1");
+    // merged staging (genes 3, 4) exists for the uint8 dedispersion kernels only; its groups are whole
+    // multiples of the chunk, its window words hold two samples, the vector-width gene is unused (V7)
+    const int MG = ddp_merge_group(c);
+    if (MG) {
+        if (geo.in_bytes != 1 || geo.nred == 0) return no("V6: merged staging is for uint8 dedispersion only");
+        if (c.unroll % MG != 0) return no("V4: unroll is not a multiple of the merge group");
+        if (c.vec_bytes != 16) return no("V7: merged staging ignores vec_bytes; must be 16");
+        if (c.samples_per_thread < 2) return no("V5: merged staging needs samples_per_thread >= 2");
+        if (c.threads_t < 32) return no("V1: merged staging needs threads_t >= 32");
+        if ((c.threads_dm * c.dms_per_thread) % 4 != 0) return no("V3: merged staging needs a DM tile of a multiple of 4 trials");
+    }
     // V5: vector width vs. what a thread loads contiguously
-    if (geo.in_bytes == 1) {
+    if (MG) {
+    } else if (geo.in_bytes == 1) {
         if (c.vec_bytes > 1 && c.vec_bytes > c.samples_per_thread) return no("V5: vec_bytes > samples_per_thread bytes");
         if (c.staging != 0) {  // the packed kernel works on whole 4-sample words, one warp per 32 of them
             if (c.samples_per_thread < 4) return no("V5: staged uint8 input needs samples_per_thread >= 4");
@@ -387,7 +535,13 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
         for (int i = 0; i < p->nwidths; ++i)
             if (p->widths[i] > 1 && TT % p->widths[i] != 0) return no("V3: a width does not divide the time tile");
     }
-    // V6: staged window fits shared memory
+    // V6: staged window fits shared memory; merged staging: the variant rows of a group fit the kernel's table
+    if (MG) {
+        const int vm = ddp_merge_vmax(p, k, (int)TD, MG);
+        if (vm > DDP_MERGE_VMAX_LIMIT) return no("V6: too many relative-shift variants per group for merged staging");
+        if (ddp_merge_table_bytes(p, k, (int)TD, MG, vm) > p->merge_capacity)
+            return no("V6: merged-staging table larger than its workspace region");
+    }
     if (ddp_smem_bytes(p, k, c) > DDP_SMEM_LIMIT) return no("V6: shared memory over 227 KB");
     return true;
 }

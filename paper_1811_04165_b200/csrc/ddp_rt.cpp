@@ -615,9 +615,12 @@ extern "C" ddp_status ddp_plan_bind_workspace(ddp_plan* plan, void* d_workspace,
         r = upload(plan->d1, &plan->d_d1);
         if (r == CUDA_SUCCESS) r = upload(plan->d2, &plan->d_d2);
         plan->d_sub = (uint32_t*)(base + off);
+        off += (size_t)round_up64((int64_t)plan->ncoarse * plan->nsub * plan->info.sub_stride * plan->info.sub_elem_bytes, 256);
     } else {
         r = upload(plan->delay, &plan->d_delay);
     }
+    plan->d_merge = (unsigned char*)(base + off);
+    plan->merge_resident[0] = -1;
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "delay table upload: " + cu_err(r));
     plan->ws = d_workspace;
     plan->ws_bytes = bytes;
@@ -723,6 +726,29 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
     }
     q.win = c.staging ? ddp_dedisp_win(p, k, c) : 0;
     q.one = 1;
+    if (const int G = ddp_merge_group(c)) {
+        const DdpMergeGeom mg = ddp_merge_geom(p, k, c);
+        q.vmax = mg.vmax;
+        q.lw = mg.lw;
+        q.le = mg.le;
+        // the (kernel, TD, G) table must be the resident one: upload it on the launch stream when it is not
+        const int TDm = c.threads_dm * c.dms_per_thread, which = k == DDP_K_DIRECT ? 0 : 1;
+        const DdpMergeTable& T = ddp_merge_table(p, k, TDm, G);
+        ddp_plan* pm = const_cast<ddp_plan*>(p);
+        if (p->merge_resident[0] != which || p->merge_resident[1] != TDm || p->merge_resident[2] != G) {
+            if ((int64_t)T.blob.size() > p->merge_capacity) return ddp_fail(p, DDP_E_WORKSPACE, "merged-staging table does not fit");
+            CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)p->d_merge, T.blob.data(), T.blob.size(), io.stream);
+            if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, "merged-staging table upload: " + cu_err(r));
+            pm->merge_resident[0] = which;
+            pm->merge_resident[1] = TDm;
+            pm->merge_resident[2] = G;
+        }
+        q.meta = p->d_merge;
+        q.meta_vdesc_off = T.off_vdesc;
+        q.meta_vid_off = T.off_vid;
+        q.meta_ngg = T.ngg;
+        q.meta_gg0_stride = k == DDP_K_SUB1 ? p->cps / G : 0;
+    }
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     return launch(p, K, cdiv(q.ns, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,

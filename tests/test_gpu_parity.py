@@ -253,7 +253,7 @@ def test_direct_plan_kernel_configuration_sweep(kernel):
             g.integrate()
         g.snr()
         compare_all(g, Yo, what="%s %r" % (ddp.KERNEL_NAMES[kernel], c))
-    assert {s for s, _ in seen} == {0, 1, 2}
+    assert {s for s, _ in seen} >= {0, 1, 2}
     g.close()
 
 
@@ -299,7 +299,94 @@ def test_subband_plan_kernel_configuration_sweep(kernel):
         Y = g.dedisperse()
         assert np.array_equal(g.subband_intermediate(), So), "S differs for %r" % c
         assert np.array_equal(Y, Yo), "Y differs for %s %r" % (ddp.KERNEL_NAMES[kernel], c)
-    assert seen == {0, 1, 2}
+    assert seen >= {0, 1, 2}
+    g.close()
+
+
+# ---------------------------------------------------------------------------------- merged staging (genes 3, 4)
+def _merged(plan, kernel, n, seed):
+    V = [c for c in plan.enumerate_kcfgs(kernel) if c.staging >= 3]
+    assert V, "no merged-staging shape is valid for this plan"
+    picks = _sample(V, n, seed)
+    # make sure both group sizes and several chunk sizes are in
+    for st in (3, 4):
+        picks += [c for c in V if c.staging == st][:2] + [c for c in V if c.staging == st][-2:]
+    return picks
+
+
+@pytest.mark.parametrize("nchan,ndm,dm_step", [(64, 41, 0.25), (80, 37, 0.25), (320, 41, 0.25), (512, 23, 0.5), (96, 64, 1.0)])
+def test_direct_merged_staging_sweep_and_saturation(nchan, ndm, dm_step):
+    """Staging genes 3 / 4: 2 / 4 adjacent channels pre-summed per distinct tuple of relative delays, then added
+    by the trials.  Bit-exact against the oracle over sampled shapes (ragged time and DM tiles, reductions of
+    64 ... 512 channels incl. the 256-row flush with and without a ragged last flush, one and several delay
+    superchunks), and with all-255 input (largest lane values)."""
+    import dataclasses
+    cfg = dataclasses.replace(small_direct(name="merge%d" % nchan, nchan=nchan, nsamp_out=2300, ndm=ndm,
+                                           widths=(1, 2, 4, 8), n_pulses=2), dm_step=dm_step)
+    g = GpuSearch(cfg)
+    Yo = oracle_direct_rows(cfg, g.X)
+    picks = _merged(g.plan, ddp.K_DIRECT, 36, seed=nchan)
+    assert {c.staging for c in picks} == {3, 4}
+    for c in picks:
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.array_equal(g.dedisperse(), Yo), "merged direct differs for %r" % c
+    g.run_all()
+    compare_all(g, Yo, what="merged direct, whole pipeline")
+    g.X[:] = 255
+    g.upload()
+    for c in picks[::4]:
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.all(g.dedisperse() == 255 * nchan), "saturated merged direct differs for %r" % c
+    g.close()
+
+
+def test_direct_merged_staging_unsorted_channel_order():
+    """Channel order is arbitrary (DD.3): with shuffled channels the relative delays of 'adjacent' rows are
+    large and of either sign; shapes that stay valid must still be exact."""
+    import dataclasses
+    base = small_direct(name="merge_shuffled", nchan=32, nsamp_out=1500, ndm=16, widths=(1, 2), n_pulses=1)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(base.nchan)
+    f = base.chan_freq_mhz()[perm]
+    plan = ddp.plan_create(f, base.t_samp_s, base.dm_list(), base.widths, base.nsamp_out)
+    info = plan.query()
+    b = ddp.alloc_buffers(plan)
+    from synth import filterbank
+    X0, _ = filterbank.make_filterbank(base, int(info.nsamp_in_required), int(info.in_stride_min))
+    X = np.ascontiguousarray(X0[perm])
+    b["d_in"].copy_(torch.from_numpy(X))
+    import oracle
+    Yo = oracle.dedisperse(X, oracle.delay_table(f, base.dm_list(), base.t_samp_s), base.nsamp_out)
+    V = [c for c in plan.enumerate_kcfgs(ddp.K_DIRECT) if c.staging >= 3]
+    assert V
+    for c in _sample(V, 16, seed=9):
+        plan.set_kcfg(ddp.K_DIRECT, c)
+        b["d_out"].fill_(-1)
+        plan.dedisperse(b["d_in"], b["d_out"])
+        torch.cuda.synchronize()
+        assert np.array_equal(u32(b["d_out"])[:, : base.nsamp_out], Yo), "merged, shuffled channels: %r" % c
+    plan.destroy()
+
+
+@pytest.mark.parametrize("cps,wide", [(16, False), (48, False), (260, True)])
+def test_subband_step1_merged_staging(cps, wide):
+    """Step 1 with merged staging: uint16 result (OUT16) and, for more than 257 channels per subband, the
+    uint32 intermediate with the 256-row flush; S and Y against the oracle."""
+    nsub = 4 if wide else 8
+    cfg = small_subband(name="merge_sb%d" % cps, nchan=nsub * cps, nsamp_out=2100, ndm=12 * 8,
+                        subband=SubbandPlan(n_subbands=nsub, n_coarse=12, coarse_first=0.0, coarse_step=2.0,
+                                            n_fine=8, fine_step=0.25))
+    g = GpuSearch(cfg)
+    assert g.info.sub_elem_bytes == (4 if wide else 2)
+    So, Yo = oracle_subband(cfg, g.X)
+    for c in _merged(g.plan, ddp.K_SUB1, 24, seed=cps):
+        g.plan.set_kcfg(ddp.K_SUB1, c)
+        g.buf["d_out"].fill_(-1)
+        Y = g.dedisperse()
+        assert np.array_equal(g.subband_intermediate(), So), "merged step 1: S differs for %r" % c
+        assert np.array_equal(Y, Yo), "merged step 1: Y differs for %r" % c
     g.close()
 
 
@@ -313,7 +400,7 @@ def test_direct_wide_reduction_sweep_and_saturation(nchan):
     g.run_all()
     Yo = oracle_direct_rows(cfg, g.X)
     compare_all(g, Yo, what="wide default")
-    staged = [c for c in g.plan.enumerate_kcfgs(ddp.K_DIRECT) if c.staging != 0]
+    staged = [c for c in g.plan.enumerate_kcfgs(ddp.K_DIRECT) if c.staging in (1, 2)]
     picks = _sample(staged, 40, seed=nchan)
     seen = set()
     for c in picks:

@@ -18,7 +18,7 @@ from synth import configs
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 GENE_DOMAINS = ((16, 32, 64, 128, 256, 512, 1024), (1, 2, 4, 8, 16, 32), (1, 2, 4, 8, 16), (1, 2, 4, 8, 16),
-                (1, 2, 4, 8, 16), (0, 1, 2), (1, 4, 8, 16))  # BASELINE.json configs[4]
+                (1, 2, 4, 8, 16), (0, 1, 2, 3, 4), (1, 4, 8, 16))  # BASELINE.json configs[4] + merged staging 3, 4
 
 
 def has_gpu():
@@ -203,7 +203,7 @@ def test_enumeration_is_exactly_the_valid_subset_of_the_raw_grid(cfg):
             assert plan.check_kcfg(k, c)
             for g, dom in enumerate(GENE_DOMAINS):
                 assert c.astuple()[g] in dom
-        # seeded sample of the 63 000-point raw grid: accepted iff enumerated
+        # seeded sample of the 105 000-point raw grid: accepted iff enumerated
         vset = set(keys)
         n_valid = 0
         for _ in range(3000):
@@ -211,7 +211,7 @@ def test_enumeration_is_exactly_the_valid_subset_of_the_raw_grid(cfg):
             ok = plan.check_kcfg(k, ddp.Kcfg(*raw))
             assert ok == (raw in vset)
             n_valid += ok
-        assert abs(n_valid / 3000.0 - len(keys) / 63000.0) < 0.03
+        assert abs(n_valid / 3000.0 - len(keys) / 105000.0) < 0.03
     plan.destroy()
 
 
