@@ -186,6 +186,48 @@ def search(Y: np.ndarray, widths: Sequence[int], ddof: int = 0):
     return planes, np.stack(S, axis=1), np.stack(A, axis=1)
 
 
+def integrate_sliding(Y: np.ndarray, w: int, ns: Optional[int] = None) -> np.ndarray:
+    """uint32 [nrows][ns - w + 1] stride-1 boxcar sums of width w (reading INT.1s)."""
+    assert Y.dtype == np.uint32 and Y.ndim == 2 and Y.flags.c_contiguous
+    if ns is None:
+        ns = Y.shape[1]
+    n = ns - w + 1
+    out = np.empty((Y.shape[0], max(n, 1)), dtype=np.uint32)
+    rc = _load().oracle_integrate_sliding(_p(Y), ctypes.c_size_t(Y.shape[1]), ctypes.c_int(Y.shape[0]),
+                                          ctypes.c_int(ns), ctypes.c_int(w), _p(out), ctypes.c_size_t(max(n, 1)))
+    if rc != 0:
+        raise ValueError("oracle_integrate_sliding rc=%d" % rc)
+    return out
+
+
+def search_sliding(Y: np.ndarray, widths: Sequence[int], ddof: int = 0):
+    """integrate_sliding + snr for every width: (planes dict w -> I^s_w, snr [nrows][nW], argmax [nrows][nW])."""
+    planes, S, A = {}, [], []
+    for w in widths:
+        I = Y if w == 1 else integrate_sliding(Y, w)
+        planes[w] = I
+        s, a = snr(np.ascontiguousarray(I), ddof)
+        S.append(s)
+        A.append(a)
+    return planes, np.stack(S, axis=1), np.stack(A, axis=1)
+
+
+def dedisperse_masked(X: np.ndarray, mask: np.ndarray, delay: np.ndarray, ns: int) -> np.ndarray:
+    """oracle dedispersion leaving out the channels whose mask byte is 0 (reading DD.7m)."""
+    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    mask = np.ascontiguousarray(mask, dtype=np.uint8)
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    nrows, nchan = delay.shape
+    assert nchan == X.shape[0] == mask.size
+    Y = np.empty((nrows, ns), dtype=np.uint32)
+    rc = _load().oracle_dedisperse_masked(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), _p(mask),
+                                          _p(delay), ctypes.c_int(nrows), ctypes.c_int(ns), _p(Y),
+                                          ctypes.c_size_t(ns))
+    if rc != 0:
+        raise ValueError("oracle_dedisperse_masked rc=%d" % rc)
+    return Y
+
+
 # ---------------------------------------------------------------------------- all-cores leg (oracle_mt.cpp)
 # Same arithmetic: every row is computed by the single-thread function above, rows are spread over
 # the host cores with `omp parallel for` (SURVEY 8(d), BASELINE.md section 3).

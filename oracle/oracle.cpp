@@ -20,7 +20,10 @@
 // every delay); constant input; linearity; brute force in pure Python on tiny inputs; subband
 // rows with zero fine offset == direct rows; nSub=1 identity; integration invariants
 // I_2w[j]=I_w[2j]+I_w[2j+1]; S/N affine + permutation invariance and numpy float64 closed form;
-// injected pulse recovered at its DM and width on BJ cfg0.
+// injected pulse recovered at its DM and width on BJ cfg0; sliding boxcar: constant / impulse closed forms,
+// numpy cumulative-sum difference, block sums are its samples at multiples of w, a misaligned pulse is
+// recovered at its true width; channel mask: pure-Python brute force over the kept channels, complement
+// identity; consecutive batches with carried samples == one long dedispersion.
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -shared -fPIC oracle.cpp -o liboracle.so
 #include <cmath>
@@ -127,6 +130,44 @@ int oracle_integrate(const uint32_t* Y, size_t stride, int nrows, int ns, int w,
             uint32_t acc = 0u;
             for (int k = 0; k < w; ++k) acc += y[(size_t)j * w + k];
             o[j] = acc;
+        }
+    }
+    return 0;
+}
+
+// INT, sliding reading (SURVEY 8(c) INT.1 alternative, 8(f) f1; BJ "boxcar integration over a set of pulse
+// widths"; reading INT.1s): the stride-1 boxcar
+//   n = ns - w + 1;  I^s_w[i][t] = sum_{k<w} Y[i][t + k],  0 <= t < n.
+// Every output is a full-width sum (no partial windows at the edges); w = 1 is Y itself.
+int oracle_integrate_sliding(const uint32_t* Y, size_t stride, int nrows, int ns, int w,
+                             uint32_t* I, size_t i_stride) {
+    if (w <= 0 || w > ns) return -1;
+    const int n = ns - w + 1;
+    for (int i = 0; i < nrows; ++i) {
+        const uint32_t* y = Y + (size_t)i * stride;
+        uint32_t* o = I + (size_t)i * i_stride;
+        for (int t = 0; t < n; ++t) {
+            uint32_t acc = 0u;
+            for (int k = 0; k < w; ++k) acc += y[(size_t)t + k];
+            o[t] = acc;
+        }
+    }
+    return 0;
+}
+
+// DD with a channel mask ("zapped channels"; reading DD.7m): channels whose mask byte is 0
+// are left out of the sum, every other channel contributes exactly as in oracle_dedisperse.
+int oracle_dedisperse_masked(const uint8_t* X, int nchan, size_t in_stride, const uint8_t* mask,
+                             const int32_t* delay, int nrows, int ns, uint32_t* Y, size_t out_stride) {
+    for (int i = 0; i < nrows; ++i) {
+        uint32_t* y = Y + (size_t)i * out_stride;
+        for (int t = 0; t < ns; ++t) y[t] = 0u;
+        for (int c = 0; c < nchan; ++c) {
+            if (mask[c] == 0) continue;
+            const int32_t d = delay[(size_t)i * nchan + c];
+            if (d < 0 || (size_t)d + (size_t)ns > in_stride) return -2;
+            const uint8_t* x = X + (size_t)c * in_stride + d;
+            for (int t = 0; t < ns; ++t) y[t] += (uint32_t)x[t];
         }
     }
     return 0;

@@ -379,3 +379,95 @@ def test_all_cores_leg_equals_pure_python_brute_force_and_single_thread_leg():
     Sm, Ym = oracle.subband_mt(Xc, d1, d2, 8, ns)
     assert np.array_equal(S1, Sm) and np.array_equal(Y2, Ym)
     assert oracle.mt_threads() >= 1
+
+
+# ----------------------------------------------------------------------------- INT.1s: sliding boxcar (8(f) f1)
+def test_sliding_boxcar_closed_forms_and_relation_to_block_sums():
+    """oracle.integrate_sliding against what fixes it: a constant series gives w*v, a single impulse gives a
+    run of w copies ending at its position, numpy's cumulative-sum difference is the third implementation,
+    and the block sums of oracle.integrate are its samples at multiples of w (INT.4 invariant)."""
+    rng = np.random.default_rng(5)
+    ns = 53
+    c = np.full((2, ns), 7, dtype=np.uint32)
+    for w in (1, 2, 3, 4, 8, 53):
+        I = oracle.integrate_sliding(c, w)
+        assert I.shape == (2, ns - w + 1) and (I == 7 * w).all()
+    imp = np.zeros((1, ns), dtype=np.uint32)
+    imp[0, 20] = 9
+    for w in (1, 2, 4, 8):
+        I = oracle.integrate_sliding(imp, w)[0]
+        want = np.zeros(ns - w + 1, dtype=np.uint32)
+        want[20 - w + 1: 21] = 9                      # windows t .. t+w-1 that contain sample 20
+        assert np.array_equal(I, want)
+    Y = rng.integers(0, 400000, size=(3, ns), dtype=np.uint32)
+    cs = np.concatenate([np.zeros((3, 1), dtype=np.uint64), np.cumsum(Y.astype(np.uint64), axis=1)], axis=1)
+    for w in (1, 2, 3, 4, 5, 8, 16, 32):
+        I = oracle.integrate_sliding(Y, w)
+        assert np.array_equal(I.astype(np.uint64), cs[:, w:] - cs[:, :-w])
+        D = oracle.integrate(Y, w)
+        assert np.array_equal(I[:, ::w][:, : D.shape[1]], D)      # decimated planes are a subset
+    with pytest.raises(ValueError):
+        oracle.integrate_sliding(Y, ns + 1)
+
+
+def test_sliding_boxcar_recovers_a_misaligned_pulse_at_its_width():
+    """SURVEY INT.1: with decimating block sums a width-4 pulse starting 1-2 samples off a multiple of 4 peaks
+    at a narrower width; the stride-1 boxcar recovers width 4 and the true start sample."""
+    import dataclasses
+    base = configs.tiny()
+    p = dataclasses.replace(base.fixed_pulses[0], t0=2002)
+    cfg = dataclasses.replace(base, fixed_pulses=(p,))
+    d = oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s)
+    X, pulses = filterbank.make_filterbank(cfg, cfg.nsamp_out + int(d.max()))
+    assert pulses[0].t0 == 2002 and pulses[0].width == 4
+    Y = oracle.dedisperse(X, d, cfg.nsamp_out)
+    _, S, A = oracle.search_sliding(Y, cfg.widths)
+    i, j = np.unravel_index(np.argmax(S), S.shape)
+    assert cfg.dm_list()[i] == 17.0 and cfg.widths[j] == 4 and A[i, j] == 2002
+    _, Sd, _ = oracle.search(Y, cfg.widths)
+    id_, jd = np.unravel_index(np.argmax(Sd), Sd.shape)
+    assert cfg.dm_list()[id_] == 17.0 and cfg.widths[jd] == 2     # decimation splits the pulse over two blocks
+    assert S[i, j] > Sd[id_, jd]
+
+
+# ----------------------------------------------------------------------------- DD.7m: channel mask (8(f) f4)
+def test_masked_dedispersion_equals_dedispersion_of_the_kept_channels():
+    """oracle.dedisperse_masked against the definitions that fix it: an all-ones mask is the plain sum; a
+    masked channel contributes nothing whatever it holds; the result equals the pure-Python brute force over
+    the kept channels only; and linearity: masked + complement = full."""
+    f, dms, ts, delay, X = small_case(21, nchan=7, ndm=6, ns=41)
+    full = oracle.dedisperse(X, delay, 41)
+    assert np.array_equal(oracle.dedisperse_masked(X, np.ones(7, np.uint8), delay, 41), full)
+    mask = np.array([1, 0, 1, 1, 0, 1, 1], dtype=np.uint8)
+    got = oracle.dedisperse_masked(X, mask, delay, 41)
+    keep = [c for c in range(7) if mask[c]]
+    want = py_dedisperse([X[c] for c in keep], [[row[c] for c in keep] for row in delay.tolist()], 41)
+    assert got.tolist() == want
+    X2 = X.copy()
+    X2[mask == 0] = 255                                  # what a zapped channel holds does not matter
+    assert np.array_equal(oracle.dedisperse_masked(X2, mask, delay, 41), got)
+    assert np.array_equal(got + oracle.dedisperse_masked(X, 1 - mask, delay, 41), full)
+    assert (oracle.dedisperse_masked(X, np.zeros(7, np.uint8), delay, 41) == 0).all()
+
+
+# ----------------------------------------------------------------------------- batches (8(f) f3; P:104, P:128)
+def test_consecutive_batches_with_carried_samples_equal_one_long_dedispersion():
+    """The paper searches consecutive batches of one observation ("10 batches").  Dedispersing
+    batch b from samples [b*ns, b*ns + ns + max_delay) -- i.e. keeping the last max_delay samples of the
+    previous upload and appending ns new ones -- gives exactly the columns [b*ns, (b+1)*ns) of one long
+    dedispersion: pure-Python brute force on the long series is the reference."""
+    f, dms, ts, delay, _ = small_case(31, nchan=5, ndm=4, ns=20)
+    md = int(delay.max())
+    nb, ns = 3, 20
+    rng = np.random.default_rng(32)
+    X = rng.integers(0, 256, size=(5, nb * ns + md), dtype=np.uint8)
+    long_ = np.array(py_dedisperse(X, delay.tolist(), nb * ns), dtype=np.uint32)
+    window = np.zeros((5, ns + md), dtype=np.uint8)
+    for b in range(nb):
+        if b == 0:
+            window[:] = X[:, : ns + md]
+        else:
+            window[:, :md] = window[:, ns: ns + md].copy()      # carried tail of the previous batch
+            window[:, md:] = X[:, b * ns + md: (b + 1) * ns + md]  # ns new samples
+        Yb = oracle.dedisperse(np.ascontiguousarray(window), delay, ns)
+        assert np.array_equal(Yb, long_[:, b * ns: (b + 1) * ns])
