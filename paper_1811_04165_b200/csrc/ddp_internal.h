@@ -43,15 +43,19 @@ struct DdpCompiled;  // runtime kernel handle (ddp_rt.cpp)
 // Merged staging (staging genes 3 / 4): per DM tile of TD trials and per group of G adjacent reduction rows,
 // the distinct tuples of relative delays ("variants") and which variant every trial uses.  Depends on the
 // delay table, TD and G only, so it is built once on the host and kept in the workspace, instead of being
-// rediscovered by every block.  blob layout (all per tile t < ntiles, global group gg < ngg = rows / G):
-//   nvar  int32 [ntiles][ngg]                     at byte 0
-//   vdesc int32 [ntiles][ngg][vmax][2 + G]        at byte off_vdesc   {min delta, max delta, tau[0..G)}
-//   vid   uint8 [ntiles][ngg][TD]                 at byte off_vid     variant of every trial
+// rediscovered by every block.  blob = one record of rw int32 words per (tile t < ntiles, global group
+// gg < ngg = rows / G), tile-major:
+//   [0] variants   [1] span = delta of the last live trial   [2..3] 0
+//   [4 .. 4+G)        delay of the tile's first trial for the G rows      (window starts)
+//   [4+G .. 4+2G)     delay of the tile's last live trial                 (window ends)
+//   [4+2G .. +vcap)   per variant: tau[1..G) as signed bytes (tau[0] = 0)
+//   [.. + TD)         per trial: variant << 24 | delta
 // delta = d[j][r0] - d[first trial][r0]; tau[m] = (d[j][r0+m] - d[j][r0]) - (same for the tile's first trial).
 struct DdpMergeTable {
-    int vmax = 0, ntiles = 0, ngg = 0;
-    int64_t off_vdesc = 0, off_vid = 0;
-    std::vector<unsigned char> blob;
+    int vmax = 0, vcap = 0, rw = 0, ntiles = 0, ngg = 0;
+    std::vector<int32_t> nvar;                 // [ntiles][ngg]
+    mutable std::map<int, int> rows_max;       // chunk length U -> largest sum of variants over a chunk's groups
+    mutable std::vector<unsigned char> blob;   // device image, built by ddp_merge_table_blob on first launch
 };
 
 struct ddp_plan {
@@ -71,7 +75,6 @@ struct ddp_plan {
     // configurations + validity caches
     ddp_kcfg kcfg[DDP_K_COUNT];
     mutable std::map<int, int> spread_cache[3];              // dedisp kernel -> (TD -> max window spread)
-    mutable std::map<std::pair<int, int>, int> vmax_cache[3]; // dedisp kernel -> ((TD, G) -> max variants per group)
     mutable std::map<std::pair<int, int>, DdpMergeTable> merge_tables[3];  // host copies, built on first use
     int64_t merge_capacity = 0;                               // bytes of the workspace region for the resident table
     unsigned char* d_merge = nullptr;                         // device: resident merge table (one (kernel, TD, G) at a time)
@@ -98,11 +101,13 @@ bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
 // Merged staging (staging genes 3 / 4: G = 2 / 4 adjacent rows pre-summed exactly; uint8 dedispersion only).
 inline int ddp_merge_group(const ddp_kcfg& c) { return c.staging == 3 ? 2 : (c.staging == 4 ? 4 : 0); }
 int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G);  // largest number of distinct relative-shift tuples
-struct DdpMergeGeom { int vmax, lw, le; };
-int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G, int vmax);
-const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, int G);
+struct DdpMergeGeom { int vmax, vcap, rw, rows_max, lw, le; };
+int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G);
+int ddp_merge_rows_max(const ddp_plan* p, ddp_kernel k, int TD, int G, int U);
+const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, int G);         // counts only
+const std::vector<unsigned char>& ddp_merge_table_blob(const ddp_plan* p, ddp_kernel k, int TD, int G);
 DdpMergeGeom ddp_merge_geom(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
-#define DDP_MERGE_VMAX_LIMIT 32                 // half of the kernel's 64 hash slots per group
+#define DDP_MERGE_VMAX_LIMIT 32                 // variants per group the kernel's tables allow
 bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::string* why);
 const std::vector<ddp_kcfg>& ddp_valid_set(const ddp_plan* p, ddp_kernel k);
 bool ddp_kcfg_equal(const ddp_kcfg& a, const ddp_kcfg& b);

@@ -666,211 +666,82 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
 // values ("variants": 2-3 for pairs, 4-8 for quads at the BASELINE.json configs) because the rounded
 // delays of neighbouring channels move almost in lockstep.  So per tile and group the block builds, for
 // every variant v, the row
-//     PW_v[y] = sum_{m<G} X[r0+m][tile_t + d[0][r0] + y + (d[j][r0+m] - d[j][r0])]        (j any trial of v)
+//     PW_v[y] = sum_{m<G} X[r0+m][tile_t + d[0][r0+m] + tau_v[m] + y]     tau_v[m] = relative shift of v minus that of trial 0
 // once, and every trial j of that variant then adds PW_v[y + (d[j][r0] - d[0][r0])]: one shared-memory
 // word and one add per 2G (sample, channel) pairs instead of LOP3 + PRMT + two adds per 4.  The result
 // is bit-identical to the plain sum (same integers, regrouped); nothing is approximated.
 //
 // Layout.  Rows are kept as 2 x 16-bit lanes per word holding samples (y, y + H), H = TT/2, so a delayed
 // window starts at ANY word whatever the delay (no byte- or element-shifted copies), and a thread's K
-// words are words {32K*(tx/32) + tx%32 + 32k}: every LDS.32 of a warp is conflict free.  Per chunk of U
-// channels: TMA bulk copies bring each channel's raw window (as the packed kernel); `stage1` expands it
-// to E_r[z] = raw[z] | raw[z + H] << 16; `stage2` sums the G expansions of a group at the variant's
-// shifts into PW_v over the y-range its trials need; the trial loop adds PW words into packed 16-bit
-// accumulators, flushed into the uint32 output every 256 channels (WIDE: plain stores the first time,
-// fire-and-forget RED.ADD afterwards).  Which variant a trial uses, and each variant's shifts and
-// y-range, depend on the delay table, TD and G only: the host tabulates them once per plan
-// (DdpMergeTable, ddp_plan.cpp) and the block copies the entries of its DM tile per superchunk of 64
-// channels, together with the delays it needs (first channel of every group for all trials; first and
-// last trial for every channel).
+// words are words {32K*(tx/32) + tx%32 + 32k}: every LDS.32 of a warp is conflict free.
+//
+// Schedule.  The kernel is PERSISTENT: the grid is one block per SM (or as many as fit) and every block
+// walks a contiguous range of work units (tile, segment of <= 256 reduction rows) as ONE stream of chunks
+// of U rows, software-pipelined over the chunks with a single __syncthreads per chunk -- the pipeline never
+// drains between units.  In iteration n the block
+//     schedules chunk n+5 (one thread: unit/tile arithmetic, bulk copy of the chunk's host-table records),
+//     turns the records of chunk n+4 into shared-memory descriptors (TMA extents, row and window offsets),
+//     issues the TMA bulk copies of the raw windows of chunk n+3,
+//     expands chunk n+2:  raw bytes -> E rows  (samples (z, z + H) of each channel as 2 x 16-bit lanes),
+//     builds   chunk n+1:  E rows -> variant rows PW_v,
+//     sums     chunk n:    every trial adds its variant row at its offset into packed 16-bit accumulators,
+// and at the last chunk of a unit flushes the accumulators: plain stores when the reduction is one segment
+// (subband step 1), RED.ADD into the zeroed output otherwise (256 rows * 255 = 65280 fits the lanes).
+// Which variant a trial uses, every variant's shifts and the tile's first / last delays depend on the delay
+// table, TD and G only: the host tabulates them once per plan (DdpMergeTable, ddp_plan.cpp), one record per
+// (DM tile, group), so the kernel never reads the delay table.
+#define DDP_MRG_DEPTH 8   // descriptor ring slots (a chunk's descriptors live for 5 iterations)
+#define DDP_MRG_EPAD 16   // words in front of every E row (variant shifts may be negative)
 template <int SPT, int DPT, int U, int G, bool WIDE, bool OUT16>
 __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) {
     static_assert(SPT >= 2 && U % G == 0 && (G == 2 || G == 4), "merged staging works on 2-sample words and whole groups");
-    static_assert(!(WIDE && OUT16), "a uint16 result never needs the wide flush");
+    static_assert(!(WIDE && OUT16), "a uint16 result never needs more than one segment");
     extern __shared__ __align__(128) unsigned char ddp_smem[];
     constexpr int K = SPT / 2;   // words per thread
     constexpr int NG = U / G;    // groups per chunk
-    constexpr int SC = 64;       // channels per delay superchunk (multiple of every U)
-    constexpr int NGS = SC / G;  // groups per superchunk
-    constexpr int VW = 2 + G;    // ints per variant descriptor {min delta, max delta, tau[G]}
-    constexpr int FL = 256;      // channels between flushes of the 16-bit lanes
+    constexpr int FL = 256;      // reduction rows per segment (16-bit lanes: 256 * 255 < 65536)
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int nthreads = blockDim.x * blockDim.y;
     const int tid = ty * blockDim.x + tx;
     const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
     const int TT = blockDim.x * SPT, TD = blockDim.y * DPT, H = TT >> 1;
-    const int g = blockIdx.z;
-    const int tile_t = blockIdx.x * TT;
-    const int tile_dm = blockIdx.y * TD;
-    const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
-    const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)g * p.in_group_stride;
-    const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
-    const int win = p.win, winw = win >> 2, lw = p.lw, le = p.le, vmax = p.vmax;
-    // this block's rows of the host table: tile blockIdx.y, groups from gg0 on
-    const ddp_i64 mrow = (ddp_i64)blockIdx.y * p.meta_ngg + (ddp_i64)g * p.meta_gg0_stride;
-    const int* m_nvar = (const int*)p.meta + mrow;
-    const int* m_vdesc = (const int*)(p.meta + p.meta_vdesc_off) + mrow * vmax * VW;
-    const ddp_u8* m_vid = p.meta + p.meta_vid_off + mrow * TD;
+    const int win = p.win, lw = p.lw, le = p.le, RW = p.meta_rw, VCAP = p.vmax, rows_max = p.rows_max;
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it); every region starts 16-byte aligned
-    ddp_u32* pw = (ddp_u32*)ddp_smem;                                  // [2][NG][vmax][lw]
-    ddp_u32* ebuf = pw + (size_t)2 * NG * vmax * lw;                   // [U][le]
-    int* dbase = (int*)(ebuf + (size_t)U * le);                        // [2][TD][NGS] delay of the first channel of every group
-    int* dmm = dbase + (size_t)2 * TD * NGS;                           // [2][2][SC] delay of the first / last live trial per channel
-    ddp_u32* offs = (ddp_u32*)(dmm + 2 * 2 * SC);                      // [2][TD][NG]
-    int* rowd = (int*)(offs + (((size_t)2 * TD * NG + 3) & ~(size_t)3));  // [NG * vmax][8] variant-row descriptors of the chunk being staged
-    int* vdesc = rowd + (size_t)NG * vmax * 8;                         // [2][NGS][vmax][VW]
-    int* nvar = vdesc + (size_t)2 * NGS * vmax * VW;                   // [2][NGS]
-    ddp_u8* vid = (ddp_u8*)(nvar + 2 * NGS);                           // [2][NGS][TD]
-    unsigned char* raw = (unsigned char*)(((size_t)(vid + (size_t)2 * NGS * TD) + 15) & ~(size_t)15);  // [2][U][win + 16]
-    ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // [2]
-    const int nchunks = p.nred / U;
+    ddp_u32* pw = (ddp_u32*)ddp_smem;                                        // [2][rows_max][lw]
+    ddp_u32* ebuf = pw + (size_t)2 * rows_max * lw;                          // [2][U][le]
+    unsigned char* raw = (unsigned char*)(ebuf + (size_t)2 * U * le);        // [2][U][win + 16]
+    int* stg = (int*)(raw + (size_t)2 * U * (win + 16));                     // [2][NG * RW] host-table records
+    int* ring = stg + (size_t)2 * NG * RW;                                   // [DEPTH][SLOTW]
+    const int SLOTW = (8 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
+    ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2]
+    int* sched = (int*)(mbar + 4);                                           // scheduler cursor {unit, chunk}
+    // ring slot: desc[8] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax} | a0[U] | bytes[U] | carry[U] | nz4[U] |
+    //            rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
+    auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
 
-    // superchunk s -> buffer s & 1: delays and the host table's entries of its groups
-    auto load_super = [&](int s) {
-        const int b = s & 1, r0 = s * SC;
-        const int nrows = (p.nred - r0 < SC ? p.nred - r0 : SC), ngs = nrows / G;
-        int* db = dbase + (size_t)b * TD * NGS;
-        for (int idx = tid; idx < TD * ngs; idx += nthreads) {
-            const int j = idx / ngs, q = idx - j * ngs;
-            db[j * NGS + q] = dl[(ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride + r0 + q * G];
-        }
-        int* mm = dmm + (size_t)b * 2 * SC;
-        for (int idx = tid; idx < 2 * nrows; idx += nthreads) {
-            const int e = idx / nrows, cc = idx - e * nrows;
-            mm[e * SC + cc] = dl[(ddp_i64)(e ? nd - 1 : 0) * p.delay_dm_stride + r0 + cc];
-        }
-        const int gq0 = r0 / G;
-        for (int idx = tid; idx < ngs; idx += nthreads) nvar[b * NGS + idx] = m_nvar[gq0 + idx];
-        for (int idx = tid; idx < ngs * vmax * VW; idx += nthreads)
-            vdesc[(size_t)b * NGS * vmax * VW + idx] = m_vdesc[(ddp_i64)gq0 * vmax * VW + idx];
-        const ddp_u32* vsrc = (const ddp_u32*)(m_vid + (ddp_i64)gq0 * TD);  // TD % 4 == 0 (validity rule): word copies
-        ddp_u32* vdst = (ddp_u32*)(vid + (size_t)b * NGS * TD);
-        for (int idx = tid; idx < (ngs * TD) >> 2; idx += nthreads) vdst[idx] = vsrc[idx];
-    };
-    auto dmin_of = [&](int r) -> int { const int s = r / SC; return dmm[(size_t)(s & 1) * 2 * SC + (r - s * SC)]; };
-    auto dmax_of = [&](int r) -> int { const int s = r / SC; return dmm[(size_t)(s & 1) * 2 * SC + SC + (r - s * SC)]; };
-    // staged extent of reduction row r: aligned start (elements from the row start) and words to stage
-    auto row_extent = [&](int r, ddp_i64& a0, int& lenw) {
-        const int dmin = dmin_of(r), dmax = dmax_of(r);  // delays do not decrease with the trial index
-        a0 = ((ddp_i64)tile_t + dmin) & ~(ddp_i64)15;
-        int need = (((int)((ddp_i64)tile_t + dmin - a0) + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
-        need = (need + 3) & ~3;
-        if (need > winw) need = winw;
-        ddp_i64 l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
-        lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
-    };
-    auto tma_issue = [&](int c) {  // warp 0, lane u < U: raw window of row u of chunk c -> raw slot c & 1
-        unsigned char* dst = raw + (size_t)(c & 1) * U * (win + 16);
-        ddp_i64 a0 = 0;
-        int lenw = 0;
-        if (lane < U) row_extent(c * U + lane, a0, lenw);
-        const ddp_u32 bytes = lenw > 0 ? (ddp_u32)lenw * 4u + 16u : 0u;
-        ddp_u32 total = bytes;
+    // this block's units: a contiguous range, tile-major / segment-minor, so that the segments of a tile
+    // follow each other (their output words are still in L2 when the next segment adds to them)
+    const int nseg = WIDE ? p.nseg : 1;
+    const long long nun = p.nunits;
+    const int unit_lo = (int)((long long)blockIdx.x * nun / gridDim.x);
+    const int unit_hi = (int)((long long)(blockIdx.x + 1) * nun / gridDim.x);
+    // chunks of this block's stream (every thread needs the trip count)
+    int nstream = 0;
+    {
+        const int full = FL / U, last = (p.nred - (nseg - 1) * FL) / U;
+        for (int u = unit_lo; u < unit_hi; ++u) nstream += (u % nseg == nseg - 1) ? last : full;
+    }
+
+    if (tid == 0) {
 #pragma unroll
-        for (int d = 16; d >= 1; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
-        if (lane == 0) ddp_mbar_expect_tx(&mbar[c & 1], total);
-        __syncwarp();
-        if (bytes)
-            ddp_bulk_g2s(dst + (size_t)lane * (win + 16), in_g + (ddp_i64)(c * U + lane) * p.in_row_stride + a0, bytes,
-                         &mbar[c & 1]);
-    };
-    // chunk c: raw slot c & 1 -> E rows (samples (z, z + H) of each channel as 2 x 16-bit lanes)
-    const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
-    auto stage1 = [&](int c) {
-        for (int unit = warp; unit < (U << parts_log2); unit += nwarps) {
-            const int u = unit >> parts_log2, part = unit & ((1 << parts_log2) - 1);
-            const int dmin = dmin_of(c * U + u), dmax = dmax_of(c * U + u);
-            const int carry = (int)(((ddp_i64)tile_t + dmin) & 15);
-            const int nz4 = (carry + (dmax - dmin) + H + 3) >> 2;  // groups of four z
-            const ddp_u32* src = (const ddp_u32*)(raw + ((size_t)(c & 1) * U + u) * (win + 16));
-            ddp_u32* dst = ebuf + (size_t)u * le;
-            const int hq = H >> 2;
-            for (int q4 = (part << 5) + lane; q4 < nz4; q4 += (32 << parts_log2)) {
-                const ddp_u32 lo = src[q4], hi = src[q4 + hq];
-                const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
-                const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
-                *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
-                                                     __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
-            }
-        }
-    };
-    // chunk c: one descriptor per variant row (group q, variant v) that stage2 will build, compacted over the
-    // groups: {ylo, yhi, destination word offset in pw, G source word offsets in ebuf}; rowd[7] (unused word
-    // of row 0) holds the row count.  Runs beside stage1 (before the barrier that precedes stage2).
-    auto prep_rows = [&](int c) {
-        const int sb = (c * U / SC) & 1, qs0 = (c * U % SC) / G;
-        const int* nv_s = nvar + sb * NGS + qs0;
-        for (int r = tid; r < NG * vmax; r += nthreads) {
-            const int q = r / vmax, v = r - q * vmax;
-            int base = 0, total = 0;
-#pragma unroll
-            for (int qq = 0; qq < NG; ++qq) {
-                const int nv = nv_s[qq];
-                if (qq < q) base += nv;
-                total += nv;
-            }
-            if (r == 0) rowd[7] = total;
-            if (v < nv_s[q]) {
-                const int* vd = vdesc + (((size_t)sb * NGS + qs0 + q) * vmax + v) * VW;
-                int* o = rowd + (size_t)(base + v) * 8;
-                o[0] = vd[0];
-                o[1] = vd[1] + H;
-                o[2] = (int)((((size_t)(c & 1) * NG + q) * vmax + v) * lw);
-#pragma unroll
-                for (int m = 0; m < G; ++m) {
-                    const int carry = (int)(((ddp_i64)tile_t + dmin_of(c * U + q * G + m)) & 15);
-                    o[3 + m] = (q * G + m) * le + carry + vd[2 + m];
-                }
-            }
-        }
-    };
-    // chunk c: E rows -> variant rows PW_v of every group, buffer c & 1.  Rows are split into 32-word blocks
-    // handed out to the warps round robin; rows carry 32 words of slack, so whole blocks are computed.
-    auto stage2 = [&](int c) {
-        const int R = rowd[7];
-        int pl2 = 0;
-        while ((R << pl2) < nwarps && pl2 < 5) ++pl2;  // parts per row: about one unit per warp or more
-        for (int unit = warp; unit < (R << pl2); unit += nwarps) {
-            const int row = unit >> pl2, part = unit & ((1 << pl2) - 1);
-            const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
-            const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-            const int ylo = d0.x, yhi = d0.y;
-            const ddp_u32* e0 = ebuf + d0.w + lane;
-            const ddp_u32* e1 = ebuf + d1.x + lane;
-            const ddp_u32* e2 = ebuf + (G > 2 ? d1.y : 0) + lane;
-            const ddp_u32* e3 = ebuf + (G > 2 ? d1.z : 0) + lane;
-            ddp_u32* dst = pw + d0.z + lane;
-            const int step = 32 << pl2;
-            int y = ylo + (part << 5);
-            for (; y + step < yhi; y += 2 * step) {  // two blocks per trip: twice the loads in flight
-                ddp_u32 s0 = e0[y] + e1[y], s1 = e0[y + step] + e1[y + step];
-                if constexpr (G > 2) {
-                    s0 += e2[y] + e3[y];
-                    s1 += e2[y + step] + e3[y + step];
-                }
-                dst[y] = s0;
-                dst[y + step] = s1;
-            }
-            if (y < yhi) {
-                ddp_u32 s0 = e0[y] + e1[y];
-                if constexpr (G > 2) s0 += e2[y] + e3[y];
-                dst[y] = s0;
-            }
-        }
-    };
-    auto prep_offs = [&](int c) {
-        const int sb = (c * U / SC) & 1, qs0 = (c * U % SC) / G;
-        const int* db = dbase + (size_t)sb * TD * NGS + qs0;
-        const ddp_u8* vi = vid + ((size_t)sb * NGS + qs0) * TD;
-        ddp_u32* ob = offs + (size_t)(c & 1) * TD * NG;
-        for (int idx = tid; idx < TD * NG; idx += nthreads) {
-            const int jj = idx / NG, q = idx - jj * NG;
-            const int delta = db[jj * NGS + q] - db[q];
-            const int v = vi[q * TD + jj];
-            ob[idx] = (ddp_u32)(((((size_t)(c & 1) * NG + q) * vmax + v) * lw + delta) * 4u);
-        }
-    };
+        for (int b = 0; b < 4; ++b) ddp_mbar_init(&mbar[b], 1);
+        ddp_mbar_fence_init();
+        sched[0] = unit_lo;
+        sched[1] = 0;
+    }
+    for (int i = tid; i < DDP_MRG_DEPTH; i += nthreads) slot(i)[5] = 0;  // nothing valid yet
+    __syncthreads();
 
     ddp_u32 acc[DPT][K];
 #pragma unroll
@@ -878,99 +749,245 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
 #pragma unroll
         for (int k = 0; k < K; ++k) acc[j][k] = 0u;
     const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
-    const ddp_u32* lanep = pw + wb;
-    // lanes of word widx hold samples tile_t + widx (low) and tile_t + widx + H (high)
-    auto emit = [&](bool add) {
+
+    for (int n = -5; n < nstream; ++n) {
+        // ---- schedule chunk n + 5 (one thread)
+        if (tid == 0) {
+            const int x = n + 5;
+            int* d = slot(x);
+            const int unit = sched[0], c = sched[1];
+            if (x < nstream && unit < unit_hi) {
+                const int tile = unit / nseg, seg = unit - tile * nseg;
+                const int tt = tile % p.n_ttiles, rest = tile / p.n_ttiles;
+                const int dt = rest % p.n_dtiles, g = rest / p.n_dtiles;
+                const int rows = p.nred - seg * FL < FL ? p.nred - seg * FL : FL;
+                const int nch = WIDE ? rows / U : p.nred / U;
+                const int r0 = seg * FL + c * U;
+                d[0] = tt * TT;
+                d[1] = dt * TD;
+                d[2] = (dt + 1) * TD <= p.ndm ? TD : p.ndm - dt * TD;
+                d[3] = g;
+                d[4] = r0;
+                d[5] = 1 | (c == 0 ? 2 : 0) | (c == nch - 1 ? 4 : 0);
+                const long long rec = ((long long)dt * p.meta_ngg + (long long)g * p.meta_gg0_stride + r0 / G) * RW;
+                ddp_mbar_expect_tx(&mbar[2 + (x & 1)], (ddp_u32)(NG * RW * 4));
+                ddp_bulk_g2s(stg + (size_t)(x & 1) * NG * RW, (const int*)p.meta + rec, (ddp_u32)(NG * RW * 4), &mbar[2 + (x & 1)]);
+                if (c + 1 == nch) { sched[0] = unit + 1; sched[1] = 0; } else { sched[1] = c + 1; }
+            } else {
+                d[5] = 0;
+            }
+        }
+        // ---- descriptors of chunk n + 4 from its records
+        {
+            const int x = n + 4;
+            int* d = slot(x);
+            if (x >= 0 && x < nstream) {
+                const int* rec = stg + (size_t)(x & 1) * NG * RW;
+                ddp_mbar_wait(&mbar[2 + (x & 1)], (ddp_u32)((x >> 1) & 1));
+                const int tile_t = d[0];
+                int* a0s = d + 8;
+                int* byts = a0s + U;
+                int* carr = byts + U;
+                int* nz4s = carr + U;
+                int* rowd = nz4s + U;
+                ddp_u32* offs = (ddp_u32*)(rowd + 8 * rows_max);
+                if (tid < U) {  // TMA extent and expansion length of reduction row tid of the chunk
+                    const int* r = rec + (tid / G) * RW;
+                    const int dmin = r[4 + tid % G], dmax = r[4 + G + tid % G];
+                    const long long src = (long long)tile_t + dmin;
+                    const long long a0 = src & ~15ll;
+                    const int carry = (int)(src - a0);
+                    int need = ((carry + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
+                    need = (need + 3) & ~3;
+                    if (need > (win >> 2)) need = win >> 2;
+                    long long l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
+                    const int lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
+                    a0s[tid] = (int)a0;
+                    byts[tid] = lenw > 0 ? lenw * 4 + 16 : 0;
+                    carr[tid] = carry;
+                    nz4s[tid] = (carry + (dmax - dmin) + H + 3) >> 2;
+                }
+                const int t1 = (tid + nthreads - 32 % nthreads) % nthreads;  // start at warp 1
+                for (int i = t1; i < NG * VCAP; i += nthreads) {
+                    const int q = i / VCAP, v = i - q * VCAP;
+                    const int* r = rec + q * RW;
+                    int base = 0, total = 0, ymax = 0;
 #pragma unroll
-        for (int j = 0; j < DPT; ++j) {
-            const int dm = tile_dm + ty * DPT + j;
-            if (dm < p.ndm) {
+                    for (int qq = 0; qq < NG; ++qq) {
+                        const int nv = rec[qq * RW];
+                        if (qq < q) base += nv;
+                        total += nv;
+                        const int yl = H + rec[qq * RW + 1] + 1;
+                        ymax = yl > ymax ? yl : ymax;
+                    }
+                    if (i == 0) { d[6] = total; d[7] = ymax; }
+                    if (v < r[0]) {
+                        const int code = r[4 + 2 * G + v];
+                        int* o = rowd + (size_t)(base + v) * 8;
+                        o[0] = H + r[1] + 1;
+                        o[1] = (base + v) * lw;
 #pragma unroll
-                for (int k = 0; k < K; ++k) {
-                    const int t = tile_t + wb + 32 * k;
-                    const ddp_u32 lo = acc[j][k] & 0xffffu, hi = acc[j][k] >> 16;
-                    if constexpr (OUT16) {
-                        ddp_u16* orow = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
-                        if (t < p.ns) orow[t] = (ddp_u16)lo;
-                        if (t + H < p.ns) orow[t + H] = (ddp_u16)hi;
+                        for (int m = 0; m < G; ++m) {
+                            const int tau = m == 0 ? 0 : (int)(signed char)((code >> (8 * (m - 1))) & 0xff);
+                            const int carry = (int)(((long long)tile_t + r[4 + m]) & 15);
+                            o[2 + m] = (q * G + m) * le + DDP_MRG_EPAD + carry + tau;
+                        }
+                    }
+                }
+                const int t4 = (tid + nthreads - 128 % nthreads) % nthreads;  // start at warp 4
+                for (int i = t4; i < TD * NG; i += nthreads) {
+                    const int j = i / NG, q = i - j * NG;
+                    int base = 0;
+#pragma unroll
+                    for (int qq = 0; qq < NG; ++qq)
+                        if (qq < q) base += rec[qq * RW];
+                    const ddp_u32 code = (ddp_u32)rec[q * RW + 4 + 2 * G + VCAP + j];
+                    offs[i] = (ddp_u32)(((base + (int)(code >> 24)) * lw + (int)(code & 0xffffffu)) * 4);
+                }
+            }
+        }
+        // ---- TMA: raw windows of chunk n + 3 (warp 0, lane u < U) -> raw slot (n + 3) & 1
+        if (warp == 0) {
+            const int x = n + 3;
+            const int* d = slot(x);
+            if (x >= 0 && x < nstream) {
+                const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)d[3] * p.in_group_stride;
+                const ddp_u32 bytes = lane < U ? (ddp_u32)d[8 + U + lane] : 0u;
+                ddp_u32 total = bytes;
+#pragma unroll
+                for (int s = 16; s >= 1; s >>= 1) total += __shfl_xor_sync(0xffffffffu, total, s);
+                if (lane == 0) ddp_mbar_expect_tx(&mbar[x & 1], total);
+                __syncwarp();
+                if (bytes)
+                    ddp_bulk_g2s(raw + ((size_t)(x & 1) * U + lane) * (win + 16),
+                                 in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[8 + lane], bytes, &mbar[x & 1]);
+            }
+        }
+        // ---- expand chunk n + 2: raw slot -> E rows (samples (z, z + H) of each channel as 2 x 16-bit lanes)
+        {
+            const int x = n + 2;
+            const int* d = slot(x);
+            if (x >= 0 && x < nstream) {
+                ddp_mbar_wait(&mbar[x & 1], (ddp_u32)((x >> 1) & 1));
+                const int* nz4s = d + 8 + 3 * U;
+                int nzmax = 0;
+#pragma unroll
+                for (int u = 0; u < U; ++u) nzmax = nz4s[u] > nzmax ? nz4s[u] : nzmax;
+                const int nblk = (nzmax + 31) >> 5, hq = H >> 2;
+                const int wrot = (warp + x) % nwarps;  // rotate the hand-out so that no warp is always the loaded one
+                for (int it = wrot; it < U * nblk; it += nwarps) {
+                    const int u = it / nblk, q4 = ((it - u * nblk) << 5) + lane;
+                    if (q4 < nz4s[u]) {
+                        const ddp_u32* src = (const ddp_u32*)(raw + ((size_t)(x & 1) * U + u) * (win + 16));
+                        ddp_u32* dst = ebuf + ((size_t)(x & 1) * U + u) * le + DDP_MRG_EPAD;
+                        const ddp_u32 lo = src[q4], hi = src[q4 + hq];
+                        const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
+                        const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
+                        *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
+                                                             __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                    }
+                }
+            }
+        }
+        // ---- build chunk n + 1: E rows -> variant rows of buffer (n + 1) & 1, 128 words per (row, block) item
+        {
+            const int x = n + 1;
+            const int* d = slot(x);
+            if (x >= 0 && x < nstream) {
+                const int R = d[6], nblk = (d[7] + 127) >> 7;
+                const int* rowd = d + 8 + 4 * U;
+                const ddp_u32* eb = ebuf + (size_t)(x & 1) * U * le;
+                ddp_u32* pb = pw + (size_t)(x & 1) * rows_max * lw;
+                const int wrot = (warp + 5 * x) % nwarps;
+                for (int it = wrot; it < R * nblk; it += nwarps) {
+                    const int row = it / nblk, y0 = ((it - row * nblk) << 7) + lane;
+                    const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                    const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
+                    const int ylen = d0.x;
+                    const ddp_u32* e0 = eb + d0.z + y0;
+                    const ddp_u32* e1 = eb + d0.w + y0;
+                    const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0) + y0;
+                    const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0) + y0;
+                    ddp_u32* dst = pb + d0.y + y0;
+                    if (y0 + 96 < ylen) {  // whole item: all loads first
+                        ddp_u32 s[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            s[i] = e0[32 * i] + e1[32 * i];
+                            if constexpr (G > 2) s[i] += e2[32 * i] + e3[32 * i];
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) dst[32 * i] = s[i];
                     } else {
-                        ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
-                        if (add) {  // the words are this thread's own: RED.ADD needs no read-back and no wait
-                            if (t < p.ns) atomicAdd(orow + t, lo);
-                            if (t + H < p.ns) atomicAdd(orow + t + H, hi);
-                        } else {
-                            if (t < p.ns) orow[t] = lo;
-                            if (t + H < p.ns) orow[t + H] = hi;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (y0 + 32 * i < ylen) {
+                                ddp_u32 s0 = e0[32 * i] + e1[32 * i];
+                                if constexpr (G > 2) s0 += e2[32 * i] + e3[32 * i];
+                                dst[32 * i] = s0;
+                            }
                         }
                     }
                 }
             }
-#pragma unroll
-            for (int k = 0; k < K; ++k) acc[j][k] = 0u;
         }
-    };
-
-    if (tid == 0) {
-        ddp_mbar_init(&mbar[0], 1);
-        ddp_mbar_init(&mbar[1], 1);
-        ddp_mbar_fence_init();
-    }
-    load_super(0);
-    __syncthreads();
-    if (warp == 0) {
-        tma_issue(0);
-        if (nchunks > 1) tma_issue(1);
-    }
-    ddp_mbar_wait(&mbar[0], 0u);
-    stage1(0);
-    prep_rows(0);
-    __syncthreads();
-    stage2(0);
-    prep_offs(0);
-    __syncthreads();
-
-    for (int c = 0; c < nchunks; ++c) {
-        const int r0 = c * U;
-        if (r0 % SC == 0 && r0 + SC < p.nred) load_super(r0 / SC + 1);  // visible after this iteration's barriers
-        if (c + 1 < nchunks) {
-            if (warp == 0 && c + 2 < nchunks) tma_issue(c + 2);  // raw slot c & 1 was expanded during iteration c - 1
-            ddp_mbar_wait(&mbar[(c + 1) & 1], (ddp_u32)(((c + 1) >> 1) & 1));
-            stage1(c + 1);
-            prep_rows(c + 1);
-            __syncthreads();
-            stage2(c + 1);
-            prep_offs(c + 1);
-        }
-        const ddp_u32* ob = offs + ((size_t)(c & 1) * TD + ty * DPT) * NG;
+        // ---- sum chunk n: every trial adds its variant rows, then (last chunk of a unit) flush
+        if (n >= 0) {
+            const int* d = slot(n);
+            const ddp_u32* ob = (const ddp_u32*)(d + 8 + 4 * U + 8 * rows_max) + (size_t)(ty * DPT) * NG;
+            const unsigned char* lanep = (const unsigned char*)(pw + (size_t)(n & 1) * rows_max * lw + wb);
 #pragma unroll
-        for (int j = 0; j < DPT; ++j) {
-            ddp_u32 o[NG];
-            if constexpr (NG == 4) {
-                const uint4 v = *(const uint4*)(ob + j * NG);
-                o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
-            } else if constexpr (NG == 2) {
-                const uint2 v = *(const uint2*)(ob + j * NG);
-                o[0] = v.x; o[1] = v.y;
-            } else {
+            for (int j = 0; j < DPT; ++j) {
+                ddp_u32 o[NG];
+                if constexpr (NG == 4) {
+                    const uint4 v = *(const uint4*)(ob + j * NG);
+                    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+                } else if constexpr (NG == 2) {
+                    const uint2 v = *(const uint2*)(ob + j * NG);
+                    o[0] = v.x; o[1] = v.y;
+                } else {
 #pragma unroll
-                for (int q = 0; q < NG; ++q) o[q] = ob[j * NG + q];
+                    for (int q = 0; q < NG; ++q) o[q] = ob[j * NG + q];
+                }
+#pragma unroll
+                for (int q = 0; q < NG; ++q) {
+                    const ddp_u32* wp = (const ddp_u32*)(lanep + o[q]);
+#pragma unroll
+                    for (int k = 0; k < K; ++k) acc[j][k] += wp[32 * k];
+                }
             }
+            if (d[5] & 4) {  // block-uniform: last chunk of the unit
+                const int tile_t = d[0], tile_dm = d[1], g = d[3];
 #pragma unroll
-            for (int q = 0; q < NG; ++q) {
-                const ddp_u32* wp = (const ddp_u32*)((const unsigned char*)lanep + o[q]);
+                for (int j = 0; j < DPT; ++j) {
+                    const int dm = tile_dm + ty * DPT + j;
+                    if (dm < p.ndm) {
 #pragma unroll
-                for (int k = 0; k < K; ++k) acc[j][k] += wp[32 * k];
+                        for (int k = 0; k < K; ++k) {
+                            const int t = tile_t + wb + 32 * k;
+                            const ddp_u32 lo = acc[j][k] & 0xffffu, hi = acc[j][k] >> 16;
+                            if constexpr (OUT16) {
+                                ddp_u16* orow = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+                                if (t < p.ns) orow[t] = (ddp_u16)lo;
+                                if (t + H < p.ns) orow[t + H] = (ddp_u16)hi;
+                            } else {
+                                ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
+                                if constexpr (WIDE) {  // several segments add into the zeroed output: fire-and-forget RED.ADD
+                                    if (t < p.ns) atomicAdd(orow + t, lo);
+                                    if (t + H < p.ns) atomicAdd(orow + t + H, hi);
+                                } else {
+                                    if (t < p.ns) orow[t] = lo;
+                                    if (t + H < p.ns) orow[t + H] = hi;
+                                }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int k = 0; k < K; ++k) acc[j][k] = 0u;
+                }
             }
-        }
-        if constexpr (WIDE) {
-            if ((r0 + U) % FL == 0) emit(r0 + U > FL);  // block-uniform
         }
         __syncthreads();
-    }
-    if constexpr (WIDE) {
-        if (p.nred % FL != 0) emit(true);  // WIDE means nred > FL: at least one flush came before
-    } else {
-        emit(false);
     }
 }
 

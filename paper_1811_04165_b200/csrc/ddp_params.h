@@ -26,14 +26,17 @@ struct DdpDedispParams {
     int ns;                      // output samples per row
     int win;                     // staged modes: elements of one staged row window in shared memory
     int one;                     // the value 1, unknown to the compiler (packed kernel: adds issued as IMAD)
-    int vmax;                    // merged staging: rows reserved per group = largest variant count of the plan
+    int vmax;                    // merged staging: variant slots per table record (largest variant count of the plan, padded to 4)
     int lw;                      // merged staging: words per variant row  (TT/2 + largest window spread, padded)
     int le;                      // merged staging: words per expanded channel row
-    const unsigned char* meta;   // merged staging: resident DdpMergeTable blob (device)
-    long long meta_vdesc_off;    //   byte offsets of its vdesc and vid arrays
-    long long meta_vid_off;
+    int rows_max;                // merged staging: variant rows per buffer = largest sum of variant counts over a chunk's groups
+    const unsigned char* meta;   // merged staging: resident DdpMergeTable blob (device), one record per (DM tile, group)
+    int meta_rw;                 //   int32 words per record
     int meta_ngg;                //   groups per DM tile in the table (all subbands)
     int meta_gg0_stride;         //   table groups between consecutive kernel groups g (subband step 1: cps / G; direct: 0)
+    int n_ttiles, n_dtiles;      // merged staging (persistent kernel): time tiles, DM tiles,
+    int nseg;                    //   segments of <= 256 reduction rows per tile,
+    int nunits;                  //   work units = groups * n_dtiles * n_ttiles * nseg
 };
 
 // Integration: plane k holds I_w[i][j] = sum_{m<w} in[i][j*w+m] for w = width[k] > 1.

@@ -281,56 +281,46 @@ int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD) {
     p->spread_cache[which][TD] = mx;
     return mx;
 }
-// Merged staging: the largest number of distinct tuples (d[j][r0+m] - d[j][r0])_{m<G} over the TD trials of
-// any DM tile and any group of G adjacent reduction rows -- the rows per group the kernel reserves.
-int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G) {
-    const int which = k == DDP_K_DIRECT ? 0 : (k == DDP_K_SUB1 ? 1 : 2);
-    auto key = std::make_pair(TD, G);
-    auto it = p->vmax_cache[which].find(key);
-    if (it != p->vmax_cache[which].end()) return it->second;
-    const std::vector<int32_t>& t = which == 0 ? p->delay : (which == 1 ? p->d1 : p->d2);
-    const int ni = which == 0 ? p->ndm : (which == 1 ? p->ncoarse : p->nfine);
-    const int nc = which == 2 ? p->nsub : p->nchan;
-    const int nred = ddp_kgeom(p, k).nred;  // groups never straddle a subband: nred % G == 0 is a validity rule
-    int vmax = 0;
-    std::vector<int32_t> found;  // distinct tuples of the current (tile, group), G - 1 ints each
-    for (int lo = 0; lo < ni && vmax <= DDP_MERGE_VMAX_LIMIT; lo += TD) {
-        const int hi = std::min(lo + TD, ni);
-        for (int r0 = 0; r0 + G <= nc; r0 += G) {
-            if (nred % G != 0) continue;
-            found.clear();
-            int nv = 0;
-            for (int j = lo; j < hi; ++j) {
-                const int32_t* d = &t[(size_t)j * nc + r0];
-                int v = 0;
-                for (; v < nv; ++v) {
-                    bool same = true;
-                    for (int m = 1; m < G; ++m) same = same && found[(size_t)v * (G - 1) + m - 1] == d[m] - d[0];
-                    if (same) break;
-                }
-                if (v == nv) {
-                    for (int m = 1; m < G; ++m) found.push_back(d[m] - d[0]);
-                    ++nv;
-                }
-            }
-            vmax = std::max(vmax, nv);
-        }
-    }
-    p->vmax_cache[which][key] = vmax;
-    return vmax;
-}
-static void merge_dims(const ddp_plan* p, ddp_kernel k, int TD, int G, int* ni, int* nc) {
+// Merged staging.  One scan of the delay table per (kernel, TD, G): for every DM tile of TD trials and every
+// group of G adjacent reduction rows, the distinct tuples tau[m] = (d[j][r0+m] - d[j][r0]) - (same for the tile's
+// first trial) over the tile's trials ("variants"), which variant every trial uses, and its window offset
+// delta = d[j][r0] - d[first][r0].  Record layout in DdpMergeTable (ddp_internal.h).
+static void merge_dims(const ddp_plan* p, ddp_kernel k, int* ni, int* nc) {
     *ni = k == DDP_K_DIRECT ? p->ndm : p->ncoarse;
     *nc = p->nchan;
-    (void)TD; (void)G;
 }
-int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G, int vmax) {
-    int ni, nc;
-    merge_dims(p, k, TD, G, &ni, &nc);
-    const int64_t ntiles = (ni + TD - 1) / TD, ngg = nc / G;
-    return round_up(ntiles * ngg * 4, 16) + round_up(ntiles * ngg * vmax * (2 + G) * 4, 16) + round_up(ntiles * ngg * TD, 16);
+// Variants of one (tile, group): tau[v][0..4), vid[j] for j < TD; returns the count, or -1 when the group cannot
+// be served (a shift outside +-15 words, more than DDP_MERGE_VMAX_LIMIT variants, a delay that decreases with
+// the trial index).  Trials past the end of a ragged tile repeat the last live one.
+static int merge_scan_group(const int32_t* t, int nc, int lo, int nd, int TD, int r0, int G, int32_t* tau,
+                            unsigned char* vid) {
+    const int32_t* d0 = &t[(size_t)lo * nc + r0];
+    int nv = 0;
+    for (int j = 0; j < TD; ++j) {
+        const int32_t* d = &t[(size_t)(lo + std::min(j, nd - 1)) * nc + r0];
+        int32_t tj[4] = {0, 0, 0, 0};
+        for (int m = 1; m < G; ++m) tj[m] = (d[m] - d[0]) - (d0[m] - d0[0]);
+        int v = 0;
+        for (; v < nv; ++v) {
+            bool same = true;
+            for (int m = 1; m < G; ++m) same = same && tau[v * 4 + m] == tj[m];
+            if (same) break;
+        }
+        if (v == nv) {
+            if (nv == DDP_MERGE_VMAX_LIMIT) return -1;
+            for (int m = 1; m < G; ++m)
+                if (tj[m] < -15 || tj[m] > 15) return -1;  // E rows carry 16 words in front
+            for (int m = 0; m < 4; ++m) tau[nv * 4 + m] = tj[m];
+            ++nv;
+        }
+        vid[j] = (unsigned char)v;
+        if (d[0] - d0[0] < 0 || d[0] - d0[0] >= (1 << 24)) return -1;
+        for (int m = 0; m < G; ++m)
+            if (d[m] < d0[m]) return -1;  // window starts are the first trial's delays
+    }
+    return nv;
 }
-// The full table (see DdpMergeTable).  Trials beyond the last one of a ragged tile repeat the last trial.
+// Light part (variant counts): what the validity rules and the shared-memory size need.
 const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, int G) {
     const int which = k == DDP_K_DIRECT ? 0 : 1;
     auto key = std::make_pair(TD, G);
@@ -339,62 +329,103 @@ const DdpMergeTable& ddp_merge_table(const ddp_plan* p, ddp_kernel k, int TD, in
     DdpMergeTable& T = p->merge_tables[which][key];
     const std::vector<int32_t>& t = which == 0 ? p->delay : p->d1;
     int ni, nc;
-    merge_dims(p, k, TD, G, &ni, &nc);
-    T.vmax = ddp_merge_vmax(p, k, TD, G);
+    merge_dims(p, k, &ni, &nc);
     T.ntiles = (ni + TD - 1) / TD;
     T.ngg = nc / G;
-    const int64_t n = (int64_t)T.ntiles * T.ngg;
-    T.off_vdesc = round_up(n * 4, 16);
-    T.off_vid = T.off_vdesc + round_up(n * T.vmax * (2 + G) * 4, 16);
-    T.blob.assign((size_t)(T.off_vid + round_up(n * TD, 16)), 0);
-    int32_t* nvar = (int32_t*)T.blob.data();
-    int32_t* vdesc = (int32_t*)(T.blob.data() + T.off_vdesc);
-    unsigned char* vid = T.blob.data() + T.off_vid;
-    const int W = 2 + G;
+    T.vmax = DDP_MERGE_VMAX_LIMIT + 1;
+    const int nred = ddp_kgeom(p, k).nred;
+    if (nred % G != 0 || nc % G != 0 || TD > 4096) return T;  // groups never straddle a subband
+    std::vector<int32_t> nvar((size_t)T.ntiles * T.ngg);
+    std::vector<int32_t> tau((size_t)4 * DDP_MERGE_VMAX_LIMIT);
+    std::vector<unsigned char> vid(TD);
+    int vmax = 0;
     for (int ti = 0; ti < T.ntiles; ++ti) {
         const int lo = ti * TD, nd = std::min(TD, ni - lo);
         for (int gg = 0; gg < T.ngg; ++gg) {
-            const int r0 = gg * G;
-            const int32_t* d0 = &t[(size_t)lo * nc + r0];
-            int32_t* vd = vdesc + ((size_t)ti * T.ngg + gg) * T.vmax * W;
-            unsigned char* vi = vid + ((size_t)ti * T.ngg + gg) * TD;
-            int nv = 0;
-            for (int j = 0; j < TD; ++j) {
-                const int32_t* d = &t[(size_t)(lo + std::min(j, nd - 1)) * nc + r0];
-                const int delta = d[0] - d0[0];
-                int v = 0;
-                for (; v < nv; ++v) {
-                    bool same = true;
-                    for (int m = 1; m < G; ++m) same = same && vd[v * W + 2 + m] == (d[m] - d[0]) - (d0[m] - d0[0]);
-                    if (same) break;
-                }
-                if (v == nv) {
-                    vd[v * W] = delta;
-                    vd[v * W + 1] = delta;
-                    vd[v * W + 2] = 0;
-                    for (int m = 1; m < G; ++m) vd[v * W + 2 + m] = (d[m] - d[0]) - (d0[m] - d0[0]);
-                    ++nv;
-                } else {
-                    vd[v * W] = std::min(vd[v * W], delta);
-                    vd[v * W + 1] = std::max(vd[v * W + 1], delta);
-                }
-                vi[j] = (unsigned char)v;
-            }
+            const int nv = merge_scan_group(t.data(), nc, lo, nd, TD, gg * G, G, tau.data(), vid.data());
+            if (nv < 0) return T;
             nvar[(size_t)ti * T.ngg + gg] = nv;
+            vmax = std::max(vmax, nv);
         }
     }
+    T.nvar.swap(nvar);
+    T.vmax = vmax;
+    T.vcap = (vmax + 3) & ~3;
+    T.rw = (4 + 2 * G + T.vcap + TD + 3) & ~3;
     return T;
+}
+// The device image (record layout in ddp_internal.h), built when a launch needs it.
+const std::vector<unsigned char>& ddp_merge_table_blob(const ddp_plan* p, ddp_kernel k, int TD, int G) {
+    const DdpMergeTable& T = ddp_merge_table(p, k, TD, G);
+    if (!T.blob.empty() || T.vmax > DDP_MERGE_VMAX_LIMIT) return T.blob;
+    const std::vector<int32_t>& t = k == DDP_K_DIRECT ? p->delay : p->d1;
+    int ni, nc;
+    merge_dims(p, k, &ni, &nc);
+    T.blob.assign((size_t)T.ntiles * T.ngg * T.rw * 4, 0);
+    int32_t* rec = (int32_t*)T.blob.data();
+    std::vector<int32_t> tau((size_t)4 * DDP_MERGE_VMAX_LIMIT);
+    std::vector<unsigned char> vid(TD);
+    for (int ti = 0; ti < T.ntiles; ++ti) {
+        const int lo = ti * TD, nd = std::min(TD, ni - lo);
+        for (int gg = 0; gg < T.ngg; ++gg, rec += T.rw) {
+            const int r0 = gg * G;
+            const int nv = merge_scan_group(t.data(), nc, lo, nd, TD, r0, G, tau.data(), vid.data());
+            const int32_t* d0 = &t[(size_t)lo * nc + r0];
+            const int32_t* dl = &t[(size_t)(lo + nd - 1) * nc + r0];
+            rec[0] = nv;
+            rec[1] = dl[0] - d0[0];  // span: largest window offset of the group
+            for (int m = 0; m < G; ++m) {
+                rec[4 + m] = d0[m];
+                rec[4 + G + m] = dl[m];
+            }
+            for (int v = 0; v < nv; ++v) {
+                uint32_t code = 0;
+                for (int m = 1; m < G; ++m) code |= (uint32_t)(tau[(size_t)v * 4 + m] & 0xff) << (8 * (m - 1));
+                rec[4 + 2 * G + v] = (int32_t)code;
+            }
+            for (int j = 0; j < TD; ++j) {
+                const int32_t* d = &t[(size_t)(lo + std::min(j, nd - 1)) * nc + r0];
+                rec[4 + 2 * G + T.vcap + j] = (int32_t)(((uint32_t)vid[j] << 24) | (uint32_t)(d[0] - d0[0]));
+            }
+        }
+    }
+    return T.blob;
+}
+int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G) { return ddp_merge_table(p, k, TD, G).vmax; }
+int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G) {
+    const DdpMergeTable& T = ddp_merge_table(p, k, TD, G);
+    return (int64_t)T.ntiles * T.ngg * T.rw * 4;
+}
+// Variant rows a chunk of U reduction rows needs at most: chunks start at multiples of U inside a kernel group.
+int ddp_merge_rows_max(const ddp_plan* p, ddp_kernel k, int TD, int G, int U) {
+    const DdpMergeTable& T = ddp_merge_table(p, k, TD, G);
+    if (T.vmax > DDP_MERGE_VMAX_LIMIT) return 0;
+    auto it = T.rows_max.find(U);
+    if (it != T.rows_max.end()) return it->second;
+    const int NG = U / G;
+    int best = 0;
+    for (int ti = 0; ti < T.ntiles; ++ti)
+        for (int gg = 0; gg + NG <= T.ngg; gg += NG) {
+            int sum = 0;
+            for (int q = 0; q < NG; ++q) sum += T.nvar[(size_t)ti * T.ngg + gg + q];
+            best = std::max(best, sum);
+        }
+    T.rows_max[U] = best;
+    return best;
 }
 DdpMergeGeom ddp_merge_geom(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const int G = ddp_merge_group(c);
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int TD = c.threads_dm * c.dms_per_thread;
     const int spread = ddp_spread_max(p, k, TD);
+    const DdpMergeTable& T = ddp_merge_table(p, k, TD, G);
     DdpMergeGeom g;
-    g.vmax = ddp_merge_vmax(p, k, TD, G);
-    // both carry 32 words of slack: the variant rows are built in whole 32-word blocks
-    g.lw = (int)round_up(TT / 2 + spread + 4 + 32, 4);   // variant row: y < TT/2 + spread
-    g.le = (int)round_up(TT / 2 + spread + 20 + 32, 4);  // expanded row: z < 16 + spread + TT/2, whole uint4 stores
+    g.vmax = T.vmax;
+    g.vcap = T.vcap;
+    g.rw = T.rw;
+    g.rows_max = T.vmax > DDP_MERGE_VMAX_LIMIT ? 0 : ddp_merge_rows_max(p, k, TD, G, c.unroll);
+    g.lw = (int)round_up(TT / 2 + spread + 4, 4);        // variant row: y <= TT/2 + spread
+    g.le = (int)round_up(16 + TT / 2 + spread + 48, 4);  // expanded row: 16 words in front, 16-byte carry, shifts within +-15
     return g;
 }
 
@@ -419,20 +450,16 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             const DdpKGeom g = ddp_kgeom(p, k);
             const size_t row = (size_t)ddp_dedisp_win(p, k, c) * g.in_bytes;
             if (g.in_bytes == 1 && ddp_merge_group(c)) {  // ddp_dedisp_merge_body (same carve-up, same order)
-                const size_t G = (size_t)ddp_merge_group(c), U = (size_t)c.unroll, NG = U / G, NGS = 64 / G;
+                const size_t G = (size_t)ddp_merge_group(c), U = (size_t)c.unroll, NG = U / G;
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
                 const DdpMergeGeom mg = ddp_merge_geom(p, k, c);
-                size_t b = 2 * NG * mg.vmax * mg.lw * 4;              // pw
-                b += U * (size_t)mg.le * 4;                           // ebuf
-                b += 2 * TD * NGS * 4;                                // dbase
-                b += 2 * 2 * 64 * 4;                                  // dmm
-                b += ((2 * TD * NG + 3) & ~(size_t)3) * 4;            // offs
-                b += NG * mg.vmax * 8 * 4;                            // rowd
-                b += 2 * NGS * mg.vmax * (2 + G) * 4;                 // vdesc
-                b += 2 * NGS * 4;                                     // nvar
-                b += 2 * NGS * TD;                                    // vid
-                b = (b + 15) & ~(size_t)15;
-                b += 2 * U * (row + 16) + 16;                         // raw, mbar
+                if (mg.vmax > DDP_MERGE_VMAX_LIMIT) return (size_t)DDP_SMEM_LIMIT + 1;
+                size_t b = 2 * (size_t)mg.rows_max * mg.lw * 4;       // pw
+                b += 2 * U * (size_t)mg.le * 4;                       // ebuf
+                b += 2 * U * (row + 16);                              // raw
+                b += 2 * NG * (size_t)mg.rw * 4;                      // record staging
+                b += 8 * (((8 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
+                b += 4 * 8 + 16;                                      // mbarriers, scheduler cursor
                 return b;
             }
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
@@ -539,7 +566,7 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
     if (MG) {
         const int vm = ddp_merge_vmax(p, k, (int)TD, MG);
         if (vm > DDP_MERGE_VMAX_LIMIT) return no("V6: too many relative-shift variants per group for merged staging");
-        if (ddp_merge_table_bytes(p, k, (int)TD, MG, vm) > p->merge_capacity)
+        if (ddp_merge_table_bytes(p, k, (int)TD, MG) > p->merge_capacity)
             return no("V6: merged-staging table larger than its workspace region");
     }
     if (ddp_smem_bytes(p, k, c) > DDP_SMEM_LIMIT) return no("V6: shared memory over 227 KB");

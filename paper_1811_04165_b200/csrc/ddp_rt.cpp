@@ -726,31 +726,58 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
     }
     q.win = c.staging ? ddp_dedisp_win(p, k, c) : 0;
     q.one = 1;
+    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
+    const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     if (const int G = ddp_merge_group(c)) {
+        // merged staging: a persistent kernel over (tile, segment of <= 256 reduction rows) units
         const DdpMergeGeom mg = ddp_merge_geom(p, k, c);
-        q.vmax = mg.vmax;
+        q.vmax = mg.vcap;
         q.lw = mg.lw;
         q.le = mg.le;
+        q.rows_max = mg.rows_max;
+        q.meta_rw = mg.rw;
         // the (kernel, TD, G) table must be the resident one: upload it on the launch stream when it is not
-        const int TDm = c.threads_dm * c.dms_per_thread, which = k == DDP_K_DIRECT ? 0 : 1;
+        const int TDm = (int)TD, which = k == DDP_K_DIRECT ? 0 : 1;
         const DdpMergeTable& T = ddp_merge_table(p, k, TDm, G);
         ddp_plan* pm = const_cast<ddp_plan*>(p);
         if (p->merge_resident[0] != which || p->merge_resident[1] != TDm || p->merge_resident[2] != G) {
-            if ((int64_t)T.blob.size() > p->merge_capacity) return ddp_fail(p, DDP_E_WORKSPACE, "merged-staging table does not fit");
-            CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)p->d_merge, T.blob.data(), T.blob.size(), io.stream);
+            const std::vector<unsigned char>& blob = ddp_merge_table_blob(p, k, TDm, G);
+            if (blob.empty() || (int64_t)blob.size() > p->merge_capacity)
+                return ddp_fail(p, DDP_E_WORKSPACE, "merged-staging table does not fit");
+            CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)p->d_merge, blob.data(), blob.size(), io.stream);
             if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, "merged-staging table upload: " + cu_err(r));
             pm->merge_resident[0] = which;
             pm->merge_resident[1] = TDm;
             pm->merge_resident[2] = G;
         }
         q.meta = p->d_merge;
-        q.meta_vdesc_off = T.off_vdesc;
-        q.meta_vid_off = T.off_vid;
         q.meta_ngg = T.ngg;
         q.meta_gg0_stride = k == DDP_K_SUB1 ? p->cps / G : 0;
+        q.n_ttiles = (int)cdiv(q.ns, TT);
+        q.n_dtiles = (int)cdiv(q.ndm, TD);
+        const bool wide = q.nred > 257;  // code_flags bit 0
+        q.nseg = wide ? (q.nred + 255) / 256 : 1;
+        const int64_t nunits = (int64_t)groups * q.n_dtiles * q.n_ttiles * q.nseg;
+        if (nunits > 0x7fffffff) return ddp_fail(p, DDP_E_CONFIG, K->name + ": too many work units");
+        q.nunits = (int)nunits;
+        const size_t smem = ddp_smem_bytes(p, k, c);
+        const int threads = c.threads_t * c.threads_dm;
+        int per_sm = 0, nsm = 0;
+        CUdevice dev;
+        if (g_api.p_cuDeviceGet(&dev, p->device) != CUDA_SUCCESS ||
+            g_api.p_cuDeviceGetAttribute(&nsm, CU_DEVICE_ATTRIBUTE_MULTIPROCESSOR_COUNT, dev) != CUDA_SUCCESS ||
+            g_api.p_cuOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K->fn[p->device], threads, smem) != CUDA_SUCCESS ||
+            per_sm < 1 || nsm < 1)
+            return ddp_fail(p, DDP_E_CUDA, K->name + ": occupancy query failed");
+        if (wide) {  // the segments of a tile add into the output with RED.ADD: it starts from zero
+            const size_t words = k == DDP_K_DIRECT ? (size_t)p->ndm * io.out_stride
+                                                   : (size_t)p->ncoarse * p->nsub * (size_t)I.sub_stride;
+            CUresult r = g_api.p_cuMemsetD32Async((CUdeviceptr)q.out, 0u, words, io.stream);
+            if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, "zeroing the output: " + cu_err(r));
+        }
+        const int64_t grid = std::min<int64_t>(nunits, (int64_t)per_sm * nsm);
+        return launch(p, K, (unsigned)grid, 1, 1, (unsigned)c.threads_t, (unsigned)c.threads_dm, smem, io.stream, &q);
     }
-    const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
-    const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     return launch(p, K, cdiv(q.ns, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,
                   ddp_smem_bytes(p, k, c), io.stream, &q);
 }
