@@ -713,10 +713,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     unsigned char* raw = (unsigned char*)(ebuf + (size_t)2 * U * le);        // [2][U][win + 16]
     int* stg = (int*)(raw + (size_t)2 * U * (win + 16));                     // [2][NG * RW] host-table records
     int* ring = stg + (size_t)2 * NG * RW;                                   // [DEPTH][SLOTW]
-    const int SLOTW = (8 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
+    const int SLOTW = (16 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
     ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2]
     int* sched = (int*)(mbar + 4);                                           // scheduler cursor {unit, chunk}
-    // ring slot: desc[8] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax} | a0[U] | bytes[U] | carry[U] | nz4[U] |
+    // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, ...} | a0[U] | bytes[U] | carry[U] | nz4[U] |
     //            rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
     auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
 
@@ -749,6 +749,12 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
 #pragma unroll
         for (int k = 0; k < K; ++k) acc[j][k] = 0u;
     const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
+    // descriptor roles: TMA extents on warp 0, variant rows from warp 1 on, window offsets from warp 4 on (blocks
+    // that small start all of them at thread 0); whole warps without a role skip the stage
+    const int offB = nthreads >= 64 ? 32 : 0, offC = nthreads >= 256 ? 128 : 0;
+    const int rB = tid - offB, sB = nthreads - offB, rC = tid - offC, sC = nthreads - offC;
+    const bool m2_role = warp == 0 || (rB >= 0 && (rB & ~31) < NG * VCAP) || (rC >= 0 && (rC & ~31) < TD * NG);
+    constexpr int LGU = U == 16 ? 4 : U == 8 ? 3 : U == 4 ? 2 : 1;
 
     for (int n = -5; n < nstream; ++n) {
         // ---- schedule chunk n + 5 (one thread)
@@ -778,37 +784,46 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             }
         }
         // ---- descriptors of chunk n + 4 from its records
-        {
+        if (m2_role) {  // warp-uniform
             const int x = n + 4;
             int* d = slot(x);
             if (x >= 0 && x < nstream) {
                 const int* rec = stg + (size_t)(x & 1) * NG * RW;
                 ddp_mbar_wait(&mbar[2 + (x & 1)], (ddp_u32)((x >> 1) & 1));
                 const int tile_t = d[0];
-                int* a0s = d + 8;
+                int* a0s = d + 16;
                 int* byts = a0s + U;
                 int* carr = byts + U;
                 int* nz4s = carr + U;
                 int* rowd = nz4s + U;
                 ddp_u32* offs = (ddp_u32*)(rowd + 8 * rows_max);
-                if (tid < U) {  // TMA extent and expansion length of reduction row tid of the chunk
-                    const int* r = rec + (tid / G) * RW;
-                    const int dmin = r[4 + tid % G], dmax = r[4 + G + tid % G];
-                    const long long src = (long long)tile_t + dmin;
-                    const long long a0 = src & ~15ll;
-                    const int carry = (int)(src - a0);
-                    int need = ((carry + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
-                    need = (need + 3) & ~3;
-                    if (need > (win >> 2)) need = win >> 2;
-                    long long l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
-                    const int lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
-                    a0s[tid] = (int)a0;
-                    byts[tid] = lenw > 0 ? lenw * 4 + 16 : 0;
-                    carr[tid] = carry;
-                    nz4s[tid] = (carry + (dmax - dmin) + H + 3) >> 2;
+                if (warp == 0) {  // TMA extent and expansion length of reduction row `lane` of the chunk
+                    int nz4 = 0;
+                    if (lane < U) {
+                        const int* r = rec + (lane / G) * RW;
+                        const int dmin = r[4 + lane % G], dmax = r[4 + G + lane % G];
+                        const long long src = (long long)tile_t + dmin;
+                        const long long a0 = src & ~15ll;
+                        const int carry = (int)(src - a0);
+                        int need = ((carry + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
+                        need = (need + 3) & ~3;
+                        if (need > (win >> 2)) need = win >> 2;
+                        long long l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
+                        const int lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
+                        nz4 = (carry + (dmax - dmin) + H + 3) >> 2;
+                        a0s[lane] = (int)a0;
+                        byts[lane] = lenw > 0 ? lenw * 4 + 16 : 0;
+                        carr[lane] = carry;
+                        nz4s[lane] = nz4;
+                    }
+#pragma unroll
+                    for (int s = 16; s >= 1; s >>= 1) {
+                        const int o = __shfl_xor_sync(0xffffffffu, nz4, s);
+                        nz4 = o > nz4 ? o : nz4;
+                    }
+                    if (lane == 0) d[8] = nz4;
                 }
-                const int t1 = (tid + nthreads - 32 % nthreads) % nthreads;  // start at warp 1
-                for (int i = t1; i < NG * VCAP; i += nthreads) {
+                for (int i = rB; i >= 0 && i < NG * VCAP; i += sB) {
                     const int q = i / VCAP, v = i - q * VCAP;
                     const int* r = rec + q * RW;
                     int base = 0, total = 0, ymax = 0;
@@ -834,8 +849,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                         }
                     }
                 }
-                const int t4 = (tid + nthreads - 128 % nthreads) % nthreads;  // start at warp 4
-                for (int i = t4; i < TD * NG; i += nthreads) {
+                for (int i = rC; i >= 0 && i < TD * NG; i += sC) {
                     const int j = i / NG, q = i - j * NG;
                     int base = 0;
 #pragma unroll
@@ -852,7 +866,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             const int* d = slot(x);
             if (x >= 0 && x < nstream) {
                 const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)d[3] * p.in_group_stride;
-                const ddp_u32 bytes = lane < U ? (ddp_u32)d[8 + U + lane] : 0u;
+                const ddp_u32 bytes = lane < U ? (ddp_u32)d[16 + U + lane] : 0u;
                 ddp_u32 total = bytes;
 #pragma unroll
                 for (int s = 16; s >= 1; s >>= 1) total += __shfl_xor_sync(0xffffffffu, total, s);
@@ -860,32 +874,38 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 __syncwarp();
                 if (bytes)
                     ddp_bulk_g2s(raw + ((size_t)(x & 1) * U + lane) * (win + 16),
-                                 in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[8 + lane], bytes, &mbar[x & 1]);
+                                 in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[16 + lane], bytes, &mbar[x & 1]);
             }
         }
-        // ---- expand chunk n + 2: raw slot -> E rows (samples (z, z + H) of each channel as 2 x 16-bit lanes)
+        // ---- expand chunk n + 2: raw slot -> E rows (samples (z, z + H) of each channel as 2 x 16-bit lanes);
+        //      item = (row, block of 64 four-sample groups), two groups per lane
         {
             const int x = n + 2;
             const int* d = slot(x);
             if (x >= 0 && x < nstream) {
                 ddp_mbar_wait(&mbar[x & 1], (ddp_u32)((x >> 1) & 1));
-                const int* nz4s = d + 8 + 3 * U;
-                int nzmax = 0;
+                const int* nz4s = d + 16 + 3 * U;
+                const int nblk = (d[8] + 63) >> 6, hq = H >> 2;
+                const unsigned char* rbase = raw + (size_t)(x & 1) * U * (win + 16);
+                ddp_u32* ebase = ebuf + (size_t)(x & 1) * U * le + DDP_MRG_EPAD;
+                for (int it = (warp + x) & (nwarps - 1); it < (nblk << LGU); it += nwarps) {  // nwarps is a power of two
+                    const int u = it & (U - 1), q4 = ((it >> LGU) << 6) + lane;
+                    const int nz = nz4s[u];
+                    const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
+                    ddp_u32* dst = ebase + (size_t)u * le;
+                    ddp_u32 lo[2], hi[2];
 #pragma unroll
-                for (int u = 0; u < U; ++u) nzmax = nz4s[u] > nzmax ? nz4s[u] : nzmax;
-                const int nblk = (nzmax + 31) >> 5, hq = H >> 2;
-                const int wrot = (warp + x) % nwarps;  // rotate the hand-out so that no warp is always the loaded one
-                for (int it = wrot; it < U * nblk; it += nwarps) {
-                    const int u = it / nblk, q4 = ((it - u * nblk) << 5) + lane;
-                    if (q4 < nz4s[u]) {
-                        const ddp_u32* src = (const ddp_u32*)(raw + ((size_t)(x & 1) * U + u) * (win + 16));
-                        ddp_u32* dst = ebuf + ((size_t)(x & 1) * U + u) * le + DDP_MRG_EPAD;
-                        const ddp_u32 lo = src[q4], hi = src[q4 + hq];
-                        const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
-                        const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
-                        *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
-                                                             __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
-                    }
+                    for (int i = 0; i < 2; ++i)
+                        if (q4 + 32 * i < nz) { lo[i] = src[q4 + 32 * i]; hi[i] = src[q4 + 32 * i + hq]; }
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+                        if (q4 + 32 * i < nz) {
+                            const ddp_u32 elo = lo[i] & 0x00ff00ffu, ehi = hi[i] & 0x00ff00ffu;
+                            const ddp_u32 olo = __byte_perm(lo[i], 0u, 0x4341u), ohi = __byte_perm(hi[i], 0u, 0x4341u);
+                            *(uint4*)(dst + 4 * (q4 + 32 * i)) =
+                                make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
+                                           __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                        }
                 }
             }
         }
@@ -895,21 +915,22 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             const int* d = slot(x);
             if (x >= 0 && x < nstream) {
                 const int R = d[6], nblk = (d[7] + 127) >> 7;
-                const int* rowd = d + 8 + 4 * U;
-                const ddp_u32* eb = ebuf + (size_t)(x & 1) * U * le;
-                ddp_u32* pb = pw + (size_t)(x & 1) * rows_max * lw;
-                const int wrot = (warp + 5 * x) % nwarps;
-                for (int it = wrot; it < R * nblk; it += nwarps) {
-                    const int row = it / nblk, y0 = ((it - row * nblk) << 7) + lane;
+                const int lgb = nblk > 1 ? 32 - __clz(nblk - 1) : 0;  // blocks per row rounded up to a power of two
+                const int* rowd = d + 16 + 4 * U;
+                const ddp_u32* eb = ebuf + (size_t)(x & 1) * U * le + lane;
+                ddp_u32* pb = pw + (size_t)(x & 1) * rows_max * lw + lane;
+                for (int it = (warp + 5 * x) & (nwarps - 1); it < (R << lgb); it += nwarps) {
+                    const int row = it >> lgb, y0 = (it & ((1 << lgb) - 1)) << 7;
                     const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                    const int ylen = d0.x - lane;  // words of this lane's column left in the row
+                    if (y0 >= d0.x) continue;      // warp-uniform
                     const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-                    const int ylen = d0.x;
                     const ddp_u32* e0 = eb + d0.z + y0;
                     const ddp_u32* e1 = eb + d0.w + y0;
                     const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0) + y0;
                     const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0) + y0;
                     ddp_u32* dst = pb + d0.y + y0;
-                    if (y0 + 96 < ylen) {  // whole item: all loads first
+                    if (y0 + 128 <= d0.x) {  // whole item (warp-uniform): all loads first
                         ddp_u32 s[4];
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
@@ -934,7 +955,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
         // ---- sum chunk n: every trial adds its variant rows, then (last chunk of a unit) flush
         if (n >= 0) {
             const int* d = slot(n);
-            const ddp_u32* ob = (const ddp_u32*)(d + 8 + 4 * U + 8 * rows_max) + (size_t)(ty * DPT) * NG;
+            const ddp_u32* ob = (const ddp_u32*)(d + 16 + 4 * U + 8 * rows_max) + (size_t)(ty * DPT) * NG;
             const unsigned char* lanep = (const unsigned char*)(pw + (size_t)(n & 1) * rows_max * lw + wb);
 #pragma unroll
             for (int j = 0; j < DPT; ++j) {

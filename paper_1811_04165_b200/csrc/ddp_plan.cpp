@@ -458,7 +458,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += 2 * U * (size_t)mg.le * 4;                       // ebuf
                 b += 2 * U * (row + 16);                              // raw
                 b += 2 * NG * (size_t)mg.rw * 4;                      // record staging
-                b += 8 * (((8 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
+                b += 8 * (((16 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
                 b += 4 * 8 + 16;                                      // mbarriers, scheduler cursor
                 return b;
             }
