@@ -715,7 +715,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     int* ring = stg + (size_t)2 * NG * RW;                                   // [DEPTH][SLOTW]
     const int SLOTW = (16 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
     ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2]
-    int* sched = (int*)(mbar + 4);                                           // scheduler cursor {unit, chunk}
+    int* sched = (int*)(mbar + 4);                                           // scheduler cursor {unit, chunk}, item counters [2]
     // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, ...} | a0[U] | bytes[U] | carry[U] | nz4[U] |
     //            rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
     auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
@@ -739,6 +739,8 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
         ddp_mbar_fence_init();
         sched[0] = unit_lo;
         sched[1] = 0;
+        sched[2] = 0;  // item counters of odd / even iterations
+        sched[3] = 0;
     }
     for (int i = tid; i < DDP_MRG_DEPTH; i += nthreads) slot(i)[5] = 0;  // nothing valid yet
     __syncthreads();
@@ -759,6 +761,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     for (int n = -5; n < nstream; ++n) {
         // ---- schedule chunk n + 5 (one thread)
         if (tid == 0) {
+            sched[2 + ((n + 1) & 1)] = 0;  // item counter of the next iteration (last used in the previous one)
             const int x = n + 5;
             int* d = slot(x);
             const int unit = sched[0], c = sched[1];
@@ -835,7 +838,13 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                         const int yl = H + rec[qq * RW + 1] + 1;
                         ymax = yl > ymax ? yl : ymax;
                     }
-                    if (i == 0) { d[6] = total; d[7] = ymax; }
+                    if (i == 0) {
+                        const int nb = (ymax + 127) >> 7;  // 128-word blocks per variant row
+                        d[6] = total;
+                        d[7] = ymax;
+                        d[9] = nb;
+                        d[10] = ((1 << 20) + nb - 1) / nb;  // item -> row by a multiplication (items < 2^20 / nb)
+                    }
                     if (v < r[0]) {
                         const int code = r[4 + 2 * G + v];
                         int* o = rowd + (size_t)(base + v) * 8;
@@ -875,81 +884,6 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 if (bytes)
                     ddp_bulk_g2s(raw + ((size_t)(x & 1) * U + lane) * (win + 16),
                                  in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[16 + lane], bytes, &mbar[x & 1]);
-            }
-        }
-        // ---- expand chunk n + 2: raw slot -> E rows (samples (z, z + H) of each channel as 2 x 16-bit lanes);
-        //      item = (row, block of 64 four-sample groups), two groups per lane
-        {
-            const int x = n + 2;
-            const int* d = slot(x);
-            if (x >= 0 && x < nstream) {
-                ddp_mbar_wait(&mbar[x & 1], (ddp_u32)((x >> 1) & 1));
-                const int* nz4s = d + 16 + 3 * U;
-                const int nblk = (d[8] + 63) >> 6, hq = H >> 2;
-                const unsigned char* rbase = raw + (size_t)(x & 1) * U * (win + 16);
-                ddp_u32* ebase = ebuf + (size_t)(x & 1) * U * le + DDP_MRG_EPAD;
-                for (int it = (warp + x) & (nwarps - 1); it < (nblk << LGU); it += nwarps) {  // nwarps is a power of two
-                    const int u = it & (U - 1), q4 = ((it >> LGU) << 6) + lane;
-                    const int nz = nz4s[u];
-                    const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
-                    ddp_u32* dst = ebase + (size_t)u * le;
-                    ddp_u32 lo[2], hi[2];
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if (q4 + 32 * i < nz) { lo[i] = src[q4 + 32 * i]; hi[i] = src[q4 + 32 * i + hq]; }
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if (q4 + 32 * i < nz) {
-                            const ddp_u32 elo = lo[i] & 0x00ff00ffu, ehi = hi[i] & 0x00ff00ffu;
-                            const ddp_u32 olo = __byte_perm(lo[i], 0u, 0x4341u), ohi = __byte_perm(hi[i], 0u, 0x4341u);
-                            *(uint4*)(dst + 4 * (q4 + 32 * i)) =
-                                make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
-                                           __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
-                        }
-                }
-            }
-        }
-        // ---- build chunk n + 1: E rows -> variant rows of buffer (n + 1) & 1, 128 words per (row, block) item
-        {
-            const int x = n + 1;
-            const int* d = slot(x);
-            if (x >= 0 && x < nstream) {
-                const int R = d[6], nblk = (d[7] + 127) >> 7;
-                const int lgb = nblk > 1 ? 32 - __clz(nblk - 1) : 0;  // blocks per row rounded up to a power of two
-                const int* rowd = d + 16 + 4 * U;
-                const ddp_u32* eb = ebuf + (size_t)(x & 1) * U * le + lane;
-                ddp_u32* pb = pw + (size_t)(x & 1) * rows_max * lw + lane;
-                for (int it = (warp + 5 * x) & (nwarps - 1); it < (R << lgb); it += nwarps) {
-                    const int row = it >> lgb, y0 = (it & ((1 << lgb) - 1)) << 7;
-                    const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
-                    const int ylen = d0.x - lane;  // words of this lane's column left in the row
-                    if (y0 >= d0.x) continue;      // warp-uniform
-                    const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-                    const ddp_u32* e0 = eb + d0.z + y0;
-                    const ddp_u32* e1 = eb + d0.w + y0;
-                    const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0) + y0;
-                    const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0) + y0;
-                    ddp_u32* dst = pb + d0.y + y0;
-                    if (y0 + 128 <= d0.x) {  // whole item (warp-uniform): all loads first
-                        ddp_u32 s[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            s[i] = e0[32 * i] + e1[32 * i];
-                            if constexpr (G > 2) s[i] += e2[32 * i] + e3[32 * i];
-                        }
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) dst[32 * i] = s[i];
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            if (y0 + 32 * i < ylen) {
-                                ddp_u32 s0 = e0[32 * i] + e1[32 * i];
-                                if constexpr (G > 2) s0 += e2[32 * i] + e3[32 * i];
-                                dst[32 * i] = s0;
-                            }
-                        }
-                    }
-                }
             }
         }
         // ---- sum chunk n: every trial adds its variant rows, then (last chunk of a unit) flush
@@ -1005,6 +939,87 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                     }
 #pragma unroll
                     for (int k = 0; k < K; ++k) acc[j][k] = 0u;
+                }
+            }
+        }
+        // ---- build chunk n + 1 and expand chunk n + 2: items handed out by a shared counter, so that the warps that
+        //      carried a descriptor role or a flush in this iteration take fewer and all reach the barrier together
+        {
+            const int xb = n + 1, xs = n + 2;
+            const int* db = slot(xb);
+            const int* ds = slot(xs);
+            const bool vb = xb >= 0 && xb < nstream, vs = xs >= 0 && xs < nstream;
+            const int R = vb ? db[6] : 0, nblk = vb ? db[9] : 1, rcp = vb ? db[10] : 0;
+            const int NB = R * nblk;                                  // build items: (variant row, 128 words)
+            const int nblks = vs ? (ds[8] + 63) >> 6 : 0;             // expand items: (channel, 64 four-sample groups)
+            const int NI = NB + (nblks << LGU);
+            const int* rowd = db + 16 + 4 * U;
+            const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
+            ddp_u32* pb = pw + (size_t)(xb & 1) * rows_max * lw + lane;
+            const int* nz4s = ds + 16 + 3 * U;
+            const int hq = H >> 2;
+            const unsigned char* rbase = raw + (size_t)(xs & 1) * U * (win + 16);
+            ddp_u32* ebase = ebuf + (size_t)(xs & 1) * U * le + DDP_MRG_EPAD;
+            bool raw_ready = false;
+            int* cnt = sched + 2 + (n & 1);
+            for (;;) {
+                int it = 0;
+                if (lane == 0) it = atomicAdd(cnt, 1);
+                it = __shfl_sync(0xffffffffu, it, 0);
+                if (it >= NI) break;
+                if (it < NB) {
+                    const int row = (int)(((ddp_u32)it * (ddp_u32)rcp) >> 20), y0 = (it - row * nblk) << 7;
+                    const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                    const int ylen = d0.x - lane;  // words of this lane's column left in the row
+                    if (y0 >= d0.x) continue;      // warp-uniform
+                    const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
+                    const ddp_u32* e0 = eb + d0.z + y0;
+                    const ddp_u32* e1 = eb + d0.w + y0;
+                    const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0) + y0;
+                    const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0) + y0;
+                    ddp_u32* dst = pb + d0.y + y0;
+                    if (y0 + 128 <= d0.x) {  // whole item (warp-uniform): all loads first
+                        ddp_u32 sm[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            sm[i] = e0[32 * i] + e1[32 * i];
+                            if constexpr (G > 2) sm[i] += e2[32 * i] + e3[32 * i];
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) dst[32 * i] = sm[i];
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (y0 + 32 * i < ylen) {
+                                ddp_u32 s0 = e0[32 * i] + e1[32 * i];
+                                if constexpr (G > 2) s0 += e2[32 * i] + e3[32 * i];
+                                dst[32 * i] = s0;
+                            }
+                        }
+                    }
+                } else {
+                    if (!raw_ready) {
+                        ddp_mbar_wait(&mbar[xs & 1], (ddp_u32)((xs >> 1) & 1));
+                        raw_ready = true;
+                    }
+                    const int is = it - NB;
+                    const int u = is & (U - 1), q4 = ((is >> LGU) << 6) + lane;
+                    const int nz = nz4s[u];
+                    const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
+                    ddp_u32* dst = ebase + (size_t)u * le;
+                    ddp_u32 lo[2], hi[2];
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+                        if (q4 + 32 * i < nz) { lo[i] = src[q4 + 32 * i]; hi[i] = src[q4 + 32 * i + hq]; }
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+                        if (q4 + 32 * i < nz) {
+                            const ddp_u32 elo = lo[i] & 0x00ff00ffu, ehi = hi[i] & 0x00ff00ffu;
+                            const ddp_u32 olo = __byte_perm(lo[i], 0u, 0x4341u), ohi = __byte_perm(hi[i], 0u, 0x4341u);
+                            *(uint4*)(dst + 4 * (q4 + 32 * i)) =
+                                make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
+                                           __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                        }
                 }
             }
         }
