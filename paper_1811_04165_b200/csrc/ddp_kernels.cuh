@@ -675,24 +675,33 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
 // window starts at ANY word whatever the delay (no byte- or element-shifted copies), and a thread's K
 // words are words {32K*(tx/32) + tx%32 + 32k}: every LDS.32 of a warp is conflict free.
 //
-// Schedule.  The kernel is PERSISTENT: the grid is one block per SM (or as many as fit) and every block
-// walks a contiguous range of work units (tile, segment of <= 256 reduction rows) as ONE stream of chunks
-// of U rows, software-pipelined over the chunks with a single __syncthreads per chunk -- the pipeline never
-// drains between units.  In iteration n the block
-//     schedules chunk n+5 (one thread: unit/tile arithmetic, bulk copy of the chunk's host-table records),
-//     turns the records of chunk n+4 into shared-memory descriptors (TMA extents, row and window offsets),
-//     issues the TMA bulk copies of the raw windows of chunk n+3,
-//     expands chunk n+2:  raw bytes -> E rows  (samples (z, z + H) of each channel as 2 x 16-bit lanes),
-//     builds   chunk n+1:  E rows -> variant rows PW_v,
-//     sums     chunk n:    every trial adds its variant row at its offset into packed 16-bit accumulators,
-// and at the last chunk of a unit flushes the accumulators: plain stores when the reduction is one segment
-// (subband step 1), RED.ADD into the zeroed output otherwise (256 rows * 255 = 65280 fits the lanes).
+// Schedule.  The kernel is PERSISTENT and WARP SPECIALISED.  The grid is one block per SM (or as many as fit)
+// and every block walks a contiguous range of work units (tile, segment of <= 256 reduction rows) as ONE stream
+// of chunks of U rows; the pipeline never drains between units.  The block is threads_t x threads_dm CONSUMER
+// threads, which own the tile's packed 16-bit accumulators and do nothing but add variant rows (and flush at the
+// end of a unit), plus 4 or 8 PRODUCER warps, which in their iteration n
+//     schedule chunk n+5 (one thread: unit/tile arithmetic, bulk copy of the chunk's host-table records),
+//     turn the records of chunk n+4 into shared-memory descriptors (TMA extents, row and window offsets),
+//     issue the TMA bulk copies of the raw windows of chunk n+3,
+//     expand chunk n+2:  raw bytes -> E rows  (samples (z, z + H) of each channel as 2 x 16-bit lanes),
+//     build  chunk n+1:  E rows -> variant rows PW_v,
+// with one named barrier per iteration among themselves.  Producers and consumers meet only at two pairs of
+// mbarriers (variant-row buffer full / empty), so neither side waits for the other's slowest warp, and with
+// setmaxnreg the consumers take the registers the producers do not need.  A unit's accumulators are flushed
+// with plain stores when the reduction is one segment (subband step 1), with RED.ADD into the zeroed output
+// otherwise (256 rows * 255 = 65280 fits the lanes).
 // Which variant a trial uses, every variant's shifts and the tile's first / last delays depend on the delay
 // table, TD and G only: the host tabulates them once per plan (DdpMergeTable, ddp_plan.cpp), one record per
 // (DM tile, group), so the kernel never reads the delay table.
-#define DDP_MRG_DEPTH 8   // descriptor ring slots (a chunk's descriptors live for 5 iterations)
+#define DDP_MRG_DEPTH 8   // descriptor ring slots (a chunk's descriptors live for 5 producer iterations + the consumers' lag)
 #define DDP_MRG_EPAD 16   // words in front of every E row (variant shifts may be negative)
-template <int SPT, int DPT, int U, int G, bool WIDE, bool OUT16>
+__device__ __forceinline__ void ddp_mbar_arrive(void* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ddp_smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void ddp_named_barrier(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+template <int SPT, int DPT, int U, int G, bool WIDE, bool OUT16, bool REGSPLIT>
 __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) {
     static_assert(SPT >= 2 && U % G == 0 && (G == 2 || G == 4), "merged staging works on 2-sample words and whole groups");
     static_assert(!(WIDE && OUT16), "a uint16 result never needs more than one segment");
@@ -700,11 +709,11 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     constexpr int K = SPT / 2;   // words per thread
     constexpr int NG = U / G;    // groups per chunk
     constexpr int FL = 256;      // reduction rows per segment (16-bit lanes: 256 * 255 < 65536)
-    const int tx = threadIdx.x, ty = threadIdx.y;
-    const int nthreads = blockDim.x * blockDim.y;
-    const int tid = ty * blockDim.x + tx;
-    const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
-    const int TT = blockDim.x * SPT, TD = blockDim.y * DPT, H = TT >> 1;
+    constexpr int LGU = U == 16 ? 4 : U == 8 ? 3 : U == 4 ? 2 : 1;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int NCT = p.threads_t * p.threads_dm, NCW = NCT >> 5;       // consumer threads / warps
+    const int NPW = ((int)blockDim.x >> 5) - NCW, NPT = NPW << 5;     // producer warps (4 or 8) / threads
+    const int TT = p.threads_t * SPT, TD = p.threads_dm * DPT, H = TT >> 1;
     const int win = p.win, lw = p.lw, le = p.le, RW = p.meta_rw, VCAP = p.vmax, rows_max = p.rows_max;
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it); every region starts 16-byte aligned
@@ -714,10 +723,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     int* stg = (int*)(raw + (size_t)2 * U * (win + 16));                     // [2][NG * RW] host-table records
     int* ring = stg + (size_t)2 * NG * RW;                                   // [DEPTH][SLOTW]
     const int SLOTW = (16 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
-    ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2]
-    int* sched = (int*)(mbar + 4);                                           // scheduler cursor {unit, chunk}, item counters [2]
-    // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, ...} | a0[U] | bytes[U] | carry[U] | nz4[U] |
-    //            rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
+    ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2], pw full[2], pw empty[2]
+    int* sched = (int*)(mbar + 8);                                           // scheduler cursor [8]
+    // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, nblk, 2^20/nblk, ...} | a0[U] | bytes[U] |
+    //            carry[U] | nz4[U] | rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
     auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
 
     // this block's units: a contiguous range, tile-major / segment-minor, so that the segments of a tile
@@ -726,8 +735,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     const long long nun = p.nunits;
     const int unit_lo = (int)((long long)blockIdx.x * nun / gridDim.x);
     const int unit_hi = (int)((long long)(blockIdx.x + 1) * nun / gridDim.x);
-    // chunks of this block's stream (every thread needs the trip count)
-    int nstream = 0;
+    int nstream = 0;  // chunks of this block's stream
     {
         const int full = FL / U, last = (p.nred - (nseg - 1) * FL) / U;
         for (int u = unit_lo; u < unit_hi; ++u) nstream += (u % nseg == nseg - 1) ? last : full;
@@ -736,159 +744,258 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < 4; ++b) ddp_mbar_init(&mbar[b], 1);
+        ddp_mbar_init(&mbar[4], NPW);
+        ddp_mbar_init(&mbar[5], NPW);
+        ddp_mbar_init(&mbar[6], NCW);
+        ddp_mbar_init(&mbar[7], NCW);
         ddp_mbar_fence_init();
+        const int tile = unit_lo / nseg, rest = tile / p.n_ttiles;
         sched[0] = unit_lo;
         sched[1] = 0;
-        sched[2] = 0;  // item counters of odd / even iterations
-        sched[3] = 0;
+        sched[2] = unit_lo - tile * nseg;
+        sched[3] = tile % p.n_ttiles;
+        sched[4] = rest % p.n_dtiles;
+        sched[5] = rest / p.n_dtiles;
     }
-    for (int i = tid; i < DDP_MRG_DEPTH; i += nthreads) slot(i)[5] = 0;  // nothing valid yet
+    for (int i = tid; i < DDP_MRG_DEPTH; i += blockDim.x) slot(i)[5] = 0;  // nothing valid yet
     __syncthreads();
 
-    ddp_u32 acc[DPT][K];
-#pragma unroll
-    for (int j = 0; j < DPT; ++j)
-#pragma unroll
-        for (int k = 0; k < K; ++k) acc[j][k] = 0u;
-    const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
-    // descriptor roles: TMA extents on warp 0, variant rows from warp 1 on, window offsets from warp 4 on (blocks
-    // that small start all of them at thread 0); whole warps without a role skip the stage
-    const int offB = nthreads >= 64 ? 32 : 0, offC = nthreads >= 256 ? 128 : 0;
-    const int rB = tid - offB, sB = nthreads - offB, rC = tid - offC, sC = nthreads - offC;
-    const bool m2_role = warp == 0 || (rB >= 0 && (rB & ~31) < NG * VCAP) || (rC >= 0 && (rC & ~31) < TD * NG);
-    constexpr int LGU = U == 16 ? 4 : U == 8 ? 3 : U == 4 ? 2 : 1;
-
-    for (int n = -5; n < nstream; ++n) {
-        // ---- schedule chunk n + 5 (one thread)
-        if (tid == 0) {
-            sched[2 + ((n + 1) & 1)] = 0;  // item counter of the next iteration (last used in the previous one)
-            const int x = n + 5;
-            int* d = slot(x);
-            const int unit = sched[0], c = sched[1];
-            if (x < nstream && unit < unit_hi) {
-                const int tile = unit / nseg, seg = unit - tile * nseg;
-                const int tt = tile % p.n_ttiles, rest = tile / p.n_ttiles;
-                const int dt = rest % p.n_dtiles, g = rest / p.n_dtiles;
-                const int rows = p.nred - seg * FL < FL ? p.nred - seg * FL : FL;
-                const int nch = WIDE ? rows / U : p.nred / U;
-                const int r0 = seg * FL + c * U;
-                d[0] = tt * TT;
-                d[1] = dt * TD;
-                d[2] = (dt + 1) * TD <= p.ndm ? TD : p.ndm - dt * TD;
-                d[3] = g;
-                d[4] = r0;
-                d[5] = 1 | (c == 0 ? 2 : 0) | (c == nch - 1 ? 4 : 0);
-                const long long rec = ((long long)dt * p.meta_ngg + (long long)g * p.meta_gg0_stride + r0 / G) * RW;
-                ddp_mbar_expect_tx(&mbar[2 + (x & 1)], (ddp_u32)(NG * RW * 4));
-                ddp_bulk_g2s(stg + (size_t)(x & 1) * NG * RW, (const int*)p.meta + rec, (ddp_u32)(NG * RW * 4), &mbar[2 + (x & 1)]);
-                if (c + 1 == nch) { sched[0] = unit + 1; sched[1] = 0; } else { sched[1] = c + 1; }
-            } else {
-                d[5] = 0;
-            }
-        }
-        // ---- descriptors of chunk n + 4 from its records
-        if (m2_role) {  // warp-uniform
-            const int x = n + 4;
-            int* d = slot(x);
-            if (x >= 0 && x < nstream) {
-                const int* rec = stg + (size_t)(x & 1) * NG * RW;
-                ddp_mbar_wait(&mbar[2 + (x & 1)], (ddp_u32)((x >> 1) & 1));
-                const int tile_t = d[0];
-                int* a0s = d + 16;
-                int* byts = a0s + U;
-                int* carr = byts + U;
-                int* nz4s = carr + U;
-                int* rowd = nz4s + U;
-                ddp_u32* offs = (ddp_u32*)(rowd + 8 * rows_max);
-                if (warp == 0) {  // TMA extent and expansion length of reduction row `lane` of the chunk
-                    int nz4 = 0;
-                    if (lane < U) {
-                        const int* r = rec + (lane / G) * RW;
-                        const int dmin = r[4 + lane % G], dmax = r[4 + G + lane % G];
-                        const long long src = (long long)tile_t + dmin;
-                        const long long a0 = src & ~15ll;
-                        const int carry = (int)(src - a0);
-                        int need = ((carry + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
-                        need = (need + 3) & ~3;
-                        if (need > (win >> 2)) need = win >> 2;
-                        long long l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
-                        const int lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
-                        nz4 = (carry + (dmax - dmin) + H + 3) >> 2;
-                        a0s[lane] = (int)a0;
-                        byts[lane] = lenw > 0 ? lenw * 4 + 16 : 0;
-                        carr[lane] = carry;
-                        nz4s[lane] = nz4;
-                    }
-#pragma unroll
-                    for (int s = 16; s >= 1; s >>= 1) {
-                        const int o = __shfl_xor_sync(0xffffffffu, nz4, s);
-                        nz4 = o > nz4 ? o : nz4;
-                    }
-                    if (lane == 0) d[8] = nz4;
-                }
-                for (int i = rB; i >= 0 && i < NG * VCAP; i += sB) {
-                    const int q = i / VCAP, v = i - q * VCAP;
-                    const int* r = rec + q * RW;
-                    int base = 0, total = 0, ymax = 0;
-#pragma unroll
-                    for (int qq = 0; qq < NG; ++qq) {
-                        const int nv = rec[qq * RW];
-                        if (qq < q) base += nv;
-                        total += nv;
-                        const int yl = H + rec[qq * RW + 1] + 1;
-                        ymax = yl > ymax ? yl : ymax;
-                    }
-                    if (i == 0) {
-                        const int nb = (ymax + 127) >> 7;  // 128-word blocks per variant row
-                        d[6] = total;
-                        d[7] = ymax;
-                        d[9] = nb;
-                        d[10] = ((1 << 20) + nb - 1) / nb;  // item -> row by a multiplication (items < 2^20 / nb)
-                    }
-                    if (v < r[0]) {
-                        const int code = r[4 + 2 * G + v];
-                        int* o = rowd + (size_t)(base + v) * 8;
-                        o[0] = H + r[1] + 1;
-                        o[1] = (base + v) * lw;
-#pragma unroll
-                        for (int m = 0; m < G; ++m) {
-                            const int tau = m == 0 ? 0 : (int)(signed char)((code >> (8 * (m - 1))) & 0xff);
-                            const int carry = (int)(((long long)tile_t + r[4 + m]) & 15);
-                            o[2 + m] = (q * G + m) * le + DDP_MRG_EPAD + carry + tau;
+    if (warp >= NCW) {
+        // =============================================================================== producers
+        if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        const int ptid = tid - NCT, pwarp = warp - NCW;
+        // descriptor roles: TMA extents on producer warp 0, variant rows from warp 1 on, window offsets from warp 2 on
+        const int rB = ptid - 32, sB = NPT - 32, rC = ptid - 64, sC = NPT - 64;
+        int rot = pwarp - 1;  // first item of this warp in the current iteration (warps 1..)
+        for (int n = -5; n < nstream; ++n) {
+            // ---- schedule chunk n + 5 (one thread; the cursor {unit, chunk, segment, time tile, DM tile, group} lives in shared memory)
+            if (ptid == 0) {
+                const int x = n + 5;
+                int* d = slot(x);
+                const int unit = sched[0], c = sched[1];
+                if (x < nstream && unit < unit_hi) {
+                    const int seg = sched[2], tt = sched[3], dt = sched[4], g = sched[5];
+                    const int rows = p.nred - seg * FL < FL ? p.nred - seg * FL : FL;
+                    const int nch = WIDE ? rows / U : p.nred / U;
+                    const int r0 = seg * FL + c * U;
+                    d[0] = tt * TT;
+                    d[1] = dt * TD;
+                    d[2] = (dt + 1) * TD <= p.ndm ? TD : p.ndm - dt * TD;
+                    d[3] = g;
+                    d[4] = r0;
+                    d[5] = 1 | (c == 0 ? 2 : 0) | (c == nch - 1 ? 4 : 0);
+                    const long long rec = ((long long)dt * p.meta_ngg + (long long)g * p.meta_gg0_stride + r0 / G) * RW;
+                    ddp_mbar_expect_tx(&mbar[2 + (x & 1)], (ddp_u32)(NG * RW * 4));
+                    ddp_bulk_g2s(stg + (size_t)(x & 1) * NG * RW, (const int*)p.meta + rec, (ddp_u32)(NG * RW * 4), &mbar[2 + (x & 1)]);
+                    if (c + 1 < nch) {
+                        sched[1] = c + 1;
+                    } else {  // next unit: segment-minor, then time tile, DM tile, group
+                        sched[0] = unit + 1;
+                        sched[1] = 0;
+                        if (seg + 1 < nseg) {
+                            sched[2] = seg + 1;
+                        } else {
+                            sched[2] = 0;
+                            if (tt + 1 < p.n_ttiles) {
+                                sched[3] = tt + 1;
+                            } else {
+                                sched[3] = 0;
+                                if (dt + 1 < p.n_dtiles) { sched[4] = dt + 1; } else { sched[4] = 0; sched[5] = g + 1; }
+                            }
                         }
                     }
-                }
-                for (int i = rC; i >= 0 && i < TD * NG; i += sC) {
-                    const int j = i / NG, q = i - j * NG;
-                    int base = 0;
-#pragma unroll
-                    for (int qq = 0; qq < NG; ++qq)
-                        if (qq < q) base += rec[qq * RW];
-                    const ddp_u32 code = (ddp_u32)rec[q * RW + 4 + 2 * G + VCAP + j];
-                    offs[i] = (ddp_u32)(((base + (int)(code >> 24)) * lw + (int)(code & 0xffffffu)) * 4);
+                } else {
+                    d[5] = 0;
                 }
             }
-        }
-        // ---- TMA: raw windows of chunk n + 3 (warp 0, lane u < U) -> raw slot (n + 3) & 1
-        if (warp == 0) {
-            const int x = n + 3;
-            const int* d = slot(x);
-            if (x >= 0 && x < nstream) {
-                const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)d[3] * p.in_group_stride;
-                const ddp_u32 bytes = lane < U ? (ddp_u32)d[16 + U + lane] : 0u;
-                ddp_u32 total = bytes;
+            // ---- descriptors of chunk n + 4 from its records
+            {
+                const int x = n + 4;
+                int* d = slot(x);
+                if (x >= 0 && x < nstream) {
+                    const int* rec = stg + (size_t)(x & 1) * NG * RW;
+                    ddp_mbar_wait(&mbar[2 + (x & 1)], (ddp_u32)((x >> 1) & 1));
+                    const int tile_t = d[0];
+                    int* a0s = d + 16;
+                    int* byts = a0s + U;
+                    int* carr = byts + U;
+                    int* nz4s = carr + U;
+                    int* rowd = nz4s + U;
+                    ddp_u32* offs = (ddp_u32*)(rowd + 8 * rows_max);
+                    if (pwarp == 0) {  // TMA extent and expansion length of reduction row `lane` of the chunk
+                        int nz4 = 0;
+                        if (lane < U) {
+                            const int* r = rec + (lane / G) * RW;
+                            const int dmin = r[4 + lane % G], dmax = r[4 + G + lane % G];
+                            const long long src = (long long)tile_t + dmin;
+                            const long long a0 = src & ~15ll;
+                            const int carry = (int)(src - a0);
+                            int need = ((carry + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
+                            need = (need + 3) & ~3;
+                            if (need > (win >> 2)) need = win >> 2;
+                            long long l = (p.in_row_len - 16 - a0) >> 2;  // the word after the last staged one stays inside the row
+                            const int lenw = (int)(l < need ? (l < 0 ? 0 : l) : need);
+                            nz4 = (carry + (dmax - dmin) + H + 3) >> 2;
+                            a0s[lane] = (int)a0;
+                            byts[lane] = lenw > 0 ? lenw * 4 + 16 : 0;
+                            carr[lane] = carry;
+                            nz4s[lane] = nz4;
+                        }
 #pragma unroll
-                for (int s = 16; s >= 1; s >>= 1) total += __shfl_xor_sync(0xffffffffu, total, s);
-                if (lane == 0) ddp_mbar_expect_tx(&mbar[x & 1], total);
-                __syncwarp();
-                if (bytes)
-                    ddp_bulk_g2s(raw + ((size_t)(x & 1) * U + lane) * (win + 16),
-                                 in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[16 + lane], bytes, &mbar[x & 1]);
+                        for (int s = 16; s >= 1; s >>= 1) {
+                            const int o = __shfl_xor_sync(0xffffffffu, nz4, s);
+                            nz4 = o > nz4 ? o : nz4;
+                        }
+                        if (lane == 0) d[8] = nz4;
+                    }
+                    for (int i = rB; i >= 0 && i < NG * VCAP; i += sB) {
+                        const int q = i / VCAP, v = i - q * VCAP;
+                        const int* r = rec + q * RW;
+                        int base = 0, total = 0, ymax = 0;
+#pragma unroll
+                        for (int qq = 0; qq < NG; ++qq) {
+                            const int nv = rec[qq * RW];
+                            if (qq < q) base += nv;
+                            total += nv;
+                            const int yl = H + rec[qq * RW + 1] + 1;
+                            ymax = yl > ymax ? yl : ymax;
+                        }
+                        if (i == 0) {
+                            const int nb = (ymax + 127) >> 7;  // 128-word blocks per variant row
+                            d[6] = total;
+                            d[7] = ymax;
+                            d[9] = nb;
+                            d[10] = ((1 << 20) + nb - 1) / nb;  // item -> row by a multiplication (items < 2^20 / nb)
+                        }
+                        if (v < r[0]) {
+                            const int code = r[4 + 2 * G + v];
+                            int* o = rowd + (size_t)(base + v) * 8;
+                            o[0] = H + r[1] + 1;
+                            o[1] = (base + v) * lw;
+#pragma unroll
+                            for (int m = 0; m < G; ++m) {
+                                const int tau = m == 0 ? 0 : (int)(signed char)((code >> (8 * (m - 1))) & 0xff);
+                                const int carry = (int)(((long long)tile_t + r[4 + m]) & 15);
+                                o[2 + m] = (q * G + m) * le + DDP_MRG_EPAD + carry + tau;
+                            }
+                        }
+                    }
+                    for (int i = rC; i >= 0 && i < TD * NG; i += sC) {
+                        const int j = i / NG, q = i - j * NG;
+                        int base = 0;
+#pragma unroll
+                        for (int qq = 0; qq < NG; ++qq)
+                            if (qq < q) base += rec[qq * RW];
+                        const ddp_u32 code = (ddp_u32)rec[q * RW + 4 + 2 * G + VCAP + j];
+                        offs[i] = (ddp_u32)(((base + (int)(code >> 24)) * lw + (int)(code & 0xffffffu)) * 4);
+                    }
+                }
             }
+            // ---- TMA: raw windows of chunk n + 3 (producer warp 0, lane u < U) -> raw slot (n + 3) & 1
+            if (pwarp == 0) {
+                const int x = n + 3;
+                const int* d = slot(x);
+                if (x >= 0 && x < nstream) {
+                    const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)d[3] * p.in_group_stride;
+                    const ddp_u32 bytes = lane < U ? (ddp_u32)d[16 + U + lane] : 0u;
+                    ddp_u32 total = bytes;
+#pragma unroll
+                    for (int s = 16; s >= 1; s >>= 1) total += __shfl_xor_sync(0xffffffffu, total, s);
+                    if (lane == 0) ddp_mbar_expect_tx(&mbar[x & 1], total);
+                    __syncwarp();
+                    if (bytes)
+                        ddp_bulk_g2s(raw + ((size_t)(x & 1) * U + lane) * (win + 16),
+                                     in_g + (ddp_i64)(d[4] + lane) * p.in_row_stride + d[16 + lane], bytes, &mbar[x & 1]);
+                }
+            }
+            // ---- build chunk n + 1 (E rows -> variant rows of buffer (n + 1) & 1) and expand chunk n + 2 (raw slot -> E rows):
+            //      items = half rows, handed out round robin to producer warps 1.. (warp 0 keeps the control work above)
+            {
+                const int xb = n + 1, xs = n + 2;
+                const int* db = slot(xb);
+                const int* ds = slot(xs);
+                const bool vb = xb >= 0 && xb < nstream, vs = xs >= 0 && xs < nstream;
+                if (vb && xb >= 2) ddp_mbar_wait(&mbar[6 + (xb & 1)], (ddp_u32)(((xb >> 1) - 1) & 1));  // consumers left this buffer
+                if (vs) ddp_mbar_wait(&mbar[xs & 1], (ddp_u32)((xs >> 1) & 1));                          // raw windows landed
+                if (pwarp > 0) {
+                    const int NB = vb ? 2 * db[6] : 0;       // build items: (variant row, half)
+                    const int NI = NB + (vs ? 2 * U : 0);    // expand items: (channel, half)
+                    const int* rowd = db + 16 + 4 * U;
+                    const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
+                    ddp_u32* pb = pw + (size_t)(xb & 1) * rows_max * lw + lane;
+                    const int* nz4s = ds + 16 + 3 * U;
+                    const int hq = H >> 2;
+                    const unsigned char* rbase = raw + (size_t)(xs & 1) * U * (win + 16);
+                    ddp_u32* ebase = ebuf + (size_t)(xs & 1) * U * le + DDP_MRG_EPAD;
+                    for (int it = rot; it < NI; it += NPW - 1) {
+                        if (it < NB) {
+                            const int row = it >> 1;
+                            const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                            const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
+                            const int half = ((d0.x >> 1) + 127) & ~127;
+                            int y = (it & 1) ? half : 0;
+                            const int yend = (it & 1) ? d0.x : (half < d0.x ? half : d0.x);
+                            const ddp_u32* e0 = eb + d0.z;
+                            const ddp_u32* e1 = eb + d0.w;
+                            const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0);
+                            const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0);
+                            ddp_u32* dst = pb + d0.y;
+                            for (; y + 128 <= yend; y += 128) {  // whole blocks of 128 words: all loads first
+                                ddp_u32 sm[4];
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) {
+                                    sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
+                                    if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
+                                }
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) dst[y + 32 * i] = sm[i];
+                            }
+                            for (; y + lane < yend; y += 32) {
+                                ddp_u32 s0 = e0[y] + e1[y];
+                                if constexpr (G > 2) s0 += e2[y] + e3[y];
+                                dst[y] = s0;
+                            }
+                        } else {
+                            const int is = it - NB;
+                            const int u = is >> 1;
+                            const int nz = nz4s[u];
+                            const int halfq = ((nz >> 1) + 31) & ~31;
+                            int q4 = ((is & 1) ? halfq : 0) + lane;
+                            const int qend = (is & 1) ? nz : (halfq < nz ? halfq : nz);
+                            const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
+                            ddp_u32* dst = ebase + (size_t)u * le;
+                            for (; q4 < qend; q4 += 32) {
+                                const ddp_u32 lo = src[q4], hi = src[q4 + hq];
+                                const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
+                                const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
+                                *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
+                                                                     __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                            }
+                        }
+                    }
+                    rot = rot + 1 < NPW - 1 ? rot + 1 : 0;  // the warp that starts the round changes every iteration
+                }
+                if (vb) {  // this warp's share of buffer (n + 1) & 1 is written
+                    __syncwarp();
+                    if (lane == 0) ddp_mbar_arrive(&mbar[4 + (xb & 1)]);
+                }
+            }
+            ddp_named_barrier(1, NPT);
         }
-        // ---- sum chunk n: every trial adds its variant rows, then (last chunk of a unit) flush
-        if (n >= 0) {
+    } else {
+        // =============================================================================== consumers
+        if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");  // 512 x 96 + 256 x 48 = the 768 x 80 registers the block was launched with
+        const int tx = tid % p.threads_t, ty = tid / p.threads_t;
+        const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
+        ddp_u32 acc[DPT][K];
+#pragma unroll
+        for (int j = 0; j < DPT; ++j)
+#pragma unroll
+            for (int k = 0; k < K; ++k) acc[j][k] = 0u;
+        for (int n = 0; n < nstream; ++n) {
             const int* d = slot(n);
+            ddp_mbar_wait(&mbar[4 + (n & 1)], (ddp_u32)((n >> 1) & 1));  // variant rows of chunk n are built
+            // ---- sum chunk n: every trial adds its variant rows
             const ddp_u32* ob = (const ddp_u32*)(d + 16 + 4 * U + 8 * rows_max) + (size_t)(ty * DPT) * NG;
             const unsigned char* lanep = (const unsigned char*)(pw + (size_t)(n & 1) * rows_max * lw + wb);
 #pragma unroll
@@ -911,8 +1018,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                     for (int k = 0; k < K; ++k) acc[j][k] += wp[32 * k];
                 }
             }
-            if (d[5] & 4) {  // block-uniform: last chunk of the unit
-                const int tile_t = d[0], tile_dm = d[1], g = d[3];
+            const int flags = d[5], tile_t = d[0], tile_dm = d[1], g = d[3];
+            __syncwarp();
+            if (lane == 0) ddp_mbar_arrive(&mbar[6 + (n & 1)]);  // this warp has left buffer n & 1
+            if (flags & 4) {  // block-uniform: last chunk of the unit -> flush
 #pragma unroll
                 for (int j = 0; j < DPT; ++j) {
                     const int dm = tile_dm + ty * DPT + j;
@@ -942,88 +1051,6 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 }
             }
         }
-        // ---- build chunk n + 1 and expand chunk n + 2: items handed out by a shared counter, so that the warps that
-        //      carried a descriptor role or a flush in this iteration take fewer and all reach the barrier together
-        {
-            const int xb = n + 1, xs = n + 2;
-            const int* db = slot(xb);
-            const int* ds = slot(xs);
-            const bool vb = xb >= 0 && xb < nstream, vs = xs >= 0 && xs < nstream;
-            const int R = vb ? db[6] : 0, nblk = vb ? db[9] : 1, rcp = vb ? db[10] : 0;
-            const int NB = R * nblk;                                  // build items: (variant row, 128 words)
-            const int nblks = vs ? (ds[8] + 63) >> 6 : 0;             // expand items: (channel, 64 four-sample groups)
-            const int NI = NB + (nblks << LGU);
-            const int* rowd = db + 16 + 4 * U;
-            const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
-            ddp_u32* pb = pw + (size_t)(xb & 1) * rows_max * lw + lane;
-            const int* nz4s = ds + 16 + 3 * U;
-            const int hq = H >> 2;
-            const unsigned char* rbase = raw + (size_t)(xs & 1) * U * (win + 16);
-            ddp_u32* ebase = ebuf + (size_t)(xs & 1) * U * le + DDP_MRG_EPAD;
-            bool raw_ready = false;
-            int* cnt = sched + 2 + (n & 1);
-            for (;;) {
-                int it = 0;
-                if (lane == 0) it = atomicAdd(cnt, 1);
-                it = __shfl_sync(0xffffffffu, it, 0);
-                if (it >= NI) break;
-                if (it < NB) {
-                    const int row = (int)(((ddp_u32)it * (ddp_u32)rcp) >> 20), y0 = (it - row * nblk) << 7;
-                    const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
-                    const int ylen = d0.x - lane;  // words of this lane's column left in the row
-                    if (y0 >= d0.x) continue;      // warp-uniform
-                    const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-                    const ddp_u32* e0 = eb + d0.z + y0;
-                    const ddp_u32* e1 = eb + d0.w + y0;
-                    const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0) + y0;
-                    const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0) + y0;
-                    ddp_u32* dst = pb + d0.y + y0;
-                    if (y0 + 128 <= d0.x) {  // whole item (warp-uniform): all loads first
-                        ddp_u32 sm[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            sm[i] = e0[32 * i] + e1[32 * i];
-                            if constexpr (G > 2) sm[i] += e2[32 * i] + e3[32 * i];
-                        }
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) dst[32 * i] = sm[i];
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            if (y0 + 32 * i < ylen) {
-                                ddp_u32 s0 = e0[32 * i] + e1[32 * i];
-                                if constexpr (G > 2) s0 += e2[32 * i] + e3[32 * i];
-                                dst[32 * i] = s0;
-                            }
-                        }
-                    }
-                } else {
-                    if (!raw_ready) {
-                        ddp_mbar_wait(&mbar[xs & 1], (ddp_u32)((xs >> 1) & 1));
-                        raw_ready = true;
-                    }
-                    const int is = it - NB;
-                    const int u = is & (U - 1), q4 = ((is >> LGU) << 6) + lane;
-                    const int nz = nz4s[u];
-                    const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
-                    ddp_u32* dst = ebase + (size_t)u * le;
-                    ddp_u32 lo[2], hi[2];
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if (q4 + 32 * i < nz) { lo[i] = src[q4 + 32 * i]; hi[i] = src[q4 + 32 * i + hq]; }
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        if (q4 + 32 * i < nz) {
-                            const ddp_u32 elo = lo[i] & 0x00ff00ffu, ehi = hi[i] & 0x00ff00ffu;
-                            const ddp_u32 olo = __byte_perm(lo[i], 0u, 0x4341u), ohi = __byte_perm(hi[i], 0u, 0x4341u);
-                            *(uint4*)(dst + 4 * (q4 + 32 * i)) =
-                                make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
-                                           __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
-                        }
-                }
-            }
-        }
-        __syncthreads();
     }
 }
 
@@ -1554,12 +1581,13 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
 // uint8 / uint16 input with staging takes the packed kernels; everything else the generic one.
 // FLAGS: bit 0 WIDE (uint8 packed: reduction longer than 256 rows), bit 1 OUT16 (uint16 result: the
 // narrow subband intermediate), bits 2-3 log2 of the uint16 packed kernel's lane-sum group, bit 4 SINGLE
-// (uint8 packed: one buffer of shifted copies, chosen by the host when two do not fit).
+// (uint8 packed: one buffer of shifted copies, chosen by the host when two do not fit), bit 5 REGSPLIT (merged
+// kernel with 512 consumer threads + 8 producer warps: setmaxnreg moves registers from the producers to the consumers).
 template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, int FLAGS>
 __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
     constexpr bool WIDE = (FLAGS & 1) != 0, OUT16 = (FLAGS & 2) != 0, SINGLE = (FLAGS & 16) != 0;
     if constexpr (sizeof(IN_T) == 1 && STAGING >= 3)
-        ddp_dedisp_merge_body<SPT, DPT, UNROLL, (STAGING == 3 ? 2 : 4), WIDE, OUT16>(p);
+        ddp_dedisp_merge_body<SPT, DPT, UNROLL, (STAGING == 3 ? 2 : 4), WIDE, OUT16, (FLAGS & 32) != 0>(p);
     else if constexpr (sizeof(IN_T) == 1 && STAGING != 0)
         ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16, SINGLE>(p);
     else if constexpr (sizeof(IN_T) == 2 && STAGING != 0)
@@ -1568,7 +1596,7 @@ __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
         ddp_dedisp_body<IN_T, SPT, DPT, UNROLL, STAGING, VEC, OUT16>(p);
 }
 #define DDP_DEFINE_DEDISP(NAME, IN_T, SPT, DPT, UNROLL, STAGING, VEC, MAXT, FLAGS)                  \
-    extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpDedispParams p) {                 \
+    extern "C" __global__ void __launch_bounds__(MAXT, 1) NAME(const DdpDedispParams p) {              \
         ddp_dedisp_entry<IN_T, SPT, DPT, UNROLL, STAGING, VEC, (FLAGS)>(p);                            \
     }
 #define DDP_DEFINE_INTEG(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                \

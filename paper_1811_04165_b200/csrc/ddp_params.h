@@ -34,6 +34,7 @@ struct DdpDedispParams {
     int meta_rw;                 //   int32 words per record
     int meta_ngg;                //   groups per DM tile in the table (all subbands)
     int meta_gg0_stride;         //   table groups between consecutive kernel groups g (subband step 1: cps / G; direct: 0)
+    int threads_t, threads_dm;   // merged staging: consumer threads along time / DM (the block adds 4 or 8 producer warps)
     int n_ttiles, n_dtiles;      // merged staging (persistent kernel): time tiles, DM tiles,
     int nseg;                    //   segments of <= 256 reduction rows per tile,
     int nunits;                  //   work units = groups * n_dtiles * n_ttiles * nseg

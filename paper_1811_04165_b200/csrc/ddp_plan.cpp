@@ -459,7 +459,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += 2 * U * (row + 16);                              // raw
                 b += 2 * NG * (size_t)mg.rw * 4;                      // record staging
                 b += 8 * (((16 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
-                b += 4 * 8 + 16;                                      // mbarriers, scheduler cursor
+                b += 8 * 8 + 32;                                      // mbarriers, scheduler cursor
                 return b;
             }
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
@@ -529,6 +529,7 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
         if (c.vec_bytes != 16) return no("V7: merged staging ignores vec_bytes; must be 16");
         if (c.samples_per_thread < 2) return no("V5: merged staging needs samples_per_thread >= 2");
         if (c.threads_t < 32) return no("V1: merged staging needs threads_t >= 32");
+        if (threads > 512) return no("V1: merged staging adds its producer warps to the block: at most 512 consumer threads");
         if ((c.threads_dm * c.dms_per_thread) % 4 != 0) return no("V3: merged staging needs a DM tile of a multiple of 4 trials");
     }
     // V5: vector width vs. what a thread loads contiguously

@@ -240,13 +240,15 @@ const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck 
 //   bit 1  OUT16  subband step 1 writes the narrow (uint16) intermediate;
 //   bits 2-3      packed uint16 kernel (step 2): log2 of how many subband words are summed in 16-bit
 //                 lanes before they are split, the largest of {1, 2, 4} that cannot overflow;
-//   bit 4  SINGLE packed uint8 kernel with one buffer of shifted copies (two do not fit in 227 KB).
+//   bit 4  SINGLE packed uint8 kernel with one buffer of shifted copies (two do not fit in 227 KB);
+//   bit 5  REGSPLIT merged kernel with 512 consumer threads: setmaxnreg hands the producers' spare registers to them.
 int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const CodeKind ck = code_kind(p, k);
     int f = 0;
     if (ck == CK_DEDISP_U8 && c.staging != 0 && ddp_kgeom(p, k).nred > 257) f |= 1;  // 257 * 255 = 65535 still fits the lanes
     if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
     if (ck == CK_DEDISP_U8 && ddp_u8_single_buffered(p, k, c)) f |= 16;
+    if (ck == CK_DEDISP_U8 && ddp_merge_group(c) && c.threads_t * c.threads_dm >= 512) f |= 32;  // REGSPLIT
     if (ck == CK_DEDISP_U16 && c.staging != 0) {
         const int64_t room = 65535 / (255 * (int64_t)p->cps);
         f |= (room >= 4 ? 2 : (room >= 2 ? 1 : 0)) << 2;
@@ -256,7 +258,8 @@ int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
 // threads_t x threads_dm is a launch parameter; the code shape only sees it through
 // __launch_bounds__, whose register cap is the same (255) for every block of <= 256 threads.
 int maxt_bucket(const ddp_kcfg& c) {
-    const int t = c.threads_t * c.threads_dm;
+    int t = c.threads_t * c.threads_dm;
+    if (ddp_merge_group(c)) t += ddp_merge_producer_threads(c);  // the merged kernel adds its producer warps to the block
     return t <= 256 ? 256 : t;
 }
 std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
@@ -761,7 +764,9 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
         if (nunits > 0x7fffffff) return ddp_fail(p, DDP_E_CONFIG, K->name + ": too many work units");
         q.nunits = (int)nunits;
         const size_t smem = ddp_smem_bytes(p, k, c);
-        const int threads = c.threads_t * c.threads_dm;
+        q.threads_t = c.threads_t;
+        q.threads_dm = c.threads_dm;
+        const int threads = c.threads_t * c.threads_dm + ddp_merge_producer_threads(c);  // consumers + producer warps
         int per_sm = 0, nsm = 0;
         CUdevice dev;
         if (g_api.p_cuDeviceGet(&dev, p->device) != CUDA_SUCCESS ||
@@ -776,7 +781,7 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
             if (r != CUDA_SUCCESS) return ddp_fail(p, DDP_E_CUDA, "zeroing the output: " + cu_err(r));
         }
         const int64_t grid = std::min<int64_t>(nunits, (int64_t)per_sm * nsm);
-        return launch(p, K, (unsigned)grid, 1, 1, (unsigned)c.threads_t, (unsigned)c.threads_dm, smem, io.stream, &q);
+        return launch(p, K, (unsigned)grid, 1, 1, (unsigned)threads, 1u, smem, io.stream, &q);
     }
     return launch(p, K, cdiv(q.ns, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,
                   ddp_smem_bytes(p, k, c), io.stream, &q);
