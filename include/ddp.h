@@ -55,7 +55,9 @@ typedef enum {
     DDP_K_SUB2 = 2,      /* step two: subbands -> fine DM trials per coarse DM     */
     DDP_K_INTEGRATE = 3, /* decimating boxcar sums per width   */
     DDP_K_SNR = 4,       /* (max-mean)/std per (DM, width)                        (BJ:cfg0)     */
-    DDP_K_COUNT = 5
+    DDP_K_ISNR = 5,      /* integration and S/N in one pass over the dedispersed series; not a
+                            slot of the tuners' joint configuration (BJ:cfg4 names four kernels)              */
+    DDP_K_COUNT = 6
 } ddp_kernel;
 
 /* One "kernel chromosome" (gene set and value ranges from BJ:cfg4, cf. Table 3):
@@ -164,13 +166,35 @@ ddp_status ddp_integrate(ddp_plan* plan, const uint32_t* d_dedisp, size_t stride
  *   of the maximum; a constant series gives snr = 0, argmax = 0. */
 ddp_status ddp_snr(ddp_plan* plan, const uint32_t* d_dedisp, size_t stride, const uint32_t* d_integ,
                    float* d_snr, uint32_t* d_argmax, void* stream);
+/* ddp_integrate_snr (INT.1-2, SNR.1-4): integration and S/N in ONE kernel.  The dedispersed series
+ *   is read once; the block sums of every width are formed in registers and fed straight into the exact integer
+ *   moment / max accumulators of their width, so d_snr / d_argmax hold bit for bit what ddp_integrate followed by
+ *   ddp_snr gives.  d_integ may be NULL: the planes are then never written (that is the point: at BJ:cfg1 they
+ *   are 199 MB written and read again); when it is given, the planes are stored too, identical to ddp_integrate's.
+ *   Kernel configuration DDP_K_ISNR: threads_t = 32 (one warp per series), threads_dm series per block,
+ *   samples_per_thread in {4, 8, 16}, dms_per_thread series per warp one after the other; the other genes are pinned. */
+ddp_status ddp_integrate_snr(ddp_plan* plan, const uint32_t* d_dedisp, size_t stride, uint32_t* d_integ, float* d_snr,
+                             uint32_t* d_argmax, void* stream);
 /* One whole search through HOST buffers (the end-to-end path): copies h_in (uint8 [nchan][in_stride],
  * pinned or pageable host memory) into the caller's device buffer d_in, runs dedisperse -> integrate
- * -> snr on `stream`, copies the S/N table (and argmax if h_argmax != NULL) back to the host and
- * synchronises the stream before returning.  Device buffers as for the calls above. */
+ * -> snr on `stream` (d_integ == NULL: dedisperse -> ddp_integrate_snr, no planes), copies the S/N table (and
+ * argmax if h_argmax != NULL) back to the host and synchronises the stream before returning.  Device buffers as
+ * for the calls above. */
 ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_t in_stride, uint8_t* d_in,
                            uint32_t* d_out, size_t out_stride, uint32_t* d_integ, float* d_snr,
                            uint32_t* d_argmax, float* h_snr, uint32_t* h_argmax, void* stream);
+/* Consecutive batches of one observation: h_in is uint8 [nchan][h_stride] host memory
+ * (pinned for the copies to overlap) holding at least nbatches*nsamp_out + max_delay samples per channel; batch b
+ * searches samples [b*nsamp_out, (b+1)*nsamp_out + max_delay) -- exactly the columns b*nsamp_out.. of one long
+ * dedispersion.  Only the nsamp_out NEW samples of a batch are uploaded: the max_delay samples shared with the
+ * previous batch are carried over on the device between the two input buffers d_in0 / d_in1 (each uint8
+ * [nchan][in_stride], as for ddp_dedisperse), and the upload of batch b+1 runs on a plan-owned copy stream while
+ * batch b is searched on `stream` (dedisperse -> ddp_integrate_snr, no planes).  h_snr float32 [nbatches][ndm]
+ * [nwidths]; h_argmax likewise or NULL.  Both streams are synchronised before returning. */
+ddp_status ddp_search_host_batches(ddp_plan* plan, const uint8_t* h_in, size_t h_stride, int nbatches,
+                                   uint8_t* d_in0, uint8_t* d_in1, size_t in_stride, uint32_t* d_out,
+                                   size_t out_stride, float* d_snr, uint32_t* d_argmax, float* h_snr,
+                                   uint32_t* h_argmax, void* stream);
 /* Debug accessor: device pointer of the subband intermediate S[n_coarse][n_subbands][sub_stride]
  * (elements of sub_elem_bytes bytes: uint16 or uint32) inside the bound workspace (NULL for a direct
  * plan or before bind). */
@@ -250,6 +274,10 @@ typedef struct {
     double wall_seconds;
     double* history; size_t history_cap; size_t history_len; /* caller array: best-so-far after each fitness call */
     double sum_isolated_min_ms;     /* brute force: sum of the per-kernel minima (GA.6)                 */
+    /* optional, caller arrays ("configurations at the end of every algorithm run"): the GA's last population,
+       best first -- random search: the last final_cap configurations it drew -- as final_len joint configurations
+       of DDP_NSLOTS ddp_kcfg each, with their fitness values; final_pop == NULL: not recorded */
+    ddp_kcfg* final_pop; double* final_fit; size_t final_cap; size_t final_len;
 } ddp_tune_result;
 
 ddp_status ddp_tune_ga(ddp_plan* plan, const ddp_tune_io* io, const ddp_ga_params* p, ddp_tune_result* res);

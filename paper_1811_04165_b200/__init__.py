@@ -8,13 +8,13 @@ that allocates the device buffers of a plan with PyTorch.
 """
 from __future__ import annotations
 
-from .binding import (DDP_NSLOTS, K_DIRECT, K_INTEGRATE, K_SNR, K_SUB1, K_SUB2, KCACHE_DIR, KERNEL_NAMES,
+from .binding import (DDP_NSLOTS, K_DIRECT, K_INTEGRATE, K_ISNR, K_SNR, K_SUB1, K_SUB2, KCACHE_DIR, KERNEL_NAMES,
                       STAGE_DIRECT, STAGE_SMEM, STAGE_TMA, SYMBOLS, DdpError, Kcfg, Plan, PlanInfo, TuneIo,
                       lib, make_tune_io, plan_create, status_str, version)
 
 __all__ = ["plan_create", "Plan", "Kcfg", "PlanInfo", "TuneIo", "DdpError", "make_tune_io", "alloc_buffers",
            "plan_from_config", "lib", "status_str", "version", "SYMBOLS", "KERNEL_NAMES", "DDP_NSLOTS",
-           "K_DIRECT", "K_SUB1", "K_SUB2", "K_INTEGRATE", "K_SNR", "STAGE_DIRECT", "STAGE_SMEM", "STAGE_TMA",
+           "K_DIRECT", "K_SUB1", "K_SUB2", "K_INTEGRATE", "K_SNR", "K_ISNR", "STAGE_DIRECT", "STAGE_SMEM", "STAGE_TMA",
            "KCACHE_DIR"]
 
 

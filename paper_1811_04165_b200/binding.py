@@ -19,15 +19,15 @@ KCACHE_DIR = os.path.join(_HERE, "kcache")
 
 DDP_MAX_WIDTHS = 16
 DDP_NSLOTS = 4
-K_DIRECT, K_SUB1, K_SUB2, K_INTEGRATE, K_SNR = 0, 1, 2, 3, 4
-KERNEL_NAMES = ("direct", "sub1", "sub2", "integrate", "snr")
+K_DIRECT, K_SUB1, K_SUB2, K_INTEGRATE, K_SNR, K_ISNR = 0, 1, 2, 3, 4, 5
+KERNEL_NAMES = ("direct", "sub1", "sub2", "integrate", "snr", "isnr")
 STAGE_DIRECT, STAGE_SMEM, STAGE_TMA = 0, 1, 2
 E_ARG, E_SHAPE, E_OVERFLOW, E_WORKSPACE, E_CONFIG, E_COMPILE, E_CUDA, E_BUDGET = -1, -2, -3, -4, -5, -6, -7, -8
 
 # every symbol include/ddp.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "ddp_plan_create", "ddp_plan_destroy", "ddp_plan_query", "ddp_plan_get_delays",
-    "ddp_plan_bind_workspace", "ddp_dedisperse", "ddp_integrate", "ddp_snr", "ddp_search_host",
+    "ddp_plan_bind_workspace", "ddp_dedisperse", "ddp_integrate", "ddp_snr", "ddp_integrate_snr", "ddp_search_host", "ddp_search_host_batches",
     "ddp_plan_subband_buffer", "ddp_get_kcfg", "ddp_set_kcfg", "ddp_check_kcfg", "ddp_repair_kcfg",
     "ddp_compile_kcfg", "ddp_enumerate_kcfgs", "ddp_tune_ga", "ddp_tune_bruteforce",
     "ddp_tune_random", "ddp_time_pipeline", "ddp_status_str", "ddp_last_error", "ddp_version",
@@ -102,7 +102,9 @@ class TuneResult(C.Structure):
     _fields_ = [("best", Kcfg * DDP_NSLOTS), ("best_ms", C.c_double), ("kernel_ms", C.c_double * DDP_NSLOTS),
                 ("n_fitness_calls", C.c_int64), ("n_kernel_timings", C.c_int64), ("n_compiles", C.c_int64),
                 ("wall_seconds", C.c_double), ("history", C.POINTER(C.c_double)), ("history_cap", C.c_size_t),
-                ("history_len", C.c_size_t), ("sum_isolated_min_ms", C.c_double)]
+                ("history_len", C.c_size_t), ("sum_isolated_min_ms", C.c_double),
+                ("final_pop", C.POINTER(Kcfg)), ("final_fit", C.POINTER(C.c_double)), ("final_cap", C.c_size_t),
+                ("final_len", C.c_size_t)]
 
 
 _lib = None
@@ -126,7 +128,10 @@ def lib():
         L.ddp_dedisperse.argtypes = [vp, vp, C.c_size_t, vp, C.c_size_t, vp]
         L.ddp_integrate.argtypes = [vp, vp, C.c_size_t, vp, vp]
         L.ddp_snr.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp]
+        L.ddp_integrate_snr.argtypes = [vp, vp, C.c_size_t, vp, vp, vp, vp]
         L.ddp_search_host.argtypes = [vp, vp, C.c_size_t, vp, vp, C.c_size_t, vp, vp, vp, vp, vp, vp]
+        L.ddp_search_host_batches.argtypes = [vp, vp, C.c_size_t, C.c_int, vp, vp, C.c_size_t, vp, C.c_size_t, vp, vp, vp,
+                                              vp, vp]
         L.ddp_plan_subband_buffer.argtypes = [vp, C.POINTER(vp)]
         for f in ("ddp_get_kcfg", "ddp_set_kcfg", "ddp_check_kcfg", "ddp_repair_kcfg", "ddp_compile_kcfg"):
             getattr(L, f).argtypes = [vp, C.c_int, C.POINTER(Kcfg)]
@@ -246,10 +251,23 @@ class Plan:
         self._check(lib().ddp_snr(self._h, _ptr(d_dedisp), _row_stride(d_dedisp, stride), _ptr(d_integ),
                                   _ptr(d_snr), _ptr(d_argmax), _stream(stream)), "ddp_snr")
 
+    def integrate_snr(self, d_dedisp, d_snr, d_argmax=None, d_integ=None, stride=None, stream=None):
+        """Fused integration + S/N; the planes are written only when d_integ is given."""
+        self._check(lib().ddp_integrate_snr(self._h, _ptr(d_dedisp), _row_stride(d_dedisp, stride), _ptr(d_integ),
+                                            _ptr(d_snr), _ptr(d_argmax), _stream(stream)), "ddp_integrate_snr")
+
     def search_host(self, h_in, d_in, d_out, d_integ, d_snr, d_argmax, h_snr, h_argmax=None, stream=None):
         self._check(lib().ddp_search_host(self._h, _ptr(h_in), _row_stride(h_in, None), _ptr(d_in), _ptr(d_out),
                                           _row_stride(d_out, None), _ptr(d_integ), _ptr(d_snr), _ptr(d_argmax),
                                           _ptr(h_snr), _ptr(h_argmax), _stream(stream)), "ddp_search_host")
+
+    def search_host_batches(self, h_in, nbatches, d_in0, d_in1, d_out, d_snr, d_argmax, h_snr, h_argmax=None,
+                            stream=None):
+        """Consecutive batches of one observation: h_in [nchan][>= nbatches*ns + max_delay], results [nbatches][ndm][nW]."""
+        self._check(lib().ddp_search_host_batches(self._h, _ptr(h_in), _row_stride(h_in, None), int(nbatches),
+                                                  _ptr(d_in0), _ptr(d_in1), _row_stride(d_in0, None), _ptr(d_out),
+                                                  _row_stride(d_out, None), _ptr(d_snr), _ptr(d_argmax), _ptr(h_snr),
+                                                  _ptr(h_argmax), _stream(stream)), "ddp_search_host_batches")
 
     # ---- kernel configurations
     def get_kcfg(self, k: int) -> Kcfg:
@@ -279,11 +297,17 @@ class Plan:
         return [arr[i].copy() for i in range(n.value)]
 
     # ---- tuning
-    def _result(self, history_cap: int):
+    def _result(self, history_cap: int, final_cap: int = 0):
         res = TuneResult()
         hist = (C.c_double * max(1, history_cap))()
         res.history = C.cast(hist, C.POINTER(C.c_double))
         res.history_cap = history_cap
+        if final_cap > 0:  # the configurations the run ends with
+            res._final_pop = (Kcfg * (final_cap * DDP_NSLOTS))()
+            res._final_fit = (C.c_double * final_cap)()
+            res.final_pop = C.cast(res._final_pop, C.POINTER(Kcfg))
+            res.final_fit = C.cast(res._final_fit, C.POINTER(C.c_double))
+            res.final_cap = final_cap
         return res, hist
 
     @staticmethod
@@ -292,14 +316,16 @@ class Plan:
                 "kernel_ms": list(res.kernel_ms), "n_fitness_calls": res.n_fitness_calls,
                 "n_kernel_timings": res.n_kernel_timings, "n_compiles": res.n_compiles,
                 "wall_seconds": res.wall_seconds, "history": [hist[i] for i in range(res.history_len)],
-                "sum_isolated_min_ms": res.sum_isolated_min_ms}
+                "sum_isolated_min_ms": res.sum_isolated_min_ms,
+                "final": [([res._final_pop[i * DDP_NSLOTS + s].copy() for s in range(DDP_NSLOTS)], res._final_fit[i])
+                          for i in range(res.final_len)] if res.final_cap else []}
 
     def tune_ga(self, io: TuneIo, seed=1, population=64, generations=50, tournament=3, p_cross=0.8,
                 crossover_kind=0, p_mut=0.05, mutation_kind=0, elitism=2, replacement=0, max_evals=0,
-                history_cap=1 << 16) -> dict:
+                history_cap=1 << 16, final_cap=0) -> dict:
         gp = GaParams(seed, population, generations, tournament, p_cross, crossover_kind, p_mut, mutation_kind,
                       elitism, replacement, max_evals)
-        res, hist = self._result(history_cap)
+        res, hist = self._result(history_cap, final_cap)
         self._check(lib().ddp_tune_ga(self._h, C.byref(io), C.byref(gp), C.byref(res)), "ddp_tune_ga")
         return self._pack(res, hist)
 
@@ -310,9 +336,9 @@ class Plan:
                     "ddp_tune_bruteforce")
         return self._pack(res, hist)
 
-    def tune_random(self, io: TuneIo, seed=1, max_evals=1000, history_cap=1 << 16) -> dict:
+    def tune_random(self, io: TuneIo, seed=1, max_evals=1000, history_cap=1 << 16, final_cap=0) -> dict:
         rp = RandParams(seed, max_evals)
-        res, hist = self._result(history_cap)
+        res, hist = self._result(history_cap, final_cap)
         self._check(lib().ddp_tune_random(self._h, C.byref(io), C.byref(rp), C.byref(res)), "ddp_tune_random")
         return self._pack(res, hist)
 

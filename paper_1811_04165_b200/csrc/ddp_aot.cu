@@ -11,6 +11,8 @@
 #define DDP_AOT_INTEG(S, D, U, G, V, T) DDP_DEFINE_INTEG(ddp_integ_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 #define DDP_AOT_SNR(S, D, U, G, V, T) DDP_DEFINE_SNR(ddp_snr_s##S##_d##D##_u##U##_g##G##_v##V##_t##T, S, D, U, G, V, T)
 
+#define DDP_AOT_ISNR(S, D, T) DDP_DEFINE_ISNR(ddp_isnr_s##S##_d##D##_t##T, S, D, T)
+
 // plan defaults (ddp_plan.cpp::default_kcfgs); W = code flags (bit 0 wide flush, bit 1 uint16 result,
 // bits 2-3 log2 lane-sum group of the packed uint16 kernel)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 1)
@@ -19,6 +21,7 @@ DDP_AOT_U16(4, 8, 8, 2, 16, 256, 8)
 DDP_AOT_U32(4, 4, 4, 0, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 0, 16, 256)
 DDP_AOT_SNR(4, 1, 4, 0, 16, 256)
+DDP_AOT_ISNR(16, 1, 256)
 // one instance of every staging mode per kernel (SASS evidence: LDS / UBLKCP paths)
 DDP_AOT_U8(8, 4, 8, 0, 4, 256, 0)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 0)

@@ -100,8 +100,8 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // packed uint8 kernel: one copy buffer
 // Merged staging (staging genes 3 / 4: G = 2 / 4 adjacent rows pre-summed exactly; uint8 dedispersion only).
 inline int ddp_merge_group(const ddp_kcfg& c) { return c.staging == 3 ? 2 : (c.staging == 4 ? 4 : 0); }
-// producer warps the merged kernel adds to its threads_t x threads_dm consumer threads (4 or 8 warps)
-inline int ddp_merge_producer_threads(const ddp_kcfg& c) { return c.threads_t * c.threads_dm >= 512 ? 256 : 128; }
+// producer warps the merged kernel adds to its threads_t x threads_dm consumer threads (4 or 12 warps)
+inline int ddp_merge_producer_threads(const ddp_kcfg& c) { return c.threads_t * c.threads_dm >= 512 ? 384 : 128; }
 int ddp_merge_vmax(const ddp_plan* p, ddp_kernel k, int TD, int G);  // largest number of distinct relative-shift tuples
 struct DdpMergeGeom { int vmax, vcap, rw, rows_max, lw, le; };
 int64_t ddp_merge_table_bytes(const ddp_plan* p, ddp_kernel k, int TD, int G);

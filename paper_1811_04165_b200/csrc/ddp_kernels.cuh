@@ -693,8 +693,21 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
 // Which variant a trial uses, every variant's shifts and the tile's first / last delays depend on the delay
 // table, TD and G only: the host tabulates them once per plan (DdpMergeTable, ddp_plan.cpp), one record per
 // (DM tile, group), so the kernel never reads the delay table.
-#define DDP_MRG_DEPTH 8   // descriptor ring slots (a chunk's descriptors live for 5 producer iterations + the consumers' lag)
+#define DDP_MRG_DEPTH 16  // descriptor ring slots: 5 producer stages ahead of the chunk being built + up to DDP_MRG_AHEAD built chunks
+#define DDP_MRG_AHEAD 8   // chunks the producers may build ahead of the consumers (if the variant-row ring has room)
 #define DDP_MRG_EPAD 16   // words in front of every E row (variant shifts may be negative)
+// Same wait, for a side that may wait long (the consumers of the merged kernel): the try_wait carries a suspend-time
+// hint, so the warp sleeps in hardware until the phase completes instead of polling shared memory.
+__device__ __forceinline__ void ddp_mbar_wait_long(void* bar, ddp_u32 parity) {
+    ddp_u32 ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(ddp_smem_addr(bar)), "r"(parity), "r"(20000u)
+            : "memory");
+    } while (!ok);
+}
 __device__ __forceinline__ void ddp_mbar_arrive(void* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ddp_smem_addr(bar)) : "memory");
 }
@@ -715,17 +728,21 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     const int NPW = ((int)blockDim.x >> 5) - NCW, NPT = NPW << 5;     // producer warps (4 or 8) / threads
     const int TT = p.threads_t * SPT, TD = p.threads_dm * DPT, H = TT >> 1;
     const int win = p.win, lw = p.lw, le = p.le, RW = p.meta_rw, VCAP = p.vmax, rows_max = p.rows_max;
+    const int PWCAP = 2 * rows_max * lw;  // a chunk needs at most half of it
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it); every region starts 16-byte aligned
-    ddp_u32* pw = (ddp_u32*)ddp_smem;                                        // [2][rows_max][lw]
+    ddp_u32* pw = (ddp_u32*)ddp_smem;                                        // ring of PWCAP words: the variant rows of the built chunks
     ddp_u32* ebuf = pw + (size_t)2 * rows_max * lw;                          // [2][U][le]
     unsigned char* raw = (unsigned char*)(ebuf + (size_t)2 * U * le);        // [2][U][win + 16]
     int* stg = (int*)(raw + (size_t)2 * U * (win + 16));                     // [2][NG * RW] host-table records
     int* ring = stg + (size_t)2 * NG * RW;                                   // [DEPTH][SLOTW]
     const int SLOTW = (16 + 4 * U + 8 * rows_max + TD * NG + 3) & ~3;
-    ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2], pw full[2], pw empty[2]
-    int* sched = (int*)(mbar + 8);                                           // scheduler cursor [8]
-    // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, nblk, 2^20/nblk, ...} | a0[U] | bytes[U] |
+    ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2], rows built [DEPTH], rows consumed [DEPTH]
+    ddp_u64* mfull = mbar + 4;
+    ddp_u64* mempty = mfull + DDP_MRG_DEPTH;
+    int* sched = (int*)(mempty + DDP_MRG_DEPTH);                             // scheduler cursor [8], ring head, extents of the last chunks [2 * AHEAD]
+    // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, -, -, first word in the variant-row ring,
+    //            chunk the consumers must have left before this one is built} | a0[U] | bytes[U] |
     //            carry[U] | nz4[U] | rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
     auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
 
@@ -744,10 +761,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     if (tid == 0) {
 #pragma unroll
         for (int b = 0; b < 4; ++b) ddp_mbar_init(&mbar[b], 1);
-        ddp_mbar_init(&mbar[4], NPW);
-        ddp_mbar_init(&mbar[5], NPW);
-        ddp_mbar_init(&mbar[6], NCW);
-        ddp_mbar_init(&mbar[7], NCW);
+        for (int b = 0; b < DDP_MRG_DEPTH; ++b) {
+            ddp_mbar_init(&mfull[b], NPW);
+            ddp_mbar_init(&mempty[b], NCW);
+        }
         ddp_mbar_fence_init();
         const int tile = unit_lo / nseg, rest = tile / p.n_ttiles;
         sched[0] = unit_lo;
@@ -756,6 +773,8 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
         sched[3] = tile % p.n_ttiles;
         sched[4] = rest % p.n_dtiles;
         sched[5] = rest / p.n_dtiles;
+        sched[8] = 0;  // ring head
+        for (int b = 0; b < 2 * DDP_MRG_AHEAD; ++b) sched[9 + b] = 0;  // empty extents
     }
     for (int i = tid; i < DDP_MRG_DEPTH; i += blockDim.x) slot(i)[5] = 0;  // nothing valid yet
     __syncthreads();
@@ -851,27 +870,46 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                     for (int i = rB; i >= 0 && i < NG * VCAP; i += sB) {
                         const int q = i / VCAP, v = i - q * VCAP;
                         const int* r = rec + q * RW;
-                        int base = 0, total = 0, ymax = 0;
+                        int base = 0, total = 0, words = 0, ymax = 0;  // base: ring words in front of group q (relative to the chunk's first)
 #pragma unroll
                         for (int qq = 0; qq < NG; ++qq) {
                             const int nv = rec[qq * RW];
-                            if (qq < q) base += nv;
+                            const int yl = H + rec[qq * RW + 1] + 1, rl = (yl + 3) & ~3;
+                            if (qq < q) base += nv * rl;
                             total += nv;
-                            const int yl = H + rec[qq * RW + 1] + 1;
+                            words += nv * rl;
                             ymax = yl > ymax ? yl : ymax;
                         }
                         if (i == 0) {
-                            const int nb = (ymax + 127) >> 7;  // 128-word blocks per variant row
+                            // place the chunk's rows in the ring (no row straddles the end) and find the newest earlier chunk
+                            // whose rows they overwrite: the consumers must have left that one (and chunk x - AHEAD)
+                            int head = sched[8];
+                            if (head + words > PWCAP) head = 0;
+                            int waitc = x - DDP_MRG_AHEAD;
+                            for (int b = 1; b < DDP_MRG_AHEAD; ++b) {
+                                const int xo = x - b;
+                                if (xo < 0) break;
+                                const int so = sched[9 + 2 * (xo & (DDP_MRG_AHEAD - 1))], eo = sched[10 + 2 * (xo & (DDP_MRG_AHEAD - 1))];
+                                if (so < head + words && head < eo) { waitc = xo; break; }
+                            }
+                            sched[9 + 2 * (x & (DDP_MRG_AHEAD - 1))] = head;
+                            sched[10 + 2 * (x & (DDP_MRG_AHEAD - 1))] = head + words;
+                            sched[8] = head + words;
                             d[6] = total;
                             d[7] = ymax;
-                            d[9] = nb;
-                            d[10] = ((1 << 20) + nb - 1) / nb;  // item -> row by a multiplication (items < 2^20 / nb)
+                            d[11] = head;
+                            d[12] = waitc;
                         }
                         if (v < r[0]) {
                             const int code = r[4 + 2 * G + v];
-                            int* o = rowd + (size_t)(base + v) * 8;
-                            o[0] = H + r[1] + 1;
-                            o[1] = (base + v) * lw;
+                            const int yl = H + r[1] + 1;
+                            int rows_before = 0;  // row index: rows of the groups in front + v
+#pragma unroll
+                            for (int qq = 0; qq < NG; ++qq)
+                                if (qq < q) rows_before += rec[qq * RW];
+                            int* o = rowd + (size_t)(rows_before + v) * 8;
+                            o[0] = yl;
+                            o[1] = base + v * ((yl + 3) & ~3);
 #pragma unroll
                             for (int m = 0; m < G; ++m) {
                                 const int tau = m == 0 ? 0 : (int)(signed char)((code >> (8 * (m - 1))) & 0xff);
@@ -885,9 +923,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                         int base = 0;
 #pragma unroll
                         for (int qq = 0; qq < NG; ++qq)
-                            if (qq < q) base += rec[qq * RW];
+                            if (qq < q) base += rec[qq * RW] * ((H + rec[qq * RW + 1] + 1 + 3) & ~3);
+                        const int rl = (H + rec[q * RW + 1] + 1 + 3) & ~3;
                         const ddp_u32 code = (ddp_u32)rec[q * RW + 4 + 2 * G + VCAP + j];
-                        offs[i] = (ddp_u32)(((base + (int)(code >> 24)) * lw + (int)(code & 0xffffffu)) * 4);
+                        offs[i] = (ddp_u32)((base + (int)(code >> 24) * rl + (int)(code & 0xffffffu)) * 4);  // relative to the chunk's first word
                     }
                 }
             }
@@ -915,14 +954,17 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 const int* db = slot(xb);
                 const int* ds = slot(xs);
                 const bool vb = xb >= 0 && xb < nstream, vs = xs >= 0 && xs < nstream;
-                if (vb && xb >= 2) ddp_mbar_wait(&mbar[6 + (xb & 1)], (ddp_u32)(((xb >> 1) - 1) & 1));  // consumers left this buffer
+                if (vb && db[12] >= 0) {  // the consumers have left the rows this chunk overwrites
+                    const int wc = db[12];
+                    ddp_mbar_wait(&mempty[wc & (DDP_MRG_DEPTH - 1)], (ddp_u32)((wc / DDP_MRG_DEPTH) & 1));
+                }
                 if (vs) ddp_mbar_wait(&mbar[xs & 1], (ddp_u32)((xs >> 1) & 1));                          // raw windows landed
                 if (pwarp > 0) {
                     const int NB = vb ? 2 * db[6] : 0;       // build items: (variant row, half)
                     const int NI = NB + (vs ? 2 * U : 0);    // expand items: (channel, half)
                     const int* rowd = db + 16 + 4 * U;
                     const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
-                    ddp_u32* pb = pw + (size_t)(xb & 1) * rows_max * lw + lane;
+                    ddp_u32* pb = pw + (vb ? db[11] : 0) + lane;
                     const int* nz4s = ds + 16 + 3 * U;
                     const int hq = H >> 2;
                     const unsigned char* rbase = raw + (size_t)(xs & 1) * U * (win + 16);
@@ -932,7 +974,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                             const int row = it >> 1;
                             const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
                             const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-                            const int half = ((d0.x >> 1) + 127) & ~127;
+                            const int half = ((d0.x >> 1) + 31) & ~31;
                             int y = (it & 1) ? half : 0;
                             const int yend = (it & 1) ? d0.x : (half < d0.x ? half : d0.x);
                             const ddp_u32* e0 = eb + d0.z;
@@ -940,20 +982,19 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                             const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0);
                             const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0);
                             ddp_u32* dst = pb + d0.y;
-                            for (; y + 128 <= yend; y += 128) {  // whole blocks of 128 words: all loads first
-                                ddp_u32 sm[4];
+                            const int yl = yend - lane;  // words of this lane's column before the end
+                            for (; y < yend; y += 256) {  // blocks of 256 words, all loads first; the ragged end is predicated
+                                ddp_u32 sm[8];
 #pragma unroll
-                                for (int i = 0; i < 4; ++i) {
-                                    sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
-                                    if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
+                                for (int i = 0; i < 8; ++i) {
+                                    if (y + 32 * i < yl) {
+                                        sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
+                                        if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
+                                    }
                                 }
 #pragma unroll
-                                for (int i = 0; i < 4; ++i) dst[y + 32 * i] = sm[i];
-                            }
-                            for (; y + lane < yend; y += 32) {
-                                ddp_u32 s0 = e0[y] + e1[y];
-                                if constexpr (G > 2) s0 += e2[y] + e3[y];
-                                dst[y] = s0;
+                                for (int i = 0; i < 8; ++i)
+                                    if (y + 32 * i < yl) dst[y + 32 * i] = sm[i];
                             }
                         } else {
                             const int is = it - NB;
@@ -964,12 +1005,21 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                             const int qend = (is & 1) ? nz : (halfq < nz ? halfq : nz);
                             const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
                             ddp_u32* dst = ebase + (size_t)u * le;
-                            for (; q4 < qend; q4 += 32) {
+                            for (; q4 < qend; q4 += 64) {  // two groups per lane in flight, the second one predicated
+                                const bool two = q4 + 32 < qend;
                                 const ddp_u32 lo = src[q4], hi = src[q4 + hq];
+                                ddp_u32 lo2 = 0u, hi2 = 0u;
+                                if (two) { lo2 = src[q4 + 32]; hi2 = src[q4 + 32 + hq]; }
                                 const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
                                 const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
+                                const ddp_u32 elo2 = lo2 & 0x00ff00ffu, ehi2 = hi2 & 0x00ff00ffu;
+                                const ddp_u32 olo2 = __byte_perm(lo2, 0u, 0x4341u), ohi2 = __byte_perm(hi2, 0u, 0x4341u);
                                 *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
                                                                      __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                                if (two)
+                                    *(uint4*)(dst + 4 * q4 + 128) =
+                                        make_uint4(__byte_perm(elo2, ehi2, 0x5410u), __byte_perm(olo2, ohi2, 0x5410u),
+                                                   __byte_perm(elo2, ehi2, 0x7632u), __byte_perm(olo2, ohi2, 0x7632u));
                             }
                         }
                     }
@@ -977,14 +1027,14 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 }
                 if (vb) {  // this warp's share of buffer (n + 1) & 1 is written
                     __syncwarp();
-                    if (lane == 0) ddp_mbar_arrive(&mbar[4 + (xb & 1)]);
+                    if (lane == 0) ddp_mbar_arrive(&mfull[xb & (DDP_MRG_DEPTH - 1)]);
                 }
             }
             ddp_named_barrier(1, NPT);
         }
     } else {
         // =============================================================================== consumers
-        if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 96;");  // 512 x 96 + 256 x 48 = the 768 x 80 registers the block was launched with
+        if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 88;");  // 512 x 88 + 384 x 48 <= the 896 x 72 registers the block was launched with
         const int tx = tid % p.threads_t, ty = tid / p.threads_t;
         const int wb = (tx >> 5) * (32 * K) + (tx & 31);  // first word of this thread inside the tile
         ddp_u32 acc[DPT][K];
@@ -994,10 +1044,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             for (int k = 0; k < K; ++k) acc[j][k] = 0u;
         for (int n = 0; n < nstream; ++n) {
             const int* d = slot(n);
-            ddp_mbar_wait(&mbar[4 + (n & 1)], (ddp_u32)((n >> 1) & 1));  // variant rows of chunk n are built
+            ddp_mbar_wait_long(&mfull[n & (DDP_MRG_DEPTH - 1)], (ddp_u32)((n / DDP_MRG_DEPTH) & 1));  // variant rows of chunk n are built
             // ---- sum chunk n: every trial adds its variant rows
             const ddp_u32* ob = (const ddp_u32*)(d + 16 + 4 * U + 8 * rows_max) + (size_t)(ty * DPT) * NG;
-            const unsigned char* lanep = (const unsigned char*)(pw + (size_t)(n & 1) * rows_max * lw + wb);
+            const unsigned char* lanep = (const unsigned char*)(pw + d[11] + wb);
 #pragma unroll
             for (int j = 0; j < DPT; ++j) {
                 ddp_u32 o[NG];
@@ -1020,7 +1070,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             }
             const int flags = d[5], tile_t = d[0], tile_dm = d[1], g = d[3];
             __syncwarp();
-            if (lane == 0) ddp_mbar_arrive(&mbar[6 + (n & 1)]);  // this warp has left buffer n & 1
+            if (lane == 0) ddp_mbar_arrive(&mempty[n & (DDP_MRG_DEPTH - 1)]);  // this warp has left the rows of chunk n
             if (flags & 4) {  // block-uniform: last chunk of the unit -> flush
 #pragma unroll
                 for (int j = 0; j < DPT; ++j) {
@@ -1577,6 +1627,197 @@ __device__ __forceinline__ void ddp_snr_body(const DdpSnrParams& p) {
     }
 }
 
+// ------------------------------------------------------------------------------------ fused integration + S/N
+// the dedispersed series is read ONCE; the block sums of every power-of-two width are formed
+// in registers (widths 2..SPT inside a thread, 2*SPT..32*SPT across the lanes of the warp that owns the row,
+// wider ones from the warp totals of consecutive chunks) and fed straight into exact integer moment / max
+// accumulators of their width; the planes are stored only when the caller passes a buffer.  One warp owns
+// a row at a time (blockDim.x == 32, blockDim.y rows per block, DPT rows per warp one after the other), walks it
+// in chunks of 32*SPT samples with the next chunk's loads in flight, and finishes every (row, width) exactly as
+// ddp_snr_body does.  Same integers as integrate followed by snr, hence bit-identical planes and S/N.
+__device__ __forceinline__ void ddp_snr_finish(ddp_u64 s1, ddp_u64 s2, ddp_u32 mx, ddp_u32 ix, int n, int ddof, float& out,
+                                               ddp_u32& am) {
+    // exact: num = n*S2 - S1^2 >= 0 in 128 bits; top = n*max - S1 >= 0
+    const unsigned __int128 num =
+        (unsigned __int128)s2 * (unsigned __int128)(ddp_u64)n - (unsigned __int128)s1 * (unsigned __int128)s1;
+    out = 0.0f;
+    am = 0u;
+    if (num != 0) {
+        const double numd = (double)(ddp_u64)(num >> 64) * 18446744073709551616.0 + (double)(ddp_u64)num;
+        const double top = (double)((ddp_u64)n * (ddp_u64)mx - s1) / (double)n;
+        const double var = numd / ((double)n * (double)(n - ddof));
+        out = (float)(top / sqrt(var));
+        am = ix;
+    }
+}
+// N block sums v[0..N) of one level with series indices idx0.. (only those below len count)
+template <int N>
+__device__ __forceinline__ void ddp_mom_add_run(DdpMoments& m, const ddp_u32 (&v)[N], int idx0, int len) {
+    ddp_u32 cm = 0u;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const ddp_u32 x = idx0 + i < len ? v[i] : 0u;
+        m.s1 += x;
+        m.s2 += (ddp_u64)x * (ddp_u64)x;
+        cm = x > cm ? x : cm;
+    }
+    if (cm > m.mx) {  // strict: a thread visits its indices in increasing order
+        m.mx = cm;
+#pragma unroll
+        for (int i = N - 1; i >= 0; --i)
+            if (v[i] == cm && idx0 + i < len) m.ix = (ddp_u32)(idx0 + i);
+    }
+}
+template <int SPT, int M, int LVLS>
+struct DdpIsnrFold {  // levels M .. log2(SPT) inside one thread; x holds SPT >> (M-1) partial sums on entry
+    template <int NIN>
+    static __device__ __forceinline__ void run(const DdpIsnrParams& p, DdpMoments (&mom)[LVLS], const ddp_u32 (&x)[NIN], int t0,
+                                               int dm, ddp_u32& total) {
+        if constexpr (NIN == 1) {
+            total = x[0];
+        } else {
+            ddp_u32 y[NIN / 2];
+#pragma unroll
+            for (int i = 0; i < NIN / 2; ++i) y[i] = x[2 * i] + x[2 * i + 1];
+            const int k = p.lvl_k[M];
+            if (k >= 0) {
+                ddp_mom_add_run<NIN / 2>(mom[M], y, t0 >> M, p.n[k]);
+                if (p.planes) ddp_store_run<NIN / 2>(p.planes + p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k], t0 >> M, p.n[k], y);
+            }
+            DdpIsnrFold<SPT, M + 1, LVLS>::template run<NIN / 2>(p, mom, y, t0, dm, total);
+        }
+    }
+};
+
+template <int SPT, int DPT>
+__device__ __forceinline__ void ddp_isnr_body(const DdpIsnrParams& p) {
+    extern __shared__ __align__(128) unsigned char ddp_smem[];
+    constexpr int LS = SPT == 16 ? 4 : SPT == 8 ? 3 : 2;  // log2(SPT), SPT in {4, 8, 16}
+    constexpr int NL = LS + 6;                            // levels kept in registers: widths 1 .. 32*SPT
+    constexpr int CH = 32 * SPT;                          // samples per chunk
+    constexpr int NWL = 8;                                // wider levels (widths 64*SPT .. 8192*SPT): lane 0, shared memory
+    const int lane = threadIdx.x, ty = threadIdx.y;
+    // per warp: running sums and moments of the wide levels
+    ddp_u32* wrun = (ddp_u32*)ddp_smem + (size_t)ty * NWL * 8;  // [NWL][8]: run, s1 lo/hi, s2 lo/hi, mx, ix, -
+    const int ns4 = (p.ns + 3) & ~3;  // rows are readable up to here (out_stride is a multiple of 4)
+    const int nchunks = (p.ns + CH - 1) / CH;
+    const bool wide = p.max_lvl >= NL;
+
+#pragma unroll 1
+    for (int j = 0; j < DPT; ++j) {
+        const int dm = (blockIdx.x * blockDim.y + ty) * DPT + j;
+        if (dm >= p.ndm) break;  // warp-uniform
+        const ddp_u32* row = p.in + (ddp_i64)dm * p.in_stride;
+        DdpMoments mom[NL];
+#pragma unroll
+        for (int m = 0; m < NL; ++m) { mom[m].s1 = 0; mom[m].s2 = 0; mom[m].mx = 0; mom[m].ix = 0xffffffffu; }
+        if (wide && lane < NWL) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) wrun[lane * 8 + i] = i == 6 ? 0xffffffffu : 0u;
+        }
+        __syncwarp();
+        auto load = [&](int c, ddp_u32 (&x)[SPT]) {
+            const int t0 = c * CH + lane * SPT;
+#pragma unroll
+            for (int v = 0; v < SPT / 4; ++v) {
+                const int t = t0 + 4 * v;
+                uint4 r = make_uint4(0u, 0u, 0u, 0u);
+                if (t + 4 <= ns4) r = __ldg((const uint4*)(row + t));
+                x[4 * v] = t < p.ns ? r.x : 0u;
+                x[4 * v + 1] = t + 1 < p.ns ? r.y : 0u;
+                x[4 * v + 2] = t + 2 < p.ns ? r.z : 0u;
+                x[4 * v + 3] = t + 3 < p.ns ? r.w : 0u;
+            }
+        };
+        ddp_u32 xn[SPT];
+        load(0, xn);
+        for (int c = 0; c < nchunks; ++c) {
+            ddp_u32 x[SPT];
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) x[s] = xn[s];
+            if (c + 1 < nchunks) load(c + 1, xn);
+            const int t0 = c * CH + lane * SPT;
+            if (p.lvl_k[0] >= 0) ddp_mom_add_run<SPT>(mom[0], x, t0, p.ns);
+            ddp_u32 v;
+            DdpIsnrFold<SPT, 1, NL>::template run<SPT>(p, mom, x, t0, dm, v);
+            // widths 2*SPT .. 32*SPT across the lanes
+#pragma unroll
+            for (int l = 1; l <= 5; ++l) {
+                v += __shfl_xor_sync(0xffffffffu, v, 1 << (l - 1));
+                const int m = LS + l;
+                const int k = p.lvl_k[m];
+                if (k >= 0 && (lane & ((1 << l) - 1)) == 0) {
+                    const int idx = t0 >> m;
+                    if (idx < p.n[k]) {
+                        mom[m].s1 += v;
+                        mom[m].s2 += (ddp_u64)v * (ddp_u64)v;
+                        if (v > mom[m].mx) { mom[m].mx = v; mom[m].ix = (ddp_u32)idx; }
+                        if (p.planes) p.planes[p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + idx] = v;
+                    }
+                }
+            }
+            // wider widths: lane 0 adds the chunk total to the running sum of every wide level; a level's block
+            // is complete when the chunk count reaches a multiple of its length in chunks
+            if (wide && lane == 0) {
+                for (int l = 1; LS + 5 + l <= p.max_lvl && l <= NWL; ++l) {
+                    ddp_u32* a = wrun + (l - 1) * 8;
+                    const ddp_u32 run = a[0] + v;
+                    if (((c + 1) & ((1 << l) - 1)) == 0) {
+                        a[0] = 0u;
+                        const int m = LS + 5 + l, k = p.lvl_k[m], idx = c >> l;
+                        if (k >= 0 && idx < p.n[k]) {
+                            ddp_u64 s1 = ((ddp_u64)a[2] << 32) | a[1], s2 = ((ddp_u64)a[4] << 32) | a[3];
+                            s1 += run;
+                            s2 += (ddp_u64)run * (ddp_u64)run;
+                            a[1] = (ddp_u32)s1; a[2] = (ddp_u32)(s1 >> 32);
+                            a[3] = (ddp_u32)s2; a[4] = (ddp_u32)(s2 >> 32);
+                            if (run > a[5]) { a[5] = run; a[6] = (ddp_u32)idx; }
+                            if (p.planes) p.planes[p.plane_off[k] + (ddp_i64)dm * p.plane_stride[k] + idx] = run;
+                        }
+                    } else {
+                        a[0] = run;
+                    }
+                }
+            }
+        }
+        // finish: warp tree per requested level (lowest index wins ties), lane 0 writes
+#pragma unroll
+        for (int m = 0; m < NL; ++m) {
+            const int k = p.lvl_k[m];
+            if (k < 0) continue;  // uniform
+            DdpMoments a = mom[m];
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) {
+                const ddp_u64 s1 = __shfl_down_sync(0xffffffffu, a.s1, d);
+                const ddp_u64 s2 = __shfl_down_sync(0xffffffffu, a.s2, d);
+                const ddp_u32 mx = __shfl_down_sync(0xffffffffu, a.mx, d);
+                const ddp_u32 ix = __shfl_down_sync(0xffffffffu, a.ix, d);
+                if (lane + d < 32) ddp_mom_merge(a, s1, s2, mx, ix);
+            }
+            if (lane == 0) {
+                float out;
+                ddp_u32 am;
+                ddp_snr_finish(a.s1, a.s2, a.mx, a.ix, p.n[k], p.ddof, out, am);
+                p.snr[(ddp_i64)dm * p.nwidths + k] = out;
+                if (p.argmax) p.argmax[(ddp_i64)dm * p.nwidths + k] = am;
+            }
+        }
+        if (wide && lane == 0) {
+            for (int l = 1; LS + 5 + l <= p.max_lvl && l <= NWL; ++l) {
+                const int k = p.lvl_k[LS + 5 + l];
+                if (k < 0) continue;
+                const ddp_u32* a = wrun + (l - 1) * 8;
+                float out;
+                ddp_u32 am;
+                ddp_snr_finish(((ddp_u64)a[2] << 32) | a[1], ((ddp_u64)a[4] << 32) | a[3], a[5], a[6], p.n[k], p.ddof, out, am);
+                p.snr[(ddp_i64)dm * p.nwidths + k] = out;
+                if (p.argmax) p.argmax[(ddp_i64)dm * p.nwidths + k] = am;
+            }
+        }
+        __syncwarp();
+    }
+}
+
 // ------------------------------------------------------------------------------------ entry points
 // uint8 / uint16 input with staging takes the packed kernels; everything else the generic one.
 // FLAGS: bit 0 WIDE (uint8 packed: reduction longer than 256 rows), bit 1 OUT16 (uint16 result: the
@@ -1606,6 +1847,11 @@ __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
 #define DDP_DEFINE_SNR(NAME, SPT, DPT, UNROLL, STAGING, VEC, MAXT)                                  \
     extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpSnrParams p) {                    \
         ddp_snr_body<SPT, DPT, UNROLL, STAGING, VEC>(p);                                               \
+    }
+
+#define DDP_DEFINE_ISNR(NAME, SPT, DPT, MAXT)                                                       \
+    extern "C" __global__ void __launch_bounds__(MAXT) NAME(const DdpIsnrParams p) {                   \
+        ddp_isnr_body<SPT, DPT>(p);                                                                    \
     }
 
 #endif  // DDP_KERNELS_CUH_

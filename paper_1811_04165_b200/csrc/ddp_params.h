@@ -69,4 +69,22 @@ struct DdpSnrParams {
     int ddof;
 };
 
+// Fused integration + S/N: level m = width 2^m; k = index of that width in the plan's width list.
+struct DdpIsnrParams {
+    const unsigned int* in;      // dedispersed series uint32 [ndm][in_stride]
+    unsigned int* planes;        // base of the integration planes, or null: planes are not written
+    long long in_stride;
+    long long plane_off[DDP_MAXW];     // by width index k (w > 1)
+    long long plane_stride[DDP_MAXW];
+    int n[DDP_MAXW];             // values of series k: floor(ns / w)
+    int lvl_k[DDP_MAXW];         // level m -> width index k, -1 if width 2^m is not requested
+    float* snr;                  // [ndm][nwidths]
+    unsigned int* argmax;        // [ndm][nwidths] or null
+    int nwidths;
+    int ndm;
+    int ns;
+    int ddof;
+    int max_lvl;                 // log2 of the largest width
+};
+
 #endif  // DDP_PARAMS_H_

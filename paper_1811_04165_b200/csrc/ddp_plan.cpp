@@ -239,7 +239,8 @@ bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k) {
         case DDP_K_SUB1:
         case DDP_K_SUB2: return p->subband;
         case DDP_K_INTEGRATE:
-        case DDP_K_SNR: return true;
+        case DDP_K_SNR:
+        case DDP_K_ISNR: return true;
         default: return false;
     }
 }
@@ -458,8 +459,8 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += 2 * U * (size_t)mg.le * 4;                       // ebuf
                 b += 2 * U * (row + 16);                              // raw
                 b += 2 * NG * (size_t)mg.rw * 4;                      // record staging
-                b += 8 * (((16 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
-                b += 8 * 8 + 32;                                      // mbarriers, scheduler cursor
+                b += 16 * (((16 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
+                b += (4 + 2 * 16) * 8 + 128;                          // mbarriers, scheduler state
                 return b;
             }
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
@@ -485,6 +486,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (c.staging != 0) b += (size_t)c.threads_dm * TT * 4 + 16;
             return b;
         }
+        case DDP_K_ISNR: return (size_t)c.threads_dm * 8 * 8 * 4;  // wide-level accumulators [threads_dm][8][8]
         case DDP_K_SNR: {
             size_t b = (size_t)c.threads_dm * 32 * 24;
             if (c.staging != 0) b += (size_t)c.threads_dm * (c.staging == 2 ? 2 : 1) * TT * 4 + (size_t)c.threads_dm * 16;
@@ -518,6 +520,16 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
     const int64_t threads = (int64_t)c.threads_t * c.threads_dm;
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    if (k == DDP_K_ISNR) {  // fused integration + S/N: one warp per series, everything else pinned (V7)
+        if (c.threads_t != 32) return no("V1: the fused kernel gives one warp to a series: threads_t must be 32");
+        if (c.samples_per_thread < 4) return no("V5: the fused kernel loads 16-byte vectors: samples_per_thread >= 4");
+        if (c.unroll != 1 || c.staging != 0 || c.vec_bytes != 16) return no("V7: the fused kernel pins unroll = 1, staging = 0, vec_bytes = 16");
+        if ((int64_t)c.threads_dm * c.dms_per_thread > pow2ceil(p->ndm)) return no("V3: DM tile larger than the problem");
+        int maxw = 1;
+        for (int i = 0; i < p->nwidths; ++i) maxw = std::max(maxw, p->widths[i]);
+        if (maxw > 32 * c.samples_per_thread * 256) return no("V3: a width is longer than 256 chunks of the fused kernel");
+        return true;
+    }
     // V7: a gene the kernel does not read is pinned (snr reads `unroll` only with direct loads)
     if (k == DDP_K_SNR && c.staging != 0 && c.unroll != 1) return no("V7: snr ignores unroll when staged; must be 1");
     // merged staging (genes 3, 4) exists for the uint8 dedispersion kernels only; its groups are whole
@@ -669,6 +681,7 @@ static void default_kcfgs(ddp_plan* p) {
         /* sub2      */ {128, 2, 4, 8, 8, 2, 16},
         /* integrate */ {256, 1, 4, 1, 1, 0, 16},
         /* snr       */ {256, 1, 4, 1, 4, 0, 16},
+        /* isnr      */ {32, 8, 16, 1, 1, 0, 16},
     };
     for (int k = 0; k < DDP_K_COUNT; ++k) {
         p->kcfg[k] = pref[k];

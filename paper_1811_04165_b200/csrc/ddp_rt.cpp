@@ -64,6 +64,10 @@ struct Api {
     DRV(cuStreamSynchronize)
     DRV(cuGetErrorString)
     DRV(cuOccupancyMaxActiveBlocksPerMultiprocessor)
+    DRV(cuMemcpy2DAsync)
+    DRV(cuStreamCreate)
+    DRV(cuStreamDestroy)
+    DRV(cuStreamWaitEvent)
 #undef DRV
 #define RTC(name) decltype(&name) p_##name = nullptr;
     RTC(nvrtcCreateProgram)
@@ -146,6 +150,10 @@ bool load_cuda_locked() {
     DRV(cuStreamSynchronize)
     DRV(cuGetErrorString)
     DRV(cuOccupancyMaxActiveBlocksPerMultiprocessor)
+    DRV(cuMemcpy2DAsync)
+    DRV(cuStreamCreate)
+    DRV(cuStreamDestroy)
+    DRV(cuStreamWaitEvent)
 #undef DRV
     if (!ok) {
         g_api.why = "libcuda.so.1 lacks a required driver entry point";
@@ -218,19 +226,20 @@ std::mutex g_load_mu;  // serialises module loads and the per-device AOT initial
 CUmodule g_aot_mod[DDP_MAX_DEVICES] = {nullptr};
 bool g_aot_tried[DDP_MAX_DEVICES] = {false};
 
-enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3, CK_DEDISP_U16 = 4 };
+enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3, CK_DEDISP_U16 = 4, CK_ISNR = 5 };
 CodeKind code_kind(const ddp_plan* p, ddp_kernel k) {
     switch (k) {
         case DDP_K_DIRECT:
         case DDP_K_SUB1: return CK_DEDISP_U8;
         case DDP_K_SUB2: return p->info.sub_elem_bytes == 2 ? CK_DEDISP_U16 : CK_DEDISP_U32;
         case DDP_K_INTEGRATE: return CK_INTEG;
+        case DDP_K_ISNR: return CK_ISNR;
         default: return CK_SNR;
     }
 }
 bool is_dedisp(CodeKind ck) { return ck == CK_DEDISP_U8 || ck == CK_DEDISP_U32 || ck == CK_DEDISP_U16; }
 const char* kind_tag(CodeKind ck) {
-    static const char* t[] = {"ddp_dedisp_u8", "ddp_dedisp_u32", "ddp_integ", "ddp_snr", "ddp_dedisp_u16"};
+    static const char* t[] = {"ddp_dedisp_u8", "ddp_dedisp_u32", "ddp_integ", "ddp_snr", "ddp_dedisp_u16", "ddp_isnr"};
     return t[ck];
 }
 const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck == CK_DEDISP_U16 ? "ddp_u16" : "ddp_u32"); }
@@ -268,6 +277,8 @@ std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     if (is_dedisp(ck))
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(ck), c.samples_per_thread,
                       c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt_bucket(c), code_flags(p, k, c));
+    else if (ck == CK_ISNR)
+        std::snprintf(b, sizeof b, "%s_s%d_d%d_t%d", kind_tag(ck), c.samples_per_thread, c.dms_per_thread, maxt_bucket(c));
     else  // integrate reads `unroll` at run time (tiles per block): not part of its code shape
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(ck), c.samples_per_thread,
                       c.dms_per_thread, ck == CK_INTEG ? 1 : c.unroll, c.staging, c.vec_bytes, maxt_bucket(c));
@@ -283,6 +294,9 @@ std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, cons
         case CK_DEDISP_U32:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_DEDISP(%s, %s, %d, %d, %d, %d, %d, %d, %d)\n", name.c_str(), kind_type(ck),
                           c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt, code_flags(p, k, c));
+            break;
+        case CK_ISNR:
+            std::snprintf(b, sizeof b, "\nDDP_DEFINE_ISNR(%s, %d, %d, %d)\n", name.c_str(), c.samples_per_thread, c.dms_per_thread, maxt);
             break;
         case CK_INTEG:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_INTEG(%s, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
@@ -565,6 +579,8 @@ void ddp_rt_precompile(const ddp_plan* p, const std::vector<std::pair<ddp_kernel
 namespace {
 struct PlanRt {
     std::vector<CUevent> ev;  // event pool of the timing harness
+    CUstream copy_stream = nullptr;  // ddp_search_host_batches: uploads run beside the compute stream
+    CUevent ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
 };
 PlanRt* rt_of(ddp_plan* p) {
     if (!p->rt) p->rt = new PlanRt();
@@ -578,6 +594,13 @@ void ddp_rt_release(ddp_plan* p) {
     PlanRt* R = (PlanRt*)p->rt;
     if (g_api.ok)
         for (CUevent e : R->ev) g_api.p_cuEventDestroy(e);
+    if (g_api.ok) {
+        for (int b = 0; b < 2; ++b) {
+            if (R->ev_in[b]) g_api.p_cuEventDestroy(R->ev_in[b]);
+            if (R->ev_done[b]) g_api.p_cuEventDestroy(R->ev_done[b]);
+        }
+        if (R->copy_stream) g_api.p_cuStreamDestroy(R->copy_stream);
+    }
     delete R;
     p->rt = nullptr;
 }
@@ -845,12 +868,42 @@ ddp_status launch_snr(const ddp_plan* p, const ddp_kcfg& c, DdpCompiled* K, cons
                   ddp_smem_bytes(p, DDP_K_SNR, c), io.stream, &q);
 }
 
+// Fused integration + S/N (ddp_isnr_body): level m = width 2^m; planes only when io.d_integ is given.
+ddp_status launch_isnr(const ddp_plan* p, const ddp_kcfg& c, DdpCompiled* K, const IoView& io) {
+    DdpIsnrParams q;
+    std::memset(&q, 0, sizeof q);
+    const ddp_plan_info& I = p->info;
+    q.in = io.d_out;
+    q.planes = io.d_integ;
+    q.in_stride = (long long)io.out_stride;
+    for (int m = 0; m < DDP_MAXW; ++m) q.lvl_k[m] = -1;
+    for (int k = 0; k < p->nwidths; ++k) {
+        int m = 0;
+        while ((1 << m) < p->widths[k]) ++m;
+        if (m >= DDP_MAXW) return ddp_fail(p, DDP_E_CONFIG, "fused kernel: width too large");
+        q.lvl_k[m] = k;
+        if (m > q.max_lvl) q.max_lvl = m;
+        q.n[k] = (int)I.plane_len[k];
+        q.plane_off[k] = p->widths[k] == 1 ? 0 : I.plane_offset[k];
+        q.plane_stride[k] = p->widths[k] == 1 ? 0 : I.plane_stride[k];
+    }
+    q.snr = io.d_snr;
+    q.argmax = io.d_argmax;
+    q.nwidths = p->nwidths;
+    q.ndm = p->ndm;
+    q.ns = p->ns;
+    q.ddof = p->ddof;
+    const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    return launch(p, K, cdiv(p->ndm, TD), 1, 1, 32u, (unsigned)c.threads_dm, ddp_smem_bytes(p, DDP_K_ISNR, c), io.stream, &q);
+}
+
 ddp_status launch_kernel(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, DdpCompiled* K, const IoView& io) {
     switch (k) {
         case DDP_K_DIRECT:
         case DDP_K_SUB1:
         case DDP_K_SUB2: return launch_dedisp(p, k, c, K, io);
         case DDP_K_INTEGRATE: return launch_integ(p, c, K, io);
+        case DDP_K_ISNR: return launch_isnr(p, c, K, io);
         default: return launch_snr(p, c, K, io);
     }
 }
@@ -917,6 +970,21 @@ extern "C" ddp_status ddp_snr(ddp_plan* plan, const uint32_t* d_dedisp, size_t s
     return launch_snr(plan, plan->kcfg[DDP_K_SNR], K, io);
 }
 
+extern "C" ddp_status ddp_integrate_snr(ddp_plan* plan, const uint32_t* d_dedisp, size_t stride, uint32_t* d_integ,
+                                        float* d_snr, uint32_t* d_argmax, void* stream) {
+    if (!plan) return DDP_E_ARG;
+    ddp_status s = ensure_ctx(plan, plan->device);
+    if (s != DDP_OK) return s;
+    if (!d_dedisp || !d_snr) return ddp_fail(plan, DDP_E_ARG, "NULL device pointer");
+    if ((int64_t)stride < plan->info.out_stride_min || stride % 4 != 0 || ((uintptr_t)d_dedisp & 15u) ||
+        ((uintptr_t)d_integ & 15u))
+        return ddp_fail(plan, DDP_E_SHAPE, "stride < out_stride_min, not a multiple of 4, or misaligned pointer");
+    IoView io{nullptr, 0, (uint32_t*)d_dedisp, stride, d_integ, d_snr, d_argmax, (CUstream)stream};
+    DdpCompiled* K = nullptr;
+    if ((s = active_kernel(plan, DDP_K_ISNR, &K)) != DDP_OK) return s;
+    return launch_isnr(plan, plan->kcfg[DDP_K_ISNR], K, io);
+}
+
 // One whole search through HOST buffers: H2D of the filterbank, dedisperse -> integrate -> snr, D2H of
 // the S/N table (and argmax), stream synchronised before returning.
 extern "C" ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_t in_stride, uint8_t* d_in,
@@ -931,13 +999,89 @@ extern "C" ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_
     CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)d_in, h_in, in_stride * (size_t)plan->nchan, st);
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "H2D copy: " + cu_err(r));
     if ((s = ddp_dedisperse(plan, d_in, in_stride, d_out, out_stride, stream)) != DDP_OK) return s;
-    if ((s = ddp_integrate(plan, d_out, out_stride, d_integ, stream)) != DDP_OK) return s;
-    if ((s = ddp_snr(plan, d_out, out_stride, d_integ, d_snr, d_argmax, stream)) != DDP_OK) return s;
+    if (d_integ) {
+        if ((s = ddp_integrate(plan, d_out, out_stride, d_integ, stream)) != DDP_OK) return s;
+        if ((s = ddp_snr(plan, d_out, out_stride, d_integ, d_snr, d_argmax, stream)) != DDP_OK) return s;
+    } else if ((s = ddp_integrate_snr(plan, d_out, out_stride, nullptr, d_snr, d_argmax, stream)) != DDP_OK) {
+        return s;
+    }
     const size_t n = (size_t)plan->ndm * plan->nwidths;
     r = g_api.p_cuMemcpyDtoHAsync(h_snr, (CUdeviceptr)d_snr, n * sizeof(float), st);
     if (r == CUDA_SUCCESS && h_argmax) r = g_api.p_cuMemcpyDtoHAsync(h_argmax, (CUdeviceptr)d_argmax, n * 4, st);
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "D2H copy: " + cu_err(r));
     r = g_api.p_cuStreamSynchronize(st);
+    if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "stream synchronize: " + cu_err(r));
+    return DDP_OK;
+}
+
+// Consecutive batches of one observation ("10 batches").  Batch b searches the samples
+// [b*ns, b*ns + ns + max_delay) of every channel.  Only the ns NEW samples of a batch cross the bus: the max_delay
+// samples it shares with the previous batch are carried over on the device (copy from the other input buffer), and
+// the upload of batch b+1 runs on a second stream while batch b is searched.
+extern "C" ddp_status ddp_search_host_batches(ddp_plan* plan, const uint8_t* h_in, size_t h_stride, int nbatches,
+                                              uint8_t* d_in0, uint8_t* d_in1, size_t in_stride, uint32_t* d_out,
+                                              size_t out_stride, float* d_snr, uint32_t* d_argmax, float* h_snr,
+                                              uint32_t* h_argmax, void* stream) {
+    if (!plan) return DDP_E_ARG;
+    if (!h_in || !h_snr || !d_in0 || !d_in1 || !d_out || !d_snr || nbatches < 1) return ddp_fail(plan, DDP_E_ARG, "NULL pointer or no batch");
+    if (h_argmax && !d_argmax) return ddp_fail(plan, DDP_E_ARG, "h_argmax given without d_argmax");
+    ddp_status s = ensure_ctx(plan, plan->device);
+    if (s != DDP_OK) return s;
+    const ddp_plan_info& I = plan->info;
+    const size_t ns = (size_t)plan->ns, carry = (size_t)I.max_delay;
+    if (h_stride < (size_t)nbatches * ns + carry) return ddp_fail(plan, DDP_E_SHAPE, "h_stride shorter than nbatches * nsamp_out + max_delay");
+    if ((s = check_io_dedisp(plan, d_in0, in_stride, d_out, out_stride)) != DDP_OK) return s;
+    if ((uintptr_t)d_in1 & 15u) return ddp_fail(plan, DDP_E_SHAPE, "d_in1 misaligned");
+    PlanRt* R = rt_of(plan);
+    if (!R->copy_stream) {
+        CUresult r = g_api.p_cuStreamCreate(&R->copy_stream, CU_STREAM_NON_BLOCKING);
+        for (int b = 0; b < 2 && r == CUDA_SUCCESS; ++b) {
+            r = g_api.p_cuEventCreate(&R->ev_in[b], CU_EVENT_DISABLE_TIMING);
+            if (r == CUDA_SUCCESS) r = g_api.p_cuEventCreate(&R->ev_done[b], CU_EVENT_DISABLE_TIMING);
+        }
+        if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "copy stream / events: " + cu_err(r));
+    }
+    CUstream st = (CUstream)stream, cs = R->copy_stream;
+    uint8_t* d_in[2] = {d_in0, d_in1};
+    const size_t n = (size_t)plan->ndm * plan->nwidths;
+    auto copy2d = [&](bool from_host, const void* src, size_t spitch, uint8_t* dst, size_t width) -> CUresult {
+        CUDA_MEMCPY2D c;
+        std::memset(&c, 0, sizeof c);
+        if (from_host) { c.srcMemoryType = CU_MEMORYTYPE_HOST; c.srcHost = src; }
+        else { c.srcMemoryType = CU_MEMORYTYPE_DEVICE; c.srcDevice = (CUdeviceptr)src; }
+        c.srcPitch = spitch;
+        c.dstMemoryType = CU_MEMORYTYPE_DEVICE;
+        c.dstDevice = (CUdeviceptr)dst;
+        c.dstPitch = in_stride;
+        c.WidthInBytes = width;
+        c.Height = (size_t)plan->nchan;
+        return g_api.p_cuMemcpy2DAsync(&c, cs);
+    };
+    // the caller's earlier work on `stream` (e.g. the previous use of the buffers) comes first
+    CUresult r = g_api.p_cuEventRecord(R->ev_done[1], st);
+    if (r == CUDA_SUCCESS) r = g_api.p_cuStreamWaitEvent(cs, R->ev_done[1], 0);
+    for (int b = 0; b < nbatches && r == CUDA_SUCCESS; ++b) {
+        uint8_t* cur = d_in[b & 1];
+        if (b >= 2) r = g_api.p_cuStreamWaitEvent(cs, R->ev_done[b & 1], 0);  // the search of batch b - 2 has left this buffer
+        if (r != CUDA_SUCCESS) break;
+        if (b == 0) {
+            r = copy2d(true, h_in, h_stride, cur, ns + carry);
+        } else {  // carried samples from the other buffer (device to device), then the new ones
+            if (carry) r = copy2d(false, d_in[(b - 1) & 1] + ns, in_stride, cur, carry);
+            if (r == CUDA_SUCCESS) r = copy2d(true, h_in + (size_t)b * ns + carry, h_stride, cur + carry, ns);
+        }
+        if (r == CUDA_SUCCESS) r = g_api.p_cuEventRecord(R->ev_in[b & 1], cs);
+        if (r == CUDA_SUCCESS) r = g_api.p_cuStreamWaitEvent(st, R->ev_in[b & 1], 0);
+        if (r != CUDA_SUCCESS) break;
+        if ((s = ddp_dedisperse(plan, cur, in_stride, d_out, out_stride, stream)) != DDP_OK) return s;
+        if ((s = ddp_integrate_snr(plan, d_out, out_stride, nullptr, d_snr, d_argmax, stream)) != DDP_OK) return s;
+        r = g_api.p_cuMemcpyDtoHAsync(h_snr + (size_t)b * n, (CUdeviceptr)d_snr, n * sizeof(float), st);
+        if (r == CUDA_SUCCESS && h_argmax) r = g_api.p_cuMemcpyDtoHAsync(h_argmax + (size_t)b * n, (CUdeviceptr)d_argmax, n * 4, st);
+        if (r == CUDA_SUCCESS) r = g_api.p_cuEventRecord(R->ev_done[b & 1], st);
+    }
+    if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "batched search: " + cu_err(r));
+    r = g_api.p_cuStreamSynchronize(st);
+    if (r == CUDA_SUCCESS) r = g_api.p_cuStreamSynchronize(cs);
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "stream synchronize: " + cu_err(r));
     return DDP_OK;
 }

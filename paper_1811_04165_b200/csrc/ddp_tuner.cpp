@@ -133,6 +133,17 @@ struct Run {
         }
         ddp_rt_precompile(p, list);
     }
+    // the configurations a run ends with (GA: last population, ranked; random: its last draws)
+    void record_final(const std::vector<Chrom>& v) {
+        res->final_len = 0;
+        if (!res->final_pop || res->final_cap == 0) return;
+        for (const Chrom& c : v) {
+            if (res->final_len >= res->final_cap) break;
+            for (int s = 0; s < DDP_NSLOTS; ++s) res->final_pop[res->final_len * DDP_NSLOTS + s] = c.k[s];
+            if (res->final_fit) res->final_fit[res->final_len] = c.fit;
+            ++res->final_len;
+        }
+    }
     ddp_status finish() {
         res->n_compiles = ddp_rt_compile_count() - compiles0;
         res->wall_seconds = now_s() - t0;
@@ -270,6 +281,8 @@ extern "C" ddp_status ddp_tune_ga(ddp_plan* plan, const ddp_tune_io* io, const d
         for (int i = 0; (int)next.size() < N; ++i) next.push_back(pop[i]);  // budget ran out mid-generation
         pop.swap(next);
     }
+    rank(pop);
+    R.record_final(pop);
     return R.finish();
 }
 
@@ -280,6 +293,7 @@ extern "C" ddp_status ddp_tune_random(ddp_plan* plan, const ddp_tune_io* io, con
     Run R(plan, io, res, rp->max_evals);
     Rng rng(rp->seed);
     int64_t stale = 0;  // consecutive draws that were already seen (tiny spaces)
+    std::vector<Chrom> last;  // the newest evaluated draws, newest last
     while (R.budget_left() && stale < 100000) {
         const int64_t room = rp->max_evals - res->n_fitness_calls;
         std::vector<Chrom> batch((size_t)std::min<int64_t>(64, room));
@@ -290,8 +304,13 @@ extern "C" ddp_status ddp_tune_random(ddp_plan* plan, const ddp_tune_io* io, con
             const int64_t before = res->n_fitness_calls;
             R.eval(c);
             stale = res->n_fitness_calls == before ? stale + 1 : 0;
+            if (res->n_fitness_calls != before && res->final_pop && res->final_cap) {
+                if (last.size() == res->final_cap) last.erase(last.begin());
+                last.push_back(c);
+            }
         }
     }
+    R.record_final(last);
     return R.finish();
 }
 

@@ -161,6 +161,53 @@ def test_search_host_end_to_end_call(subband):
     h_snr2 = np.full((i.ndm, i.nwidths), -3.0, dtype=np.float32)
     g.plan.search_host(g.X, g.buf["d_in"], g.buf["d_out"], g.buf["d_integ"], g.buf["d_snr"], None, h_snr2, None)
     assert_snr_close(h_snr2, So, "search_host pageable, no argmax")
+    # no plane buffer: dedisperse -> fused integrate + S/N (ddp_integrate_snr), same table
+    h_snr3 = np.full((i.ndm, i.nwidths), -3.0, dtype=np.float32)
+    h_arg3 = np.full((i.ndm, i.nwidths), -1, dtype=np.int32)
+    g.plan.search_host(g.X, g.buf["d_in"], g.buf["d_out"], None, g.buf["d_snr"], g.buf["d_argmax"], h_snr3, h_arg3)
+    assert_snr_close(h_snr3, So, "search_host without planes")
+    assert np.array_equal(h_arg3.view(np.uint32), Ao)
+    g.close()
+
+
+@pytest.mark.parametrize("subband", [False, True])
+def test_search_host_batches_equal_one_long_dedispersion(subband):
+    """ddp_search_host_batches (8(f) f3): three consecutive batches, only the new samples uploaded, the
+    shared max_delay samples carried on the device, uploads overlapped on a second stream -- every batch's S/N table
+    equals the oracle's search of the matching columns of ONE long dedispersion of the whole observation."""
+    import oracle
+    from synth import filterbank
+    cfg = small_subband(nsamp_out=1900) if subband else small_direct(name="batches", nchan=40, nsamp_out=2304, ndm=19)
+    g = GpuSearch(cfg)
+    i = g.info
+    nb, ns, md = 3, cfg.nsamp_out, i.max_delay
+    nlong = nb * ns + md
+    X, _ = filterbank.make_filterbank(cfg, nlong, (nlong + 47) // 16 * 16)
+    if subband:
+        sb = cfg.subband
+        A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+        F = sb.fine_step * np.arange(sb.n_fine)
+        d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F)
+        S = oracle.subband_step1(X, d1, sb.n_subbands, nb * ns + int(d2.max()))
+        Ylong = oracle.subband_step2(S, d2, nb * ns)
+    else:
+        Ylong = oracle.dedisperse(X, oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s), nb * ns)
+    d_in1 = torch.empty_like(g.buf["d_in"])
+    g.buf["d_in"].zero_()
+    d_in1.zero_()
+    h_in = torch.from_numpy(X).pin_memory()
+    h_snr = torch.full((nb, i.ndm, i.nwidths), -3.0, dtype=torch.float32).pin_memory()
+    h_arg = torch.full((nb, i.ndm, i.nwidths), -1, dtype=torch.int32).pin_memory()
+    for rep in range(2):  # the second call reuses the plan's copy stream and events
+        g.plan.search_host_batches(h_in, nb, g.buf["d_in"], d_in1, g.buf["d_out"], g.buf["d_snr"], g.buf["d_argmax"],
+                                   h_snr, h_arg)
+        for b in range(nb):
+            _, So, Ao = oracle_search(np.ascontiguousarray(Ylong[:, b * ns: (b + 1) * ns]), list(cfg.widths), 0)
+            assert_snr_close(h_snr[b].numpy(), So, "batch %d" % b)
+            assert np.array_equal(h_arg[b].numpy().view(np.uint32), Ao), "argmax of batch %d" % b
+        h_snr.fill_(-3.0)
+    # the last batch's dedispersed rows are still on the device
+    assert np.array_equal(u32(g.buf["d_out"])[:, :ns], Ylong[:, (nb - 1) * ns:])
     g.close()
 
 
@@ -279,6 +326,52 @@ def test_integrate_and_snr_sparse_wide_widths_sweep():
             g.integrate()
             g.snr()
             compare_all(g, Yo, what="%s %r" % (ddp.KERNEL_NAMES[kernel], c))
+    g.close()
+
+
+# ---------------------------------------------------------------------------------- fused integration + S/N (8(f) f1)
+@pytest.mark.parametrize("widths,ns,ddof", [((1, 2, 4, 8, 16, 32, 64, 128, 256), 4099, 0),
+                                            ((1, 2, 8, 64, 512, 1024, 2048), 9217, 0),
+                                            ((2, 16, 4096), 12290, 1),
+                                            ((1,), 700, 0)])
+def test_fused_integrate_snr_equals_oracle(widths, ns, ddof):
+    """ddp_integrate_snr (one pass over Y) against the oracle's integrate + snr: S/N within 1e-5, argmax exact, for
+    every valid kernel shape (all block-sum levels: in-thread, across lanes, across chunks), ragged lengths, sparse
+    width sets, both ddof; with a plane buffer the planes are bit-exact too, without one nothing is written."""
+    cfg = small_direct(name="fused%d" % ns, nchan=24, nsamp_out=ns, ndm=21, widths=widths, n_pulses=2)
+    g = GpuSearch(cfg, snr_ddof=ddof)
+    Yg = g.dedisperse()
+    Yo = oracle_direct_rows(cfg, g.X)
+    assert np.array_equal(Yg, Yo)
+    Po, So, Ao = oracle_search(Yo, list(widths), ddof)
+    V = g.plan.enumerate_kcfgs(ddp.K_ISNR)
+    assert len(V) >= 10
+    for c in V:
+        g.plan.set_kcfg(ddp.K_ISNR, c)
+        g.buf["d_integ"].fill_(-1)
+        g.buf["d_snr"].fill_(-7.0)
+        g.buf["d_argmax"].fill_(-1)
+        g.plan.integrate_snr(g.buf["d_out"], g.buf["d_snr"], g.buf["d_argmax"])  # no planes
+        g.torch.cuda.synchronize()
+        assert_snr_close(g.buf["d_snr"].cpu().numpy(), So, "fused %r" % c)
+        assert np.array_equal(u32(g.buf["d_argmax"]), Ao), "fused argmax differs for %r" % c
+        assert bool((g.buf["d_integ"] == -1).all()), "fused kernel wrote planes it was not given"
+    for c in (V[0], V[len(V) // 2], V[-1]):
+        g.plan.set_kcfg(ddp.K_ISNR, c)
+        g.buf["d_snr"].fill_(-7.0)
+        g.plan.integrate_snr(g.buf["d_out"], g.buf["d_snr"], None, d_integ=g.buf["d_integ"])  # planes, no argmax
+        g.torch.cuda.synchronize()
+        assert_snr_close(g.buf["d_snr"].cpu().numpy(), So, "fused with planes %r" % c)
+        Pg = g.planes()
+        for w in widths:
+            if w > 1:
+                assert np.array_equal(Pg[w], Po[w]), "fused plane w=%d differs for %r" % (w, c)
+    # the separate kernels give the same bits
+    g.integrate()
+    S2, A2 = g.snr()
+    g.plan.integrate_snr(g.buf["d_out"], g.buf["d_snr"], g.buf["d_argmax"])
+    g.torch.cuda.synchronize()
+    assert np.array_equal(g.buf["d_snr"].cpu().numpy(), S2) and np.array_equal(u32(g.buf["d_argmax"]), A2)
     g.close()
 
 
