@@ -90,7 +90,14 @@ typedef struct {
     int snr_ddof;          /* 0 = population std (default, SNR.2), 1 = sample std                     */
     int device;            /* CUDA device ordinal                                                      */
     const char* cache_dir; /* directory for compiled-kernel cubins; NULL = no disk cache               */
+    int integration_mode;  /* DDP_INTEG_DECIMATE (0, default: block sums, stride w; INT.1) or DDP_INTEG_SLIDING (1:
+                              stride-1 boxcar I^s_w[t] = sum_{k<w} Y[t+k], t <= nsamp_out - w).  In sliding
+                              mode the sums are never materialised: only ddp_integrate_snr (d_integ = NULL) and the
+                              search calls run; ddp_integrate, ddp_snr and the tuners return DDP_E_CONFIG         */
+    const uint8_t* chan_mask; /* host, nchan bytes or NULL: channels whose byte is 0 are left out of every sum
+                              (zapped channels); copied at plan creation                  */
 } ddp_options;
+enum { DDP_INTEG_DECIMATE = 0, DDP_INTEG_SLIDING = 1 };
 
 /* Geometry of a plan (all counts in elements unless named *_bytes). */
 typedef struct {
@@ -105,7 +112,7 @@ typedef struct {
     int64_t nsamp_sub;           /* subband: samples per intermediate row = nsamp_out + max_d2 (SB.4)   */
     int64_t sub_stride;          /* subband: element stride of the intermediate rows                    */
     int widths[DDP_MAX_WIDTHS];
-    int64_t plane_len[DDP_MAX_WIDTHS];    /* n_w = floor(nsamp_out / w)                       (INT.2) */
+    int64_t plane_len[DDP_MAX_WIDTHS];    /* values per series: floor(nsamp_out / w) (INT.2); sliding mode: nsamp_out - w + 1 */
     int64_t plane_stride[DDP_MAX_WIDTHS]; /* row stride of plane w in d_integ; 0 for w == 1            */
     int64_t plane_offset[DDP_MAX_WIDTHS]; /* element offset of plane w in d_integ; -1 for w == 1       */
     int64_t integ_elems;         /* uint32 elements the caller allocates for d_integ                    */
@@ -113,6 +120,8 @@ typedef struct {
     double adds_dedisp;          /* algorithmic integer adds of one dedisperse call                     */
     int sub_elem_bytes;          /* subband: bytes per element of the intermediate S: 2 (uint16) when
                                     255 * channels-per-subband <= 65535 makes that exact, else 4 (SB.4)  */
+    int integration_mode;        /* DDP_INTEG_DECIMATE or DDP_INTEG_SLIDING                               */
+    int nchan_masked;            /* channels left out by the plan's channel mask                          */
 } ddp_plan_info;
 
 /* ---- plan -------------------------------------------------------------------------------------

@@ -68,6 +68,11 @@ struct ddp_plan {
     int nsub = 0, ncoarse = 0, nfine = 0, cps = 0;
     double coarse_first = 0, coarse_step = 0, fine_step = 0;
     int ddof = 0, device = 0;
+    int integ_mode = 0;                    // DDP_INTEG_DECIMATE / DDP_INTEG_SLIDING
+    std::vector<unsigned char> chan_mask;  // empty = every channel used; else nchan bytes, 0 = left out
+    std::vector<int32_t> rowmap_host;      // host copy of the row map (outlives the asynchronous upload)
+    int32_t* d_rowmap = nullptr;           // device: input row of every reduction row, -1 = masked (null without a mask)
+    unsigned char* d_zero_row = nullptr;   // device: in_stride_min zero bytes a masked row reads
     std::string cache_dir;
     // host tables
     std::vector<int32_t> delay, d1, d2;
@@ -95,6 +100,7 @@ struct ddp_plan {
 DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k);
 bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k);
 int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD);           // dedisp kernels only
+int ddp_slide_nb(const ddp_plan* p, const ddp_kcfg& c);                 // sliding boxcar kernel: prefix-sum ring length in chunks
 int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // staged row window (elements)
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // packed uint8 kernel: one copy buffer

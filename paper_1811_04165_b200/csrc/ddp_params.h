@@ -25,6 +25,8 @@ struct DdpDedispParams {
     int ndm;                     // length of the i axis
     int ns;                      // output samples per row
     int win;                     // staged modes: elements of one staged row window in shared memory
+    const int* rowmap;           // channel mask: input row of reduction row g*nred + r, -1 = masked; null = no mask
+    const unsigned char* zero_row;  //   the row of zeros a masked reduction row reads (in_row_len bytes)
     int one;                     // the value 1, unknown to the compiler (packed kernel: adds issued as IMAD)
     int vmax;                    // merged staging: variant slots per table record (largest variant count of the plan, padded to 4)
     int lw;                      // merged staging: words per variant row  (TT/2 + largest window spread, padded)
@@ -85,6 +87,8 @@ struct DdpIsnrParams {
     int ns;
     int ddof;
     int max_lvl;                 // log2 of the largest width
+    int width[DDP_MAXW];         // sliding mode: the widths themselves
+    int slide_nb;                // sliding mode: prefix-sum ring length in chunks = 1 + ceil(largest width / chunk)
 };
 
 #endif  // DDP_PARAMS_H_

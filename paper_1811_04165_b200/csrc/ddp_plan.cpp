@@ -101,12 +101,15 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
         p->ddof = opt->snr_ddof;
         p->device = opt->device;
         if (opt->cache_dir) p->cache_dir = opt->cache_dir;
+        p->integ_mode = opt->integration_mode;
+        if (opt->chan_mask) p->chan_mask.assign(opt->chan_mask, opt->chan_mask + nchan);
     }
     auto bail = [&](ddp_status s) {
         delete p;
         return s;
     };
     if (p->ddof != 0 && p->ddof != 1) return bail(DDP_E_ARG);
+    if (p->integ_mode != DDP_INTEG_DECIMATE && p->integ_mode != DDP_INTEG_SLIDING) return bail(DDP_E_ARG);
     if (nsamp_out / widths[nwidths - 1] - p->ddof < 1) return bail(DDP_E_ARG);
     const double f_ref = *std::max_element(p->freq.begin(), p->freq.end());  // DD.3
 
@@ -181,11 +184,14 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     // SB.4: the intermediate is stored as uint16 whenever that is exact (255 * channels per subband
     // fits 16 bits), which halves its HBM and shared-memory traffic; uint32 otherwise.
     I.sub_elem_bytes = p->subband ? (255 * (int64_t)p->cps <= 65535 ? 2 : 4) : 0;
+    I.integration_mode = p->integ_mode;
+    I.nchan_masked = 0;
+    for (unsigned char m : p->chan_mask) I.nchan_masked += m == 0;
     int64_t off = 0;
     for (int k = 0; k < nwidths; ++k) {
         I.widths[k] = widths[k];
-        I.plane_len[k] = nsamp_out / widths[k];
-        if (widths[k] == 1) {
+        I.plane_len[k] = p->integ_mode == DDP_INTEG_SLIDING ? nsamp_out - widths[k] + 1 : nsamp_out / widths[k];
+        if (widths[k] == 1 || p->integ_mode == DDP_INTEG_SLIDING) {  // sliding sums are never materialised
             I.plane_stride[k] = 0;
             I.plane_offset[k] = -1;
         } else {
@@ -200,9 +206,12 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     int64_t sbytes = p->subband ? round_up((int64_t)p->ncoarse * p->nsub * I.sub_stride * I.sub_elem_bytes, 256) : 0;
     // region for the resident merged-staging table (one (kernel, TD, G) at a time; DdpMergeTable)
     p->merge_capacity = round_up(2 * (int64_t)(p->subband ? p->d1.size() : p->delay.size()) * 4 + (1 << 20), 256);
-    I.workspace_bytes = tbytes + sbytes + p->merge_capacity + 256;
-    I.adds_dedisp = p->subband ? (double)p->ncoarse * nchan * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
-                               : (double)p->ndm * nchan * nsamp_out;
+    // channel mask: row map (one int per channel) and the row of zeros a masked channel reads
+    const int64_t mbytes = p->chan_mask.empty() ? 0 : round_up((int64_t)nchan * 4, 256) + round_up(I.in_stride_min, 256);
+    I.workspace_bytes = tbytes + sbytes + p->merge_capacity + mbytes + 256;
+    const double nused = (double)(nchan - I.nchan_masked);  // masked channels are not part of the algorithmic work
+    I.adds_dedisp = p->subband ? (double)p->ncoarse * nused * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
+                               : (double)p->ndm * nused * nsamp_out;
     default_kcfgs(p);
     *out = p;
     return DDP_OK;
@@ -239,7 +248,7 @@ bool ddp_kernel_in_plan(const ddp_plan* p, ddp_kernel k) {
         case DDP_K_SUB1:
         case DDP_K_SUB2: return p->subband;
         case DDP_K_INTEGRATE:
-        case DDP_K_SNR:
+        case DDP_K_SNR: return p->integ_mode == DDP_INTEG_DECIMATE;
         case DDP_K_ISNR: return true;
         default: return false;
     }
@@ -264,6 +273,13 @@ DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k) {
     return g;
 }
 
+// Sliding boxcar kernel: chunks of prefix sums a warp keeps = 1 + ceil(largest width / chunk).
+int ddp_slide_nb(const ddp_plan* p, const ddp_kcfg& c) {
+    int maxw = 1;
+    for (int i = 0; i < p->nwidths; ++i) maxw = std::max(maxw, p->widths[i]);
+    const int ch = 32 * c.samples_per_thread;
+    return 1 + (maxw + ch - 1) / ch;
+}
 // Largest (dmax - dmin) of any reduction row over any DM tile of TD trials: bounds the staged window.
 int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD) {
     const int which = k == DDP_K_DIRECT ? 0 : (k == DDP_K_SUB1 ? 1 : 2);
@@ -486,7 +502,13 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (c.staging != 0) b += (size_t)c.threads_dm * TT * 4 + 16;
             return b;
         }
-        case DDP_K_ISNR: return (size_t)c.threads_dm * 8 * 8 * 4;  // wide-level accumulators [threads_dm][8][8]
+        case DDP_K_ISNR: {
+            if (p->integ_mode == DDP_INTEG_SLIDING) {  // prefix-sum ring per warp: (1 + ceil(wmax / chunk)) chunks, skewed
+                const int64_t ring = (int64_t)ddp_slide_nb(p, c) * 32 * c.samples_per_thread;
+                return (size_t)c.threads_dm * (size_t)(ring + (ring >> 5)) * 4;
+            }
+            return (size_t)c.threads_dm * 8 * 8 * 4;  // wide-level accumulators [threads_dm][8][8]
+        }
         case DDP_K_SNR: {
             size_t b = (size_t)c.threads_dm * 32 * 24;
             if (c.staging != 0) b += (size_t)c.threads_dm * (c.staging == 2 ? 2 : 1) * TT * 4 + (size_t)c.threads_dm * 16;
@@ -528,6 +550,7 @@ bool ddp_kcfg_valid(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, std::str
         int maxw = 1;
         for (int i = 0; i < p->nwidths; ++i) maxw = std::max(maxw, p->widths[i]);
         if (maxw > 32 * c.samples_per_thread * 256) return no("V3: a width is longer than 256 chunks of the fused kernel");
+        if (ddp_smem_bytes(p, k, c) > DDP_SMEM_LIMIT) return no("V6: shared memory over 227 KB");
         return true;
     }
     // V7: a gene the kernel does not read is pinned (snr reads `unroll` only with direct loads)

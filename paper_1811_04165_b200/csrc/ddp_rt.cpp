@@ -278,7 +278,8 @@ std::string kernel_name(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d_w%d", kind_tag(ck), c.samples_per_thread,
                       c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt_bucket(c), code_flags(p, k, c));
     else if (ck == CK_ISNR)
-        std::snprintf(b, sizeof b, "%s_s%d_d%d_t%d", kind_tag(ck), c.samples_per_thread, c.dms_per_thread, maxt_bucket(c));
+        std::snprintf(b, sizeof b, "%s%s_s%d_d%d_t%d", kind_tag(ck), p->integ_mode == DDP_INTEG_SLIDING ? "_slide" : "",
+                      c.samples_per_thread, c.dms_per_thread, maxt_bucket(c));
     else  // integrate reads `unroll` at run time (tiles per block): not part of its code shape
         std::snprintf(b, sizeof b, "%s_s%d_d%d_u%d_g%d_v%d_t%d", kind_tag(ck), c.samples_per_thread,
                       c.dms_per_thread, ck == CK_INTEG ? 1 : c.unroll, c.staging, c.vec_bytes, maxt_bucket(c));
@@ -296,7 +297,8 @@ std::string define_line(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, cons
                           c.samples_per_thread, c.dms_per_thread, c.unroll, c.staging, c.vec_bytes, maxt, code_flags(p, k, c));
             break;
         case CK_ISNR:
-            std::snprintf(b, sizeof b, "\nDDP_DEFINE_ISNR(%s, %d, %d, %d)\n", name.c_str(), c.samples_per_thread, c.dms_per_thread, maxt);
+            std::snprintf(b, sizeof b, "\nDDP_DEFINE_ISNR%s(%s, %d, %d, %d)\n", p->integ_mode == DDP_INTEG_SLIDING ? "_SLIDE" : "",
+                          name.c_str(), c.samples_per_thread, c.dms_per_thread, maxt);
             break;
         case CK_INTEG:
             std::snprintf(b, sizeof b, "\nDDP_DEFINE_INTEG(%s, %d, %d, %d, %d, %d, %d)\n", name.c_str(),
@@ -647,6 +649,18 @@ extern "C" ddp_status ddp_plan_bind_workspace(ddp_plan* plan, void* d_workspace,
     }
     plan->d_merge = (unsigned char*)(base + off);
     plan->merge_resident[0] = -1;
+    off += (size_t)plan->merge_capacity;
+    plan->d_rowmap = nullptr;
+    plan->d_zero_row = nullptr;
+    if (!plan->chan_mask.empty() && r == CUDA_SUCCESS) {  // DD.7m: masked channels read a row of zeros
+        plan->rowmap_host.resize(plan->nchan);
+        for (int c = 0; c < plan->nchan; ++c) plan->rowmap_host[c] = plan->chan_mask[c] ? c : -1;
+        r = upload(plan->rowmap_host, &plan->d_rowmap);
+        plan->d_zero_row = (unsigned char*)(base + off);
+        if (r == CUDA_SUCCESS)
+            r = g_api.p_cuMemsetD32Async((CUdeviceptr)plan->d_zero_row, 0u, (size_t)round_up64(plan->info.in_stride_min, 256) / 4,
+                                         (CUstream)stream);
+    }
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "delay table upload: " + cu_err(r));
     plan->ws = d_workspace;
     plan->ws_bytes = bytes;
@@ -752,6 +766,11 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
     }
     q.win = c.staging ? ddp_dedisp_win(p, k, c) : 0;
     q.one = 1;
+    if (p->d_rowmap && k != DDP_K_SUB2) {  // channel mask: the zero row is in_stride_min long, which covers every needed sample
+        q.rowmap = p->d_rowmap;
+        q.zero_row = p->d_zero_row;
+        q.in_row_len = std::min<long long>(q.in_row_len, (long long)I.in_stride_min);
+    }
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
     if (const int G = ddp_merge_group(c)) {
@@ -894,6 +913,13 @@ ddp_status launch_isnr(const ddp_plan* p, const ddp_kcfg& c, DdpCompiled* K, con
     q.ns = p->ns;
     q.ddof = p->ddof;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
+    if (p->integ_mode == DDP_INTEG_SLIDING) {  // ddp_isnr_slide_body: a grid row per 4 widths, no planes
+        if (io.d_integ) return ddp_fail(p, DDP_E_ARG, "sliding boxcar sums are never materialised: d_integ must be NULL");
+        for (int k = 0; k < p->nwidths; ++k) q.width[k] = p->widths[k];
+        q.slide_nb = ddp_slide_nb(p, c);
+        return launch(p, K, cdiv(p->ndm, TD), cdiv(p->nwidths, 4), 1, 32u, (unsigned)c.threads_dm,
+                      ddp_smem_bytes(p, DDP_K_ISNR, c), io.stream, &q);
+    }
     return launch(p, K, cdiv(p->ndm, TD), 1, 1, 32u, (unsigned)c.threads_dm, ddp_smem_bytes(p, DDP_K_ISNR, c), io.stream, &q);
 }
 
@@ -944,6 +970,8 @@ extern "C" ddp_status ddp_integrate(ddp_plan* plan, const uint32_t* d_dedisp, si
     if (!plan) return DDP_E_ARG;
     ddp_status s = ensure_ctx(plan, plan->device);
     if (s != DDP_OK) return s;
+    if (plan->integ_mode != DDP_INTEG_DECIMATE)
+        return ddp_fail(plan, DDP_E_CONFIG, "sliding boxcar plan: the sums are not materialised, use ddp_integrate_snr");
     if (!d_dedisp || (!d_integ && plan->info.integ_elems > 0)) return ddp_fail(plan, DDP_E_ARG, "NULL device pointer");
     if ((int64_t)stride < plan->info.out_stride_min || stride % 4 != 0 || ((uintptr_t)d_dedisp & 15u) ||
         ((uintptr_t)d_integ & 15u))
@@ -959,6 +987,8 @@ extern "C" ddp_status ddp_snr(ddp_plan* plan, const uint32_t* d_dedisp, size_t s
     if (!plan) return DDP_E_ARG;
     ddp_status s = ensure_ctx(plan, plan->device);
     if (s != DDP_OK) return s;
+    if (plan->integ_mode != DDP_INTEG_DECIMATE)
+        return ddp_fail(plan, DDP_E_CONFIG, "sliding boxcar plan: use ddp_integrate_snr");
     if (!d_dedisp || !d_snr || (!d_integ && plan->info.integ_elems > 0))
         return ddp_fail(plan, DDP_E_ARG, "NULL device pointer");
     if ((int64_t)stride < plan->info.out_stride_min || stride % 4 != 0 || ((uintptr_t)d_dedisp & 15u) ||
@@ -999,7 +1029,7 @@ extern "C" ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_
     CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)d_in, h_in, in_stride * (size_t)plan->nchan, st);
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "H2D copy: " + cu_err(r));
     if ((s = ddp_dedisperse(plan, d_in, in_stride, d_out, out_stride, stream)) != DDP_OK) return s;
-    if (d_integ) {
+    if (d_integ && plan->integ_mode == DDP_INTEG_DECIMATE) {
         if ((s = ddp_integrate(plan, d_out, out_stride, d_integ, stream)) != DDP_OK) return s;
         if ((s = ddp_snr(plan, d_out, out_stride, d_integ, d_snr, d_argmax, stream)) != DDP_OK) return s;
     } else if ((s = ddp_integrate_snr(plan, d_out, out_stride, nullptr, d_snr, d_argmax, stream)) != DDP_OK) {

@@ -187,6 +187,7 @@ bool io_ok(const ddp_plan* p, const ddp_tune_io* io, const ddp_tune_result* res)
 // ------------------------------------------------------------------------------------ GA
 extern "C" ddp_status ddp_tune_ga(ddp_plan* plan, const ddp_tune_io* io, const ddp_ga_params* gp, ddp_tune_result* res) {
     if (!io_ok(plan, io, res) || !gp) return DDP_E_ARG;
+    if (plan->integ_mode != DDP_INTEG_DECIMATE) return ddp_fail(plan, DDP_E_CONFIG, "the tuners time the integrate and snr kernels: the plan must use DDP_INTEG_DECIMATE");
     const int N = gp->population, G = gp->generations, T = gp->tournament, E = gp->elitism;
     if (N < 2 || G < 0 || T < 1 || E < 0 || E >= N || !(gp->p_cross >= 0.0 && gp->p_cross <= 1.0) ||
         !(gp->p_mut >= 0.0 && gp->p_mut <= 1.0))
@@ -289,6 +290,7 @@ extern "C" ddp_status ddp_tune_ga(ddp_plan* plan, const ddp_tune_io* io, const d
 // ------------------------------------------------------------------------------------ random search
 extern "C" ddp_status ddp_tune_random(ddp_plan* plan, const ddp_tune_io* io, const ddp_rand_params* rp, ddp_tune_result* res) {
     if (!io_ok(plan, io, res) || !rp) return DDP_E_ARG;
+    if (plan->integ_mode != DDP_INTEG_DECIMATE) return ddp_fail(plan, DDP_E_CONFIG, "the tuners time the integrate and snr kernels: the plan must use DDP_INTEG_DECIMATE");
     if (rp->max_evals <= 0) return ddp_fail(plan, DDP_E_BUDGET, "random search needs a positive evaluation budget");
     Run R(plan, io, res, rp->max_evals);
     Rng rng(rp->seed);
@@ -320,6 +322,7 @@ extern "C" ddp_status ddp_tune_random(ddp_plan* plan, const ddp_tune_io* io, con
 // together once, which is the figure comparable with the GA's joint fitness (GA.6).
 extern "C" ddp_status ddp_tune_bruteforce(ddp_plan* plan, const ddp_tune_io* io, const ddp_bf_params* bp, ddp_tune_result* res) {
     if (!io_ok(plan, io, res) || !bp) return DDP_E_ARG;
+    if (plan->integ_mode != DDP_INTEG_DECIMATE) return ddp_fail(plan, DDP_E_CONFIG, "the tuners time the integrate and snr kernels: the plan must use DDP_INTEG_DECIMATE");
     if (bp->max_evals_per_kernel < 0) return ddp_fail(plan, DDP_E_BUDGET, "negative evaluation budget");
     Run R(plan, io, res, 0);
     Chrom ref;

@@ -375,6 +375,119 @@ def test_fused_integrate_snr_equals_oracle(widths, ns, ddof):
     g.close()
 
 
+@pytest.mark.parametrize("widths,ns", [((1, 2, 4, 8, 16, 32, 64, 128, 256), 4099), ((1, 2, 8, 64, 512, 1024), 5203),
+                                       ((4,), 777)])
+def test_sliding_boxcar_mode_equals_oracle(widths, ns):
+    """integration_mode = SLIDING (8(f) f1, INT.1s): the stride-1 boxcar S/N of ddp_integrate_snr against
+    oracle.search_sliding (S/N within 1e-5, argmax = first sample of the best window, exact) for every kernel shape;
+    the calls that need materialised sums refuse the plan."""
+    import oracle
+    cfg = small_direct(name="slide%d" % ns, nchan=24, nsamp_out=ns, ndm=13, widths=widths, n_pulses=2)
+    g = GpuSearch(cfg, integration_mode=1)
+    assert g.info.integration_mode == 1 and g.info.integ_elems == 0
+    assert [g.info.plane_len[k] for k in range(len(widths))] == [ns - w + 1 for w in widths]
+    Yg = g.dedisperse()
+    Yo = oracle_direct_rows(cfg, g.X)
+    assert np.array_equal(Yg, Yo)
+    _, So, Ao = oracle.search_sliding(Yo, list(widths))
+    V = g.plan.enumerate_kcfgs(ddp.K_ISNR)
+    assert len(V) >= 10
+    for c in V:
+        g.plan.set_kcfg(ddp.K_ISNR, c)
+        g.buf["d_snr"].fill_(-7.0)
+        g.buf["d_argmax"].fill_(-1)
+        g.plan.integrate_snr(g.buf["d_out"], g.buf["d_snr"], g.buf["d_argmax"])
+        g.torch.cuda.synchronize()
+        assert_snr_close(g.buf["d_snr"].cpu().numpy(), So, "sliding %r" % c)
+        assert np.array_equal(u32(g.buf["d_argmax"]), Ao), "sliding argmax differs for %r" % c
+    for call in (lambda: g.plan.integrate(g.buf["d_out"], g.buf["d_snr"]),
+                 lambda: g.plan.snr(g.buf["d_out"], None, g.buf["d_snr"], g.buf["d_argmax"])):
+        with pytest.raises(ddp.DdpError) as e:
+            call()
+        assert e.value.status == ddp.binding.E_CONFIG
+    # the end-to-end call works without a plane buffer
+    h_snr = np.full(So.shape, -3.0, dtype=np.float32)
+    g.plan.search_host(g.X, g.buf["d_in"], g.buf["d_out"], None, g.buf["d_snr"], g.buf["d_argmax"], h_snr, None)
+    assert_snr_close(h_snr, So, "sliding search_host")
+    g.close()
+
+
+def test_sliding_boxcar_recovers_the_misaligned_cfg0_pulse_at_its_width():
+    """SURVEY INT.1: the BJ:cfg0 pulse moved to t0 = 2002 (not a multiple of its width 4) is found at (DM 17, w 4,
+    t 2002) by the sliding search, while the decimating search of the same data peaks at width 2."""
+    import dataclasses
+    base = configs.tiny()
+    cfg = dataclasses.replace(base, fixed_pulses=(dataclasses.replace(base.fixed_pulses[0], t0=2002),))
+    gs = GpuSearch(cfg, integration_mode=1)
+    gs.dedisperse()
+    gs.plan.integrate_snr(gs.buf["d_out"], gs.buf["d_snr"], gs.buf["d_argmax"])
+    gs.torch.cuda.synchronize()
+    S, A = gs.buf["d_snr"].cpu().numpy(), u32(gs.buf["d_argmax"])
+    i, k = np.unravel_index(np.argmax(S), S.shape)
+    assert cfg.dm_list()[i] == 17.0 and cfg.widths[k] == 4 and A[i, k] == 2002
+    gd = GpuSearch(cfg, X=gs.X)
+    gd.run_all()
+    Sd = gd.buf["d_snr"].cpu().numpy()
+    i2, k2 = np.unravel_index(np.argmax(Sd), Sd.shape)
+    assert cfg.dm_list()[i2] == 17.0 and cfg.widths[k2] == 2 and S[i, k] > Sd[i2, k2]
+    gs.close()
+    gd.close()
+
+
+# ---------------------------------------------------------------------------------- channel mask (8(f) f4, P:126)
+def test_channel_mask_direct_every_staging_mode():
+    """A plan with zapped channels (reading DD.7m) against oracle.dedisperse_masked, bit-exact, for direct loads,
+    cooperative and TMA staging, the packed kernel's wide flush (320 channels) and merged staging; what the masked
+    channels hold must not matter (they are filled with 255 here)."""
+    import oracle
+    nchan = 320
+    cfg = small_direct(name="mask", nchan=nchan, nsamp_out=2300, ndm=41, widths=(1, 2, 4, 8), n_pulses=2)
+    rng = np.random.default_rng(7)
+    mask = (rng.random(nchan) > 0.2).astype(np.uint8)
+    mask[:3] = 0
+    mask[-1] = 0
+    g = GpuSearch(cfg, chan_mask=mask)
+    assert g.info.nchan_masked == int((mask == 0).sum()) > 10
+    g.X[mask == 0] = 255
+    g.upload()
+    delay = oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s)
+    Yo = oracle.dedisperse_masked(g.X, mask, delay, cfg.nsamp_out)
+    V = g.plan.enumerate_kcfgs(ddp.K_DIRECT)
+    picks = []
+    for st in (0, 1, 2, 3, 4):
+        picks += _sample([c for c in V if c.staging == st], 6, seed=st)
+    assert {c.staging for c in picks} == {0, 1, 2, 3, 4}
+    for c in picks:
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        g.buf["d_out"].fill_(-1)
+        assert np.array_equal(g.dedisperse(), Yo), "masked direct differs for %r" % c
+    g.run_all()
+    compare_all(g, Yo, what="masked, whole pipeline")
+    # all channels kept == no mask at all
+    g2 = GpuSearch(cfg, X=g.X, chan_mask=np.ones(nchan, np.uint8))
+    assert np.array_equal(g2.dedisperse(), oracle_direct_rows(cfg, g.X))
+    g.close()
+    g2.close()
+
+
+def test_channel_mask_subband_plan():
+    """Masked channels in a two-step plan: equal to the subband oracle on a copy of the input whose masked channels
+    are zero (a zero row adds nothing), S and Y bit-exact."""
+    cfg = small_subband(name="mask_sb")
+    mask = np.ones(cfg.nchan, np.uint8)
+    mask[[0, 5, 11, 12, 13, 40, 95]] = 0
+    g = GpuSearch(cfg, chan_mask=mask)
+    Xz = g.X.copy()
+    Xz[mask == 0] = 0
+    g.X[mask == 0] = 200
+    g.upload()
+    So, Yo = oracle_subband(cfg, Xz)
+    g.run_all()
+    assert np.array_equal(g.subband_intermediate(), So)
+    compare_all(g, Yo, what="masked subband")
+    g.close()
+
+
 @pytest.mark.parametrize("kernel", [ddp.K_SUB1, ddp.K_SUB2])
 def test_subband_plan_kernel_configuration_sweep(kernel):
     cfg = small_subband(name="sweep_sb", nchan=128, nsamp_out=2100, ndm=24 * 8,
