@@ -458,7 +458,6 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     const int tile_t = blockIdx.x * TT;
     const int tile_dm = blockIdx.y * TD;
     const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
-    const ddp_u8* in_g = (const ddp_u8*)p.in + (ddp_i64)g * p.in_group_stride;
     const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
     const int win = p.win, winw = win >> 2;
     const ddp_u32 one = (ddp_u32)p.one;
@@ -750,7 +749,8 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     ddp_u64* mbar = (ddp_u64*)(ring + (size_t)DDP_MRG_DEPTH * SLOTW);        // raw[2], stg[2], rows built [DEPTH], rows consumed [DEPTH]
     ddp_u64* mfull = mbar + 4;
     ddp_u64* mempty = mfull + DDP_MRG_DEPTH;
-    int* sched = (int*)(mempty + DDP_MRG_DEPTH);                             // scheduler cursor [8], ring head, extents of the last chunks [2 * AHEAD]
+    ddp_u64* mexp = mempty + DDP_MRG_DEPTH;                                  // E rows of chunk x expanded (by the consumers) [2]
+    int* sched = (int*)(mexp + 2);                                           // scheduler cursor [8], ring head, extents of the last chunks [2 * AHEAD]
     // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, -, -, first word in the variant-row ring,
     //            chunk the consumers must have left before this one is built} | a0[U] | bytes[U] |
     //            carry[U] | nz4[U] | rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
@@ -775,6 +775,8 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             ddp_mbar_init(&mfull[b], NPW);
             ddp_mbar_init(&mempty[b], NCW);
         }
+        ddp_mbar_init(&mexp[0], NCW);
+        ddp_mbar_init(&mexp[1], NCW);
         ddp_mbar_fence_init();
         const int tile = unit_lo / nseg, rest = tile / p.n_ttiles;
         sched[0] = unit_lo;
@@ -945,6 +947,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                 const int x = n + 3;
                 const int* d = slot(x);
                 if (x >= 0 && x < nstream) {
+                    if (x >= 2) ddp_mbar_wait(&mexp[x & 1], (ddp_u32)(((x >> 1) - 1) & 1));  // chunk x - 2 has been expanded out of this raw slot
                     const ddp_u32 bytes = lane < U ? (ddp_u32)d[16 + U + lane] : 0u;
                     ddp_u32 total = bytes;
 #pragma unroll
@@ -956,85 +959,54 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                                      ddp_in_row<ddp_u8>(p, d[3], d[4] + lane) + d[16 + lane], bytes, &mbar[x & 1]);
                 }
             }
-            // ---- build chunk n + 1 (E rows -> variant rows of buffer (n + 1) & 1) and expand chunk n + 2 (raw slot -> E rows):
-            //      items = half rows, handed out round robin to producer warps 1.. (warp 0 keeps the control work above)
+            // ---- build chunk n + 1 (E rows, expanded by the consumers -> variant rows in the ring): items = half rows,
+            //      handed out round robin to producer warps 1.. (warp 0 keeps the control work above)
             {
-                const int xb = n + 1, xs = n + 2;
+                const int xb = n + 1;
                 const int* db = slot(xb);
-                const int* ds = slot(xs);
-                const bool vb = xb >= 0 && xb < nstream, vs = xs >= 0 && xs < nstream;
-                if (vb && db[12] >= 0) {  // the consumers have left the rows this chunk overwrites
-                    const int wc = db[12];
-                    ddp_mbar_wait(&mempty[wc & (DDP_MRG_DEPTH - 1)], (ddp_u32)((wc / DDP_MRG_DEPTH) & 1));
+                const bool vb = xb >= 0 && xb < nstream;
+                if (vb) {
+                    if (db[12] >= 0) {  // the consumers have left the rows this chunk overwrites
+                        const int wc = db[12];
+                        ddp_mbar_wait(&mempty[wc & (DDP_MRG_DEPTH - 1)], (ddp_u32)((wc / DDP_MRG_DEPTH) & 1));
+                    }
+                    ddp_mbar_wait(&mexp[xb & 1], (ddp_u32)((xb >> 1) & 1));  // its E rows are there
                 }
-                if (vs) ddp_mbar_wait(&mbar[xs & 1], (ddp_u32)((xs >> 1) & 1));                          // raw windows landed
-                if (pwarp > 0) {
-                    const int NB = vb ? 2 * db[6] : 0;       // build items: (variant row, half)
-                    const int NI = NB + (vs ? 2 * U : 0);    // expand items: (channel, half)
+                if (pwarp > 0 && vb) {
+                    const int NB = 2 * db[6];  // build items: (variant row, half)
                     const int* rowd = db + 16 + 4 * U;
                     const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
-                    ddp_u32* pb = pw + (vb ? db[11] : 0) + lane;
-                    const int* nz4s = ds + 16 + 3 * U;
-                    const int hq = H >> 2;
-                    const unsigned char* rbase = raw + (size_t)(xs & 1) * U * (win + 16);
-                    ddp_u32* ebase = ebuf + (size_t)(xs & 1) * U * le + DDP_MRG_EPAD;
-                    for (int it = rot; it < NI; it += NPW - 1) {
-                        if (it < NB) {
-                            const int row = it >> 1;
-                            const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
-                            const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
-                            const int half = ((d0.x >> 1) + 31) & ~31;
-                            int y = (it & 1) ? half : 0;
-                            const int yend = (it & 1) ? d0.x : (half < d0.x ? half : d0.x);
-                            const ddp_u32* e0 = eb + d0.z;
-                            const ddp_u32* e1 = eb + d0.w;
-                            const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0);
-                            const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0);
-                            ddp_u32* dst = pb + d0.y;
-                            const int yl = yend - lane;  // words of this lane's column before the end
-                            for (; y < yend; y += 256) {  // blocks of 256 words, all loads first; the ragged end is predicated
-                                ddp_u32 sm[8];
+                    ddp_u32* pb = pw + db[11] + lane;
+                    for (int it = rot; it < NB; it += NPW - 1) {
+                        const int row = it >> 1;
+                        const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                        const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
+                        const int half = ((d0.x >> 1) + 31) & ~31;
+                        int y = (it & 1) ? half : 0;
+                        const int yend = (it & 1) ? d0.x : (half < d0.x ? half : d0.x);
+                        const ddp_u32* e0 = eb + d0.z;
+                        const ddp_u32* e1 = eb + d0.w;
+                        const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0);
+                        const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0);
+                        ddp_u32* dst = pb + d0.y;
+                        const int yl = yend - lane;  // words of this lane's column before the end
+                        for (; y < yend; y += 256) {  // blocks of 256 words, all loads first; the ragged end is predicated
+                            ddp_u32 sm[8];
 #pragma unroll
-                                for (int i = 0; i < 8; ++i) {
-                                    if (y + 32 * i < yl) {
-                                        sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
-                                        if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
-                                    }
+                            for (int i = 0; i < 8; ++i) {
+                                if (y + 32 * i < yl) {
+                                    sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
+                                    if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
                                 }
+                            }
 #pragma unroll
-                                for (int i = 0; i < 8; ++i)
-                                    if (y + 32 * i < yl) dst[y + 32 * i] = sm[i];
-                            }
-                        } else {
-                            const int is = it - NB;
-                            const int u = is >> 1;
-                            const int nz = nz4s[u];
-                            const int halfq = ((nz >> 1) + 31) & ~31;
-                            int q4 = ((is & 1) ? halfq : 0) + lane;
-                            const int qend = (is & 1) ? nz : (halfq < nz ? halfq : nz);
-                            const ddp_u32* src = (const ddp_u32*)(rbase + (size_t)u * (win + 16));
-                            ddp_u32* dst = ebase + (size_t)u * le;
-                            for (; q4 < qend; q4 += 64) {  // two groups per lane in flight, the second one predicated
-                                const bool two = q4 + 32 < qend;
-                                const ddp_u32 lo = src[q4], hi = src[q4 + hq];
-                                ddp_u32 lo2 = 0u, hi2 = 0u;
-                                if (two) { lo2 = src[q4 + 32]; hi2 = src[q4 + 32 + hq]; }
-                                const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
-                                const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
-                                const ddp_u32 elo2 = lo2 & 0x00ff00ffu, ehi2 = hi2 & 0x00ff00ffu;
-                                const ddp_u32 olo2 = __byte_perm(lo2, 0u, 0x4341u), ohi2 = __byte_perm(hi2, 0u, 0x4341u);
-                                *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
-                                                                     __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
-                                if (two)
-                                    *(uint4*)(dst + 4 * q4 + 128) =
-                                        make_uint4(__byte_perm(elo2, ehi2, 0x5410u), __byte_perm(olo2, ohi2, 0x5410u),
-                                                   __byte_perm(elo2, ehi2, 0x7632u), __byte_perm(olo2, ohi2, 0x7632u));
-                            }
+                            for (int i = 0; i < 8; ++i)
+                                if (y + 32 * i < yl) dst[y + 32 * i] = sm[i];
                         }
                     }
                     rot = rot + 1 < NPW - 1 ? rot + 1 : 0;  // the warp that starts the round changes every iteration
                 }
-                if (vb) {  // this warp's share of buffer (n + 1) & 1 is written
+                if (vb) {  // this warp's share of the chunk's variant rows is written
                     __syncwarp();
                     if (lane == 0) ddp_mbar_arrive(&mfull[xb & (DDP_MRG_DEPTH - 1)]);
                 }
@@ -1051,7 +1023,35 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
         for (int j = 0; j < DPT; ++j)
 #pragma unroll
             for (int k = 0; k < K; ++k) acc[j][k] = 0u;
-        for (int n = 0; n < nstream; ++n) {
+        // Expanding chunk x (raw slot -> E rows: samples (z, z + H) of each channel as 2 x 16-bit lanes) is the consumers'
+        // job too: they would otherwise wait for the producers, whose build is the longer half of an iteration.
+        const int hq = H >> 2;
+        const int epl = NCW > U ? 31 - __clz(NCW / U) : 0;  // log2(warps per channel row)
+        auto expand = [&](int x) {
+            const int* ds = slot(x);
+            ddp_mbar_wait(&mbar[x & 1], (ddp_u32)((x >> 1) & 1));  // raw windows landed (and the chunk's descriptors with them)
+            const int* nz4s = ds + 16 + 3 * U;
+            for (int unit = warp; unit < (U << epl); unit += NCW) {
+                const int u = unit >> epl, part = unit & ((1 << epl) - 1);
+                const int nz = nz4s[u];
+                const ddp_u32* src = (const ddp_u32*)(raw + ((size_t)(x & 1) * U + u) * (win + 16));
+                ddp_u32* dst = ebuf + ((size_t)(x & 1) * U + u) * le + DDP_MRG_EPAD;
+                for (int q4 = (part << 5) + lane; q4 < nz; q4 += 32 << epl) {  // four samples and their partners H later
+                    const ddp_u32 lo = src[q4], hi = src[q4 + hq];
+                    const ddp_u32 elo = lo & 0x00ff00ffu, ehi = hi & 0x00ff00ffu;
+                    const ddp_u32 olo = __byte_perm(lo, 0u, 0x4341u), ohi = __byte_perm(hi, 0u, 0x4341u);
+                    *(uint4*)(dst + 4 * q4) = make_uint4(__byte_perm(elo, ehi, 0x5410u), __byte_perm(olo, ohi, 0x5410u),
+                                                         __byte_perm(elo, ehi, 0x7632u), __byte_perm(olo, ohi, 0x7632u));
+                }
+            }
+            __syncwarp();
+            if (lane == 0) ddp_mbar_arrive(&mexp[x & 1]);
+        };
+        for (int n = -2; n < nstream; ++n) {
+            if (n < 0) {  // the first two chunks are expanded before the first sum
+                if (n + 2 < nstream) expand(n + 2);
+                continue;
+            }
             const int* d = slot(n);
             ddp_mbar_wait_long(&mfull[n & (DDP_MRG_DEPTH - 1)], (ddp_u32)((n / DDP_MRG_DEPTH) & 1));  // variant rows of chunk n are built
             // ---- sum chunk n: every trial adds its variant rows
@@ -1080,6 +1080,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
             const int flags = d[5], tile_t = d[0], tile_dm = d[1], g = d[3];
             __syncwarp();
             if (lane == 0) ddp_mbar_arrive(&mempty[n & (DDP_MRG_DEPTH - 1)]);  // this warp has left the rows of chunk n
+            if (n + 2 < nstream) expand(n + 2);  // its E buffer was last read by the build of chunk n, which is complete
             if (flags & 4) {  // block-uniform: last chunk of the unit -> flush
 #pragma unroll
                 for (int j = 0; j < DPT; ++j) {

@@ -476,7 +476,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += 2 * U * (row + 16);                              // raw
                 b += 2 * NG * (size_t)mg.rw * 4;                      // record staging
                 b += 16 * (((16 + 4 * U + 8 * (size_t)mg.rows_max + TD * NG) + 3) & ~(size_t)3) * 4;  // descriptor ring
-                b += (4 + 2 * 16) * 8 + 128;                          // mbarriers, scheduler state
+                b += (4 + 2 * 16 + 2) * 8 + 128;                      // mbarriers, scheduler state
                 return b;
             }
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar

@@ -1,5 +1,5 @@
-"""Multi-GPU plumbing of the bench: how independent beams are spread over ranks and how per-rank
-device times are combined.  No data-path collective exists (the paper's cluster runs one beam per
+"""Multi-GPU plumbing: how independent beams (the bench) or one beam's DM rows (dm_rows_of_rank / gather_rows) are
+spread over ranks and how per-rank device times are combined.  No data-path collective exists (the paper's cluster runs one beam per
 GPU): ranks only agree on a time (max over ranks) and
 on a unit count (sum over ranks), through `torch.distributed` (NCCL on the GPU box, gloo in the CPU
 tests).  Nothing here computes any part of the search.
@@ -17,6 +17,37 @@ def beams_of_rank(n_beams: int, rank: int, world: int) -> List[int]:
     base, extra = divmod(n_beams, world)
     lo = rank * base + min(rank, extra)
     return list(range(lo, lo + base + (1 if rank < extra else 0)))
+
+
+def dm_rows_of_rank(ndm: int, rank: int, world: int, multiple: int = 1) -> Tuple[int, int]:
+    """[lo, hi) of the DM rows rank `rank` searches when ONE beam's trial list is split over the ranks (SURVEY 8(e):
+    contiguous ranges, so that a rank's delay apron only grows with its own largest DM; 8(f) f3).  `multiple` keeps
+    range boundaries on multiples of a block of rows (e.g. the fine DMs of one coarse DM of a subband plan).  Every
+    row belongs to exactly one rank; sizes differ by at most one block."""
+    if world <= 0 or not (0 <= rank < world) or ndm < 0 or multiple < 1 or ndm % multiple:
+        raise ValueError("bad (ndm, rank, world, multiple) = (%d, %d, %d, %d)" % (ndm, rank, world, multiple))
+    blocks = ndm // multiple
+    base, extra = divmod(blocks, world)
+    lo = rank * base + min(rank, extra)
+    return lo * multiple, (lo + base + (1 if rank < extra else 0)) * multiple
+
+
+def gather_rows(local, ndm: int, device=None):
+    """The [ndm][nW] table of a search whose DM rows were split with dm_rows_of_rank: every rank passes its own rows
+    (a float32 or int32 tensor [hi - lo][nW]); all ranks get the whole table.  This gather of at most a few hundred
+    kilobytes is the only exchange of a DM-sharded search: every rank reads the whole input itself."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return local
+    world = dist.get_world_size()
+    sizes = [dm_rows_of_rank(ndm, r, world)[1] - dm_rows_of_rank(ndm, r, world)[0] for r in range(world)]
+    most = max(sizes)  # all_gather wants equal shapes: pad every rank's rows to the largest share, trim afterwards
+    mine = torch.zeros((most,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
+    mine[: local.shape[0]] = local
+    parts = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine)
+    return torch.cat([p[:n] for p, n in zip(parts, sizes)], dim=0)
 
 
 from synth.filterbank import beam_seed  # noqa: E402,F401  (data recipe: lives with the generator)

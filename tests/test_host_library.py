@@ -359,3 +359,34 @@ def test_compute_calls_fail_loudly_without_a_device():
     with pytest.raises(RuntimeError):
         ddp.alloc_buffers(plan)
     plan.destroy()
+
+
+def test_sliding_mode_and_channel_mask_plans_host_side():
+    """integration_mode = SLIDING and chan_mask as far as the host sees them: geometry, which
+    kernels belong to the plan, validity of the fused kernel's shapes, algorithmic work of a masked plan."""
+    from synth import configs
+    cfg = configs.tiny()
+    plan = ddp.plan_from_config(cfg, integration_mode=1)
+    i = plan.query()
+    assert i.integration_mode == 1 and i.integ_elems == 0
+    assert [i.plane_len[k] for k in range(i.nwidths)] == [cfg.nsamp_out - w + 1 for w in cfg.widths]
+    for k in (ddp.K_INTEGRATE, ddp.K_SNR):                      # the sums are never materialised in this mode
+        with pytest.raises(ddp.DdpError):
+            plan.get_kcfg(k)
+    V = plan.enumerate_kcfgs(ddp.K_ISNR)
+    assert V and all(c.threads_t == 32 and c.staging == 0 and c.unroll == 1 for c in V)
+    plan.compile_kcfg(ddp.K_ISNR, V[0])                         # NVRTC, no GPU needed
+    with pytest.raises(ddp.DdpError):
+        ddp.plan_from_config(cfg, integration_mode=2)
+    plan.destroy()
+    mask = np.ones(cfg.nchan, np.uint8)
+    mask[::4] = 0
+    pm = ddp.plan_from_config(cfg, chan_mask=mask)
+    im, i0 = pm.query(), ddp.plan_from_config(cfg).query()
+    assert im.nchan_masked == cfg.nchan // 4
+    assert im.adds_dedisp == pytest.approx(i0.adds_dedisp * 0.75)
+    assert im.workspace_bytes > i0.workspace_bytes              # row map + zero row
+    assert np.array_equal(pm.get_delays(0), ddp.plan_from_config(cfg).get_delays(0))  # the tables do not change
+    with pytest.raises(ValueError):
+        ddp.plan_from_config(cfg, chan_mask=np.ones(3, np.uint8))
+    pm.destroy()

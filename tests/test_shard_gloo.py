@@ -12,7 +12,7 @@ torch = pytest.importorskip("torch")
 import torch.distributed as dist  # noqa: E402
 import torch.multiprocessing as mp  # noqa: E402
 
-from paper_1811_04165_b200.shard import beam_seed, beams_of_rank, combine  # noqa: E402
+from paper_1811_04165_b200.shard import beam_seed, beams_of_rank, combine, dm_rows_of_rank, gather_rows  # noqa: E402
 
 
 def test_beam_partition_is_exact_and_balanced():
@@ -26,6 +26,21 @@ def test_beam_partition_is_exact_and_balanced():
     with pytest.raises(ValueError):
         beams_of_rank(4, 2, 2)
     assert beam_seed(100, 0) == 100 and len({beam_seed(100, b) for b in range(8)}) == 8
+
+
+def test_dm_row_partition_is_exact_contiguous_and_block_aligned():
+    for world in (1, 2, 3, 8):
+        for ndm, mult in ((2048, 1), (2048, 32), (37, 1), (96, 8), (0, 1)):
+            r = [dm_rows_of_rank(ndm, k, world, mult) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == ndm
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))      # contiguous, every row exactly once
+            assert all(lo % mult == 0 and hi % mult == 0 for lo, hi in r)
+            sizes = [hi - lo for lo, hi in r]
+            assert max(sizes) - min(sizes) <= mult
+    with pytest.raises(ValueError):
+        dm_rows_of_rank(10, 0, 2, 4)
+    t = torch.arange(6.0).reshape(3, 2)
+    assert gather_rows(t, 3) is t                                          # no process group: identity
 
 
 def test_combine_without_process_group_is_identity():
@@ -49,8 +64,12 @@ def _worker(rank, world, port, out):
         local_ms = 10.0 + 5.0 * rank                          # rank 1 is the slower one
         local_units = 1000.0 * len(beams)
         ms, units = combine(local_ms, local_units, torch.device("cpu"))
+        # a DM-sharded search: 5 rows x 3 widths split 3 + 2; row i of the whole table holds i*10 + width index
+        lo, hi = dm_rows_of_rank(5, rank, world)
+        mine = torch.tensor([[10.0 * i + k for k in range(3)] for i in range(lo, hi)], dtype=torch.float32)
+        table = gather_rows(mine, 5)
         dist.barrier()
-        out[rank] = (beams, ms, units)
+        out[rank] = (beams, ms, units, table.tolist())
     finally:
         dist.destroy_process_group()
 
@@ -62,6 +81,7 @@ def test_world_size_two_gloo_agrees_on_max_time_and_summed_units():
     mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
     assert out[0][0] == [0] and out[1][0] == [1]
     for r in range(world):
-        _, ms, units = out[r]
+        _, ms, units, table = out[r]
         assert ms == 15.0                                     # max over ranks, never wall clock of rank 0
         assert units == 2000.0                                # whole-job units
+        assert table == [[10.0 * i + k for k in range(3)] for i in range(5)]   # every rank holds the whole table
