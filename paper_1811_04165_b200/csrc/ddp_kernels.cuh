@@ -796,8 +796,10 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
         if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
         const int ptid = tid - NCT, pwarp = warp - NCW;
         // descriptor roles: TMA extents on producer warp 0, variant rows from warp 1 on, window offsets from warp 2 on
-        const int rB = ptid - 32, sB = NPT - 32, rC = ptid - 64, sC = NPT - 64;
-        int rot = pwarp - 1;  // first item of this warp in the current iteration (warps 1..)
+        // control work: warp 0 schedules, computes the TMA extents and issues the copies; warp 1 turns the records into
+        // row and window descriptors; warps 2.. build, so that none of them starts its items late
+        const int rB = ptid - 32, sB = 32, rC = ptid - 32, sC = 32;
+        int rot = pwarp - 2;  // first item of this warp in the current iteration (warps 2..)
         for (int n = -5; n < nstream; ++n) {
             // ---- schedule chunk n + 5 (one thread; the cursor {unit, chunk, segment, time tile, DM tile, group} lives in shared memory)
             if (ptid == 0) {
@@ -879,7 +881,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                         }
                         if (lane == 0) d[8] = nz4;
                     }
-                    for (int i = rB; i >= 0 && i < NG * VCAP; i += sB) {
+                    for (int i = rB; i >= 0 && i < NG * VCAP && pwarp == 1; i += sB) {
                         const int q = i / VCAP, v = i - q * VCAP;
                         const int* r = rec + q * RW;
                         int base = 0, total = 0, words = 0, ymax = 0;  // base: ring words in front of group q (relative to the chunk's first)
@@ -930,7 +932,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                             }
                         }
                     }
-                    for (int i = rC; i >= 0 && i < TD * NG; i += sC) {
+                    for (int i = rC; i >= 0 && i < TD * NG && pwarp == 1; i += sC) {
                         const int j = i / NG, q = i - j * NG;
                         int base = 0;
 #pragma unroll
@@ -972,12 +974,12 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                     }
                     ddp_mbar_wait(&mexp[xb & 1], (ddp_u32)((xb >> 1) & 1));  // its E rows are there
                 }
-                if (pwarp > 0 && vb) {
+                if (pwarp > 1 && vb) {
                     const int NB = 2 * db[6];  // build items: (variant row, half)
                     const int* rowd = db + 16 + 4 * U;
                     const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
                     ddp_u32* pb = pw + db[11] + lane;
-                    for (int it = rot; it < NB; it += NPW - 1) {
+                    for (int it = rot; it < NB; it += NPW - 2) {
                         const int row = it >> 1;
                         const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
                         const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
@@ -1004,7 +1006,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                                 if (y + 32 * i < yl) dst[y + 32 * i] = sm[i];
                         }
                     }
-                    rot = rot + 1 < NPW - 1 ? rot + 1 : 0;  // the warp that starts the round changes every iteration
+                    rot = rot + 1 < NPW - 2 ? rot + 1 : 0;  // the warp that starts the round changes every iteration
                 }
                 if (vb) {  // this warp's share of the chunk's variant rows is written
                     __syncwarp();
