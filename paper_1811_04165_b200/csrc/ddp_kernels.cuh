@@ -753,7 +753,7 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
     int* sched = (int*)(mexp + 2);                                           // scheduler cursor [8], ring head, extents of the last chunks [2 * AHEAD]
     // ring slot: desc[16] {tile_t, tile_dm, nd, g, r0, flags, nrows, ymax, nzmax, -, -, first word in the variant-row ring,
     //            chunk the consumers must have left before this one is built} | a0[U] | bytes[U] |
-    //            carry[U] | nz4[U] | rowd[rows_max][8] {words, dst, shifts vs the group's first variant, variants, src[4]} | offs[TD][NG]
+    //            carry[U] | nz4[U] | rowd[rows_max][8] {ylen, dst, src[4], -, -} | offs[TD][NG]
     auto slot = [&](int x) -> int* { return ring + (size_t)(x & (DDP_MRG_DEPTH - 1)) * SLOTW; };
 
     // this block's units: a contiguous range, tile-major / segment-minor, so that the segments of a tile
@@ -921,23 +921,15 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
 #pragma unroll
                             for (int qq = 0; qq < NG; ++qq)
                                 if (qq < q) rows_before += rec[qq * RW];
-                            // row descriptor {words, first ring word (relative), shifts against the group's first variant as
-                            // signed bytes, variants of the group, first E word of the G channels}
                             int* o = rowd + (size_t)(rows_before + v) * 8;
-                            const int code0 = r[4 + 2 * G];
-                            int deltas = 0;
                             o[0] = yl;
                             o[1] = base + v * ((yl + 3) & ~3);
 #pragma unroll
                             for (int m = 0; m < G; ++m) {
                                 const int tau = m == 0 ? 0 : (int)(signed char)((code >> (8 * (m - 1))) & 0xff);
-                                const int tau0 = m == 0 ? 0 : (int)(signed char)((code0 >> (8 * (m - 1))) & 0xff);
                                 const int carry = (int)(((long long)tile_t + r[4 + m]) & 15);
-                                o[4 + m] = (q * G + m) * le + DDP_MRG_EPAD + carry + tau;
-                                if (m) deltas |= ((tau - tau0) & 0xff) << (8 * (m - 1));
+                                o[2 + m] = (q * G + m) * le + DDP_MRG_EPAD + carry + tau;
                             }
-                            o[2] = deltas;
-                            o[3] = r[0];
                         }
                     }
                     for (int i = rC; i >= 0 && i < TD * NG && pwarp == 1; i += sC) {
@@ -983,54 +975,36 @@ __device__ __forceinline__ void ddp_dedisp_merge_body(const DdpDedispParams& p) 
                     ddp_mbar_wait(&mexp[xb & 1], (ddp_u32)((xb >> 1) & 1));  // its E rows are there
                 }
                 if (pwarp > 1 && vb) {
-                    // items = (group, block of 64 words of its y range): the G channel words of the group's first variant
-                    // are loaded once, every further variant only reloads the channels whose shift differs from it
+                    const int NB = 2 * db[6];  // build items: (variant row, half)
                     const int* rowd = db + 16 + 4 * U;
                     const ddp_u32* eb = ebuf + (size_t)(xb & 1) * U * le + lane;
                     ddp_u32* pb = pw + db[11] + lane;
-                    const int nblk = (db[7] + 63) >> 6;  // blocks of the longest group
-                    int it = rot, row0 = 0;
-#pragma unroll 1
-                    for (int q = 0; q < NG; ++q) {
-                        const int4 g0 = *(const int4*)(rowd + (size_t)row0 * 8);      // {words, dst, -, variants}
-                        const int4 g1 = *(const int4*)(rowd + (size_t)row0 * 8 + 4);  // first E words of the channels
-                        const int nv = g0.w;
-                        for (; it < (q + 1) * nblk; it += NPW - 2) {
-                            const int y = (it - q * nblk) << 6;
-                            if (y >= g0.x) continue;  // warp-uniform
-                            const bool in0 = y < g0.x - lane, in1 = y + 32 < g0.x - lane;
-                            ddp_u32 e[G][2], s0[2] = {0u, 0u};
+                    for (int it = rot; it < NB; it += NPW - 2) {
+                        const int row = it >> 1;
+                        const int4 d0 = *(const int4*)(rowd + (size_t)row * 8);
+                        const int4 d1 = *(const int4*)(rowd + (size_t)row * 8 + 4);
+                        const int half = ((d0.x >> 1) + 31) & ~31;
+                        int y = (it & 1) ? half : 0;
+                        const int yend = (it & 1) ? d0.x : (half < d0.x ? half : d0.x);
+                        const ddp_u32* e0 = eb + d0.z;
+                        const ddp_u32* e1 = eb + d0.w;
+                        const ddp_u32* e2 = eb + (G > 2 ? d1.x : 0);
+                        const ddp_u32* e3 = eb + (G > 2 ? d1.y : 0);
+                        ddp_u32* dst = pb + d0.y;
+                        const int yl = yend - lane;  // words of this lane's column before the end
+                        for (; y < yend; y += 256) {  // blocks of 256 words, all loads first; the ragged end is predicated
+                            ddp_u32 sm[8];
 #pragma unroll
-                            for (int m = 0; m < G; ++m) {
-                                const ddp_u32* em = eb + (m == 0 ? g1.x : m == 1 ? g1.y : m == 2 ? g1.z : g1.w) + y;
-                                e[m][0] = in0 ? em[0] : 0u;
-                                e[m][1] = in1 ? em[32] : 0u;
-                            }
-#pragma unroll
-                            for (int m = 0; m < G; ++m) { s0[0] += e[m][0]; s0[1] += e[m][1]; }
-                            {
-                                ddp_u32* dst = pb + g0.y + y;
-                                if (in0) dst[0] = s0[0];
-                                if (in1) dst[32] = s0[1];
-                            }
-                            for (int v = 1; v < nv; ++v) {
-                                const int4 dv = *(const int4*)(rowd + (size_t)(row0 + v) * 8);  // {words, dst, shifts, -}
-                                ddp_u32 t0 = s0[0], t1 = s0[1];
-#pragma unroll
-                                for (int m = 1; m < G; ++m) {
-                                    const int dm = (int)(signed char)((dv.z >> (8 * (m - 1))) & 0xff);
-                                    if (dm != 0) {  // warp-uniform: this channel sits at another shift in variant v
-                                        const ddp_u32* em = eb + (m == 1 ? g1.y : m == 2 ? g1.z : g1.w) + dm + y;
-                                        if (in0) t0 += em[0] - e[m][0];
-                                        if (in1) t1 += em[32] - e[m][1];
-                                    }
+                            for (int i = 0; i < 8; ++i) {
+                                if (y + 32 * i < yl) {
+                                    sm[i] = e0[y + 32 * i] + e1[y + 32 * i];
+                                    if constexpr (G > 2) sm[i] += e2[y + 32 * i] + e3[y + 32 * i];
                                 }
-                                ddp_u32* dst = pb + dv.y + y;
-                                if (in0) dst[0] = t0;
-                                if (in1) dst[32] = t1;
                             }
+#pragma unroll
+                            for (int i = 0; i < 8; ++i)
+                                if (y + 32 * i < yl) dst[y + 32 * i] = sm[i];
                         }
-                        row0 += nv;
                     }
                     rot = rot + 1 < NPW - 2 ? rot + 1 : 0;  // the warp that starts the round changes every iteration
                 }
