@@ -1719,6 +1719,24 @@ struct DdpIsnrFold {  // levels M .. log2(SPT) inside one thread; x holds SPT >>
     }
 };
 
+// The same fold when every level is requested and no planes are written (the usual case: widths 1, 2, 4, ... 2^max):
+// no per-level tests and no parameter reads inside the loop.
+template <int SPT, int M, int LVLS>
+struct DdpIsnrFoldDense {
+    template <int NIN>
+    static __device__ __forceinline__ void run(DdpMoments (&mom)[LVLS], const ddp_u32 (&x)[NIN], int t0, ddp_u32& total) {
+        if constexpr (NIN == 1) {
+            total = x[0];
+        } else {
+            ddp_u32 y[NIN / 2];
+#pragma unroll
+            for (int i = 0; i < NIN / 2; ++i) y[i] = x[2 * i] + x[2 * i + 1];
+            ddp_mom_add_full<NIN / 2>(mom[M], y, t0 >> M);
+            DdpIsnrFoldDense<SPT, M + 1, LVLS>::template run<NIN / 2>(mom, y, t0, total);
+        }
+    }
+};
+
 template <int SPT, int DPT>
 __device__ __forceinline__ void ddp_isnr_body(const DdpIsnrParams& p) {
     extern __shared__ __align__(128) unsigned char ddp_smem[];
@@ -1733,6 +1751,10 @@ __device__ __forceinline__ void ddp_isnr_body(const DdpIsnrParams& p) {
     const int nchunks = (p.ns + CH - 1) / CH;
     const int nfull = p.ns / CH;      // chunks wholly inside the series: none of their block sums needs a validity test
     const bool wide = p.max_lvl >= NL;
+    // dense: every level up to the largest width is requested and no planes are written; levels above the largest
+    // width are then accumulated too (a handful of values per chunk) and simply not reported
+    bool dense = p.planes == nullptr;
+    for (int m = 0; m <= p.max_lvl && m < NL; ++m) dense = dense && p.lvl_k[m] >= 0;
 
 #pragma unroll 1
     for (int j = 0; j < DPT; ++j) {
@@ -1769,15 +1791,23 @@ __device__ __forceinline__ void ddp_isnr_body(const DdpIsnrParams& p) {
                 }
             }
         };
-        ddp_u32 xn[SPT];
-        load(0, xn);
-        for (int c = 0; c < nchunks; ++c) {
-            ddp_u32 x[SPT];
-#pragma unroll
-            for (int s = 0; s < SPT; ++s) x[s] = xn[s];
-            if (c + 1 < nchunks) load(c + 1, xn);
+        auto process = [&](int c, const ddp_u32 (&x)[SPT]) {
             const int t0 = c * CH + lane * SPT;
             ddp_u32 v;
+            if (c < nfull && dense) {  // warp-uniform: no tests at all
+                ddp_mom_add_full<SPT>(mom[0], x, t0);
+                DdpIsnrFoldDense<SPT, 1, NL>::template run<SPT>(mom, x, t0, v);
+                s1full += v;
+#pragma unroll
+                for (int l = 1; l <= 5; ++l) {
+                    v += __shfl_xor_sync(0xffffffffu, v, 1 << (l - 1));
+                    if ((lane & ((1 << l) - 1)) == 0) {
+                        const int m = LS + l;
+                        mom[m].s2 += (ddp_u64)v * (ddp_u64)v;
+                        if (v > mom[m].mx) { mom[m].mx = v; mom[m].ix = (ddp_u32)(t0 >> m); }
+                    }
+                }
+            } else
             if (c < nfull) {  // warp-uniform fast path
                 if (p.lvl_k[0] >= 0) ddp_mom_add_full<SPT>(mom[0], x, t0);
                 DdpIsnrFold<SPT, 1, NL, true>::template run<SPT>(p, mom, x, t0, dm, v);
@@ -1837,6 +1867,15 @@ __device__ __forceinline__ void ddp_isnr_body(const DdpIsnrParams& p) {
                     }
                 }
             }
+        };
+        // two chunks per trip, the loads of the next one always in flight (no register copies)
+        ddp_u32 xa[SPT], xb[SPT];
+        load(0, xa);
+        for (int c = 0; c < nchunks; c += 2) {
+            if (c + 1 < nchunks) load(c + 1, xb);
+            process(c, xa);
+            if (c + 2 < nchunks) load(c + 2, xa);
+            if (c + 1 < nchunks) process(c + 1, xb);
         }
         // the plain sum of the full chunks, over the warp: part of every register level's sum
 #pragma unroll
