@@ -96,8 +96,13 @@ typedef struct {
                               search calls run; ddp_integrate, ddp_snr and the tuners return DDP_E_CONFIG         */
     const uint8_t* chan_mask; /* host, nchan bytes or NULL: channels whose byte is 0 are left out of every sum
                               (zapped channels); copied at plan creation                  */
+    int subband_ref;       /* subband plan: frequency the step-2 delays of a subband are computed at (SB.2; the paper
+                              does not say): DDP_SUBREF_TOP (0, default) = its highest channel frequency,
+                              DDP_SUBREF_CENTRE (1) = (highest + lowest channel frequency of the subband) / 2
+                              (SURVEY 8(c) SB.2 alternative, 8(f) f4).  Ignored by a direct plan                  */
 } ddp_options;
 enum { DDP_INTEG_DECIMATE = 0, DDP_INTEG_SLIDING = 1 };
+enum { DDP_SUBREF_TOP = 0, DDP_SUBREF_CENTRE = 1 };
 
 /* Geometry of a plan (all counts in elements unless named *_bytes). */
 typedef struct {
@@ -122,6 +127,7 @@ typedef struct {
                                     255 * channels-per-subband <= 65535 makes that exact, else 4 (SB.4)  */
     int integration_mode;        /* DDP_INTEG_DECIMATE or DDP_INTEG_SLIDING                               */
     int nchan_masked;            /* channels left out by the plan's channel mask                          */
+    int subband_ref;             /* DDP_SUBREF_TOP or DDP_SUBREF_CENTRE (0 for a direct plan)                */
 } ddp_plan_info;
 
 /* ---- plan -------------------------------------------------------------------------------------

@@ -133,14 +133,17 @@ def subband_step2(S: np.ndarray, d2: np.ndarray, ns: int) -> np.ndarray:
     return Y
 
 
-def subband_tables(f_mhz, t_samp_s: float, nsub: int, coarse_dm, fine_dm) -> Tuple[np.ndarray, np.ndarray]:
-    """(d1[ncoarse][nchan], d2[nfine][nsub]) for reading SB.1 "B" with SB.2 (subband reference =
-    highest channel frequency of the subband) -- both tables relative to the global f_ref."""
+def subband_tables(f_mhz, t_samp_s: float, nsub: int, coarse_dm, fine_dm, ref: str = "top") -> Tuple[np.ndarray, np.ndarray]:
+    """(d1[ncoarse][nchan], d2[nfine][nsub]) for reading SB.1 "B" -- both tables relative to the global f_ref.
+    SB.2: the subband reference frequency is its highest channel frequency (ref="top", default) or, reading SB.2c
+    (SURVEY 8(c) SB.2 alternative, 8(f) f4), the centre of the subband, (highest + lowest channel frequency) / 2
+    (ref="centre")."""
     f = np.asarray(f_mhz, dtype=np.float64)
     cps = f.size // nsub
-    assert cps * nsub == f.size
+    assert cps * nsub == f.size and ref in ("top", "centre")
     f_ref = float(f.max())
-    f_sub = f.reshape(nsub, cps).max(axis=1)
+    fs = f.reshape(nsub, cps)
+    f_sub = fs.max(axis=1) if ref == "top" else 0.5 * (fs.max(axis=1) + fs.min(axis=1))
     d1 = delay_table(f, coarse_dm, t_samp_s, f_ref)
     d2 = delay_table(f_sub, fine_dm, t_samp_s, f_ref)
     return d1, d2

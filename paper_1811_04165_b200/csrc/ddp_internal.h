@@ -68,6 +68,7 @@ struct ddp_plan {
     int nsub = 0, ncoarse = 0, nfine = 0, cps = 0;
     double coarse_first = 0, coarse_step = 0, fine_step = 0;
     int ddof = 0, device = 0;
+    int subband_ref = 0;                   // DDP_SUBREF_TOP / DDP_SUBREF_CENTRE (SB.2)
     int integ_mode = 0;                    // DDP_INTEG_DECIMATE / DDP_INTEG_SLIDING
     std::vector<unsigned char> chan_mask;  // empty = every channel used; else nchan bytes, 0 = left out
     std::vector<int32_t> rowmap_host;      // host copy of the row map (outlives the asynchronous upload)

@@ -103,6 +103,7 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
         if (opt->cache_dir) p->cache_dir = opt->cache_dir;
         p->integ_mode = opt->integration_mode;
         if (opt->chan_mask) p->chan_mask.assign(opt->chan_mask, opt->chan_mask + nchan);
+        p->subband_ref = opt->subband_ref;
     }
     auto bail = [&](ddp_status s) {
         delete p;
@@ -140,8 +141,12 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
         if (dm_list)
             for (int i = 0; i < p->ndm; ++i)
                 if (dm_list[i] != p->dms[i]) return bail(DDP_E_ARG);
-        for (int s = 0; s < p->nsub; ++s)  // SB.2: subband reference = its highest channel frequency
-            fsub[s] = *std::max_element(p->freq.begin() + (size_t)s * p->cps, p->freq.begin() + (size_t)(s + 1) * p->cps);
+        if (p->subband_ref != DDP_SUBREF_TOP && p->subband_ref != DDP_SUBREF_CENTRE) return bail(DDP_E_ARG);
+        for (int s = 0; s < p->nsub; ++s) {  // SB.2: subband reference = its highest channel frequency, or its centre
+            const auto b = p->freq.begin() + (size_t)s * p->cps, e = b + p->cps;
+            const double hi = *std::max_element(b, e);
+            fsub[s] = p->subband_ref == DDP_SUBREF_CENTRE ? 0.5 * (hi + *std::min_element(b, e)) : hi;
+        }
         if (!fill_delays(p->freq.data(), nchan, f_ref, A.data(), p->ncoarse, t_samp_s, p->d1, &max_d1)) return bail(DDP_E_ARG);
         if (!fill_delays(fsub.data(), p->nsub, f_ref, F.data(), p->nfine, t_samp_s, p->d2, &max_d2)) return bail(DDP_E_ARG);
         max_delay = max_d1 + max_d2;
@@ -185,6 +190,7 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     // fits 16 bits), which halves its HBM and shared-memory traffic; uint32 otherwise.
     I.sub_elem_bytes = p->subband ? (255 * (int64_t)p->cps <= 65535 ? 2 : 4) : 0;
     I.integration_mode = p->integ_mode;
+    I.subband_ref = p->nsub > 0 ? p->subband_ref : 0;
     I.nchan_masked = 0;
     for (unsigned char m : p->chan_mask) I.nchan_masked += m == 0;
     int64_t off = 0;

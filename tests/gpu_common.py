@@ -125,13 +125,13 @@ def oracle_direct_rows(cfg, X, rows=None):
     return oracle.dedisperse(np.ascontiguousarray(X), delay, cfg.nsamp_out)
 
 
-def oracle_subband(cfg, X, coarse_rows=None):
+def oracle_subband(cfg, X, coarse_rows=None, ref="top"):
     sb = cfg.subband
     A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
     F = sb.fine_step * np.arange(sb.n_fine)
     if coarse_rows is not None:
         A = A[np.asarray(coarse_rows)]
-    d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F)
+    d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F, ref=ref)
     ns1 = cfg.nsamp_out + int(d2.max())
     S = oracle.subband_step1(np.ascontiguousarray(X), d1, sb.n_subbands, ns1)
     Y = oracle.subband_step2(S, d2, cfg.nsamp_out)

@@ -596,6 +596,28 @@ def test_subband_step1_merged_staging(cps, wide):
     g.close()
 
 
+def test_subband_centre_reference_against_the_oracle():
+    """SB.2 alternative: step-2 delays computed at the centre of every subband (option subband_ref = 1).  Only the
+    table changes, so S, Y, the sums and the S/N must equal the oracle run with its own centre-reference table --
+    and Y must differ from the default reading's on this input (the option is really in effect)."""
+    cfg = small_subband(name="centre_sb", nchan=384, nsamp_out=2500, ndm=12 * 16,
+                        subband=SubbandPlan(n_subbands=8, n_coarse=12, coarse_first=0.0, coarse_step=16.0,
+                                            n_fine=16, fine_step=1.0))
+    g = GpuSearch(cfg, subband_ref=1)
+    assert g.info.subband_ref == 1
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X, ref="centre")
+    assert np.array_equal(g.subband_intermediate(), So[:, :, : g.info.nsamp_sub])
+    compare_all(g, Yo, what="centre reference")
+    g2 = GpuSearch(cfg)
+    assert g2.info.subband_ref == 0 and g2.info.max_d2 < g.info.max_d2
+    assert not np.array_equal(g2.plan.get_delays(2), g.plan.get_delays(2))
+    g2.run_all()
+    compare_all(g2, oracle_subband(cfg, g2.X)[1], what="top reference")
+    g2.close()
+    g.close()
+
+
 @pytest.mark.parametrize("nchan", [320, 512])
 def test_direct_wide_reduction_sweep_and_saturation(nchan):
     """More than 257 channels: the packed kernel flushes its 16-bit lanes every 256 rows (WIDE), with a

@@ -123,6 +123,33 @@ def test_subband_plan_tables_equal_oracle_tables():
     plan.destroy()
 
 
+def test_subband_centre_reference_plan_tables_equal_oracle_tables():
+    """SB.2 alternative (SURVEY 8(f) f4): subband_ref = 1 computes the step-2 delays at the centre of every subband;
+    (a lower frequency than its top channel, so the delays grow: max 172 instead of 168 samples at BJ:cfg2);
+    step 1 is untouched; a direct plan ignores the option; an unknown value is refused."""
+    cfg = configs.apertif_subband()
+    sb = cfg.subband
+    A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+    F = sb.fine_step * np.arange(sb.n_fine)
+    d1o, d2o = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, sb.n_subbands, A, F, ref="centre")
+    plan = ddp.plan_from_config(cfg, cache_dir=None, subband_ref=1)
+    i = plan.query()
+    assert i.subband_ref == 1
+    assert np.array_equal(plan.get_delays(1), d1o)
+    assert np.array_equal(plan.get_delays(2), d2o)
+    assert (i.max_d1, i.max_d2) == (int(d1o.max()), int(d2o.max()))
+    assert i.max_d2 == 172 and i.nsamp_sub == cfg.nsamp_out + i.max_d2
+    plan.destroy()
+    top = ddp.plan_from_config(cfg, cache_dir=None)
+    assert top.query().subband_ref == 0 and top.query().max_d2 == 168
+    top.destroy()
+    pd = ddp.plan_from_config(configs.tiny(), cache_dir=None, subband_ref=1)
+    assert pd.query().subband_ref == 0
+    pd.destroy()
+    with pytest.raises(ddp.DdpError):
+        ddp.plan_from_config(cfg, cache_dir=None, subband_ref=2)
+
+
 def test_plan_create_rejects_bad_arguments():
     f = np.array([1500.0, 1400.0, 1300.0, 1200.0])
     ok = dict(chan_freq_mhz=f, t_samp_s=1e-3, dm_list=[0.0, 10.0], widths=[1, 2], nsamp_out=64, cache_dir=None)

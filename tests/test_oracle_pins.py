@@ -271,6 +271,35 @@ def test_subband_cfg2_geometry():
     assert (err[::sb.n_fine] == 0).all()
 
 
+def test_subband_centre_reference_tables():
+    """Reading SB.2c (subband reference = centre of the subband): only the step-2 table changes; with one channel
+    per subband the centre IS the channel, so it equals the default; at BJ:cfg2 the per-channel total delay then
+    differs from direct by -5..+4 samples instead of -8..+1 (computed there independently), and
+    a closed-form entry checks the frequency that is used."""
+    cfg = configs.apertif_subband()
+    sb = cfg.subband
+    A = sb.coarse_first + sb.coarse_step * np.arange(sb.n_coarse)
+    F = sb.fine_step * np.arange(sb.n_fine)
+    f = cfg.chan_freq_mhz()
+    d1t, d2t = oracle.subband_tables(f, cfg.t_samp_s, sb.n_subbands, A, F)
+    d1c, d2c = oracle.subband_tables(f, cfg.t_samp_s, sb.n_subbands, A, F, ref="centre")
+    assert np.array_equal(d1c, d1t) and not np.array_equal(d2c, d2t)
+    direct = oracle.delay_table(f, cfg.dm_list(), cfg.t_samp_s)
+    cps = cfg.nchan // sb.n_subbands
+    tot = (d1c[:, None, :] + np.repeat(d2c, cps, axis=1)[None, :, :]).reshape(cfg.ndm, cfg.nchan)
+    err = tot.astype(np.int64) - direct
+    assert err.min() == -5 and err.max() == 4
+    # closed form: last subband, largest fine offset, centre of its 48 channels
+    fs = f.reshape(sb.n_subbands, cps)[-1]
+    fc = 0.5 * (fs.max() + fs.min())
+    x = ((K * F[-1]) * (1.0 / (fc * fc) - 1.0 / (f.max() * f.max()))) / cfg.t_samp_s
+    assert d2c[-1, -1] == math.floor(x + 0.5)
+    # one channel per subband: centre == the channel
+    a1, a2 = oracle.subband_tables(f[:16], cfg.t_samp_s, 16, A[:3], F[:5])
+    b1, b2 = oracle.subband_tables(f[:16], cfg.t_samp_s, 16, A[:3], F[:5], ref="centre")
+    assert np.array_equal(a1, b1) and np.array_equal(a2, b2)
+
+
 # ----------------------------------------------------------------------------- INT
 def test_integrate_invariants():
     rng = np.random.default_rng(31)
