@@ -100,6 +100,11 @@ typedef struct {
                               does not say): DDP_SUBREF_TOP (0, default) = its highest channel frequency,
                               DDP_SUBREF_CENTRE (1) = (highest + lowest channel frequency of the subband) / 2
                               (SURVEY 8(c) SB.2 alternative, 8(f) f4).  Ignored by a direct plan                  */
+    int input_bits;        /* bits per input sample (P:90 INPUT_BITS): 0 or 8 = unsigned 8-bit (default, DD.6), 16 =
+                              unsigned 16-bit.  With 16 every `uint8_t* in` argument of this header
+                              points at uint16 elements, strides stay in ELEMENTS, sums stay uint32 (plan creation
+                              proves 65535 * nchan * max width < 2^32), the subband intermediate is uint32, and the
+                              merged staging genes (3, 4) are not valid                                           */
 } ddp_options;
 enum { DDP_INTEG_DECIMATE = 0, DDP_INTEG_SLIDING = 1 };
 enum { DDP_SUBREF_TOP = 0, DDP_SUBREF_CENTRE = 1 };
@@ -128,6 +133,7 @@ typedef struct {
     int integration_mode;        /* DDP_INTEG_DECIMATE or DDP_INTEG_SLIDING                               */
     int nchan_masked;            /* channels left out by the plan's channel mask                          */
     int subband_ref;             /* DDP_SUBREF_TOP or DDP_SUBREF_CENTRE (0 for a direct plan)                */
+    int input_bits;              /* 8 or 16: width of one input sample                                       */
 } ddp_plan_info;
 
 /* ---- plan -------------------------------------------------------------------------------------

@@ -90,13 +90,14 @@ def delay_table(f_mhz, dm, t_samp_s: float, f_ref_mhz: Optional[float] = None) -
 
 
 def dedisperse(X: np.ndarray, delay: np.ndarray, ns: int) -> np.ndarray:
-    """uint32 [nrows][ns] for the delay rows given (X: uint8 [nchan][in_stride])."""
-    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    """uint32 [nrows][ns] for the delay rows given (X: uint8, or uint16 for INPUT_BITS = 16, [nchan][in_stride])."""
+    assert X.dtype in (np.uint8, np.uint16) and X.ndim == 2 and X.flags.c_contiguous
     delay = np.ascontiguousarray(delay, dtype=np.int32)
     nrows, nchan = delay.shape
     assert nchan == X.shape[0]
     Y = np.empty((nrows, ns), dtype=np.uint32)
-    rc = _load().oracle_dedisperse(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), _p(delay),
+    fn = _load().oracle_dedisperse if X.dtype == np.uint8 else _load().oracle_dedisperse_u16
+    rc = fn(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]), _p(delay),
                                    ctypes.c_int(nrows), ctypes.c_int(ns), _p(Y), ctypes.c_size_t(ns))
     if rc != 0:
         raise ValueError("oracle_dedisperse rc=%d (input too short for the delays?)" % rc)
@@ -104,12 +105,13 @@ def dedisperse(X: np.ndarray, delay: np.ndarray, ns: int) -> np.ndarray:
 
 
 def subband_step1(X: np.ndarray, d1: np.ndarray, nsub: int, ns1: int) -> np.ndarray:
-    """uint32 S[ncoarse][nsub][ns1]."""
-    assert X.dtype == np.uint8 and X.ndim == 2 and X.flags.c_contiguous
+    """uint32 S[ncoarse][nsub][ns1] (X: uint8, or uint16 for INPUT_BITS = 16)."""
+    assert X.dtype in (np.uint8, np.uint16) and X.ndim == 2 and X.flags.c_contiguous
     d1 = np.ascontiguousarray(d1, dtype=np.int32)
     ncoarse, nchan = d1.shape
     S = np.empty((ncoarse, nsub, ns1), dtype=np.uint32)
-    rc = _load().oracle_subband_step1(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]),
+    fn = _load().oracle_subband_step1 if X.dtype == np.uint8 else _load().oracle_subband_step1_u16
+    rc = fn(_p(X), ctypes.c_int(nchan), ctypes.c_size_t(X.shape[1]),
                                       ctypes.c_int(nsub), _p(d1), ctypes.c_int(ncoarse), ctypes.c_int(ns1),
                                       _p(S), ctypes.c_size_t(ns1))
     if rc != 0:

@@ -173,6 +173,42 @@ int oracle_dedisperse_masked(const uint8_t* X, int nchan, size_t in_stride, cons
     return 0;
 }
 
+// INPUT_BITS = 16 (P:90 lists the sample width as a parameter of the setup): the same two sums over
+// unsigned 16-bit samples.  Nothing else changes: uint32 totals, same delays, same ranges.
+int oracle_dedisperse_u16(const uint16_t* X, int nchan, size_t in_stride, const int32_t* delay, int nrows, int ns,
+                          uint32_t* Y, size_t out_stride) {
+    for (int i = 0; i < nrows; ++i) {
+        uint32_t* y = Y + (size_t)i * out_stride;
+        for (int t = 0; t < ns; ++t) y[t] = 0u;
+        for (int c = 0; c < nchan; ++c) {
+            const int32_t d = delay[(size_t)i * nchan + c];
+            if (d < 0 || (size_t)d + (size_t)ns > in_stride) return -2;
+            const uint16_t* x = X + (size_t)c * in_stride + d;
+            for (int t = 0; t < ns; ++t) y[t] += (uint32_t)x[t];
+        }
+    }
+    return 0;
+}
+int oracle_subband_step1_u16(const uint16_t* X, int nchan, size_t in_stride, int nsub, const int32_t* d1, int ncoarse,
+                             int ns1, uint32_t* S, size_t s_stride) {
+    if (nsub <= 0 || nchan % nsub != 0) return -1;
+    const int cps = nchan / nsub;
+    for (int a = 0; a < ncoarse; ++a) {
+        for (int s = 0; s < nsub; ++s) {
+            uint32_t* out = S + ((size_t)a * nsub + s) * s_stride;
+            for (int t = 0; t < ns1; ++t) out[t] = 0u;
+            for (int k = 0; k < cps; ++k) {
+                const int c = s * cps + k;
+                const int32_t d = d1[(size_t)a * nchan + c];
+                if (d < 0 || (size_t)d + (size_t)ns1 > in_stride) return -2;
+                const uint16_t* x = X + (size_t)c * in_stride + d;
+                for (int t = 0; t < ns1; ++t) out[t] += (uint32_t)x[t];
+            }
+        }
+    }
+    return 0;
+}
+
 // SNR ("signal-to-noise (S/N) computation"; definition BJ cfg0; readings SNR.1-SNR.4):
 //   over the n values v_j of one (DM, width) series:
 //   mean = (sum v_j)/n;  var = sum (v_j - mean)^2 / (n - ddof);  snr = (max - mean)/sqrt(var)

@@ -30,7 +30,7 @@ def plan_from_config(cfg, **kw) -> Plan:
 
 def alloc_buffers(plan: Plan, device="cuda:0", bind: bool = True) -> dict:
     """Device buffers of one search, allocated with PyTorch (the library never allocates):
-    d_in uint8 [nchan][in_stride], d_out int32-typed uint32 [ndm][out_stride], d_integ [integ_elems],
+    d_in uint8 (int16-typed uint16 for a 16-bit plan) [nchan][in_stride], d_out int32-typed uint32 [ndm][out_stride], d_integ [integ_elems],
     d_snr float32 [ndm][nwidths], d_argmax [ndm][nwidths], workspace (delay tables + subband buffer)."""
     import torch
     if not torch.cuda.is_available():
@@ -38,7 +38,7 @@ def alloc_buffers(plan: Plan, device="cuda:0", bind: bool = True) -> dict:
     i = plan.query()
     dev = torch.device(device)
     b = {
-        "d_in": torch.zeros((i.nchan, i.in_stride_min), dtype=torch.uint8, device=dev),
+        "d_in": torch.zeros((i.nchan, i.in_stride_min), dtype=torch.uint8 if i.input_bits == 8 else torch.int16, device=dev),
         "d_out": torch.zeros((i.ndm, i.out_stride_min), dtype=torch.int32, device=dev),
         "d_integ": torch.zeros((max(1, i.integ_elems),), dtype=torch.int32, device=dev),
         "d_snr": torch.zeros((i.ndm, i.nwidths), dtype=torch.float32, device=dev),

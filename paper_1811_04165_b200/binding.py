@@ -59,7 +59,7 @@ class Options(C.Structure):
     _fields_ = [("n_subbands", C.c_int), ("n_coarse", C.c_int), ("coarse_dm_first", C.c_double),
                 ("coarse_dm_step", C.c_double), ("n_fine", C.c_int), ("fine_dm_step", C.c_double),
                 ("snr_ddof", C.c_int), ("device", C.c_int), ("cache_dir", C.c_char_p), ("integration_mode", C.c_int),
-                ("chan_mask", C.c_void_p), ("subband_ref", C.c_int)]
+                ("chan_mask", C.c_void_p), ("subband_ref", C.c_int), ("input_bits", C.c_int)]
 
 
 class PlanInfo(C.Structure):
@@ -72,7 +72,7 @@ class PlanInfo(C.Structure):
                 ("plane_stride", C.c_int64 * DDP_MAX_WIDTHS), ("plane_offset", C.c_int64 * DDP_MAX_WIDTHS),
                 ("integ_elems", C.c_int64), ("workspace_bytes", C.c_int64), ("adds_dedisp", C.c_double),
                 ("sub_elem_bytes", C.c_int), ("integration_mode", C.c_int), ("nchan_masked", C.c_int),
-                ("subband_ref", C.c_int)]
+                ("subband_ref", C.c_int), ("input_bits", C.c_int)]
 
 
 FITNESS_FN = C.CFUNCTYPE(C.c_double, C.c_void_p, C.POINTER(Kcfg))
@@ -356,7 +356,7 @@ def plan_create(chan_freq_mhz, t_samp_s: float, dm_list, widths, nsamp_out: int,
                 n_coarse: int = 0, coarse_dm_first: float = 0.0, coarse_dm_step: float = 0.0, n_fine: int = 0,
                 fine_dm_step: float = 0.0, snr_ddof: int = 0, device: int = 0,
                 cache_dir: Optional[str] = KCACHE_DIR, integration_mode: int = 0, chan_mask=None,
-                subband_ref: int = 0) -> Plan:
+                subband_ref: int = 0, input_bits: int = 8) -> Plan:
     f = np.ascontiguousarray(chan_freq_mhz, dtype=np.float64)
     w = np.ascontiguousarray(widths, dtype=np.int32)
     dm = None if dm_list is None else np.ascontiguousarray(dm_list, dtype=np.float64)
@@ -367,7 +367,7 @@ def plan_create(chan_freq_mhz, t_samp_s: float, dm_list, widths, nsamp_out: int,
         raise ValueError("chan_mask needs one byte per channel")
     opt = Options(n_subbands, n_coarse, coarse_dm_first, coarse_dm_step, n_fine, fine_dm_step, snr_ddof, device,
                   cache_dir.encode() if cache_dir else None, int(integration_mode),
-                  None if mask is None else mask.ctypes.data, int(subband_ref))
+                  None if mask is None else mask.ctypes.data, int(subband_ref), int(input_bits))
     h = C.c_void_p()
     st = lib().ddp_plan_create(C.byref(h), f.ctypes.data, f.size, float(t_samp_s),
                                None if dm is None else dm.ctypes.data, 0 if dm is None else dm.size,

@@ -35,7 +35,7 @@ struct DdpKGeom {
     int ns_k;      // time-axis length the kernel tiles
     int ndm_k;     // DM-axis length the kernel tiles
     int nred;      // reduction trip count (0 = no reduction loop rule)
-    int in_bytes;  // bytes per input element (1 or 4)
+    int in_bytes;  // bytes per input element (1, 2 or 4)
 };
 
 struct DdpCompiled;  // runtime kernel handle (ddp_rt.cpp)
@@ -69,6 +69,7 @@ struct ddp_plan {
     double coarse_first = 0, coarse_step = 0, fine_step = 0;
     int ddof = 0, device = 0;
     int subband_ref = 0;                   // DDP_SUBREF_TOP / DDP_SUBREF_CENTRE (SB.2)
+    int in_bytes = 1;                      // bytes per input sample: 1 (uint8, DD.6) or 2 (uint16, INPUT_BITS = 16)
     int integ_mode = 0;                    // DDP_INTEG_DECIMATE / DDP_INTEG_SLIDING
     std::vector<unsigned char> chan_mask;  // empty = every channel used; else nchan bytes, 0 = left out
     std::vector<int32_t> rowmap_host;      // host copy of the row map (outlives the asynchronous upload)

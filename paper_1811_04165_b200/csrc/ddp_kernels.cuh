@@ -1182,7 +1182,6 @@ __device__ __forceinline__ void ddp_dedisp_packed16_body(const DdpDedispParams& 
     const int tile_t = blockIdx.x * TT;
     const int tile_dm = blockIdx.y * TD;
     const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
-    const ddp_u16* in_g = (const ddp_u16*)p.in + (ddp_i64)g * p.in_group_stride;
     const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
     const int winw = p.win >> 1;             // words per staged row copy (multiple of 4)
     const int nredp = (p.nred + 3) & ~3;
@@ -1211,8 +1210,8 @@ __device__ __forceinline__ void ddp_dedisp_packed16_body(const DdpDedispParams& 
         if (lane == 0) ddp_mbar_expect_tx(&mbar[b], total);
         __syncwarp();
         if (bytes)
-            ddp_bulk_g2s(copies + ((size_t)b * U + lane) * 2 * winw, in_g + (ddp_i64)(c * U + lane) * p.in_row_stride + a0,
-                         bytes, &mbar[b]);
+            ddp_bulk_g2s(copies + ((size_t)b * U + lane) * 2 * winw, ddp_in_row<ddp_u16>(p, g, c * U + lane) + a0, bytes,
+                         &mbar[b]);
     };
     // chunk c in buffer b: copy 1 from copy 0 (TMA), or both copies from global memory
     const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
@@ -1226,7 +1225,7 @@ __device__ __forceinline__ void ddp_dedisp_packed16_body(const DdpDedispParams& 
             ddp_u32* d0 = cb + (size_t)u * 2 * winw;
             const ddp_u32* src;
             if constexpr (STAGING == 2) src = d0;
-            else src = (const ddp_u32*)(in_g + (ddp_i64)(c * U + u) * p.in_row_stride + a0);
+            else src = (const ddp_u32*)(ddp_in_row<ddp_u16>(p, g, c * U + u) + a0);
             for (int v = ((part << 5) + lane) * VW; v + VW < lenw; v += (32 << parts_log2) * VW)
                 ddp_shift16_store<VW, STAGING == 1>(src + v, d0 + v, d0 + winw + v);
         }

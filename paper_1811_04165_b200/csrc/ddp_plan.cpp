@@ -104,6 +104,11 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
         p->integ_mode = opt->integration_mode;
         if (opt->chan_mask) p->chan_mask.assign(opt->chan_mask, opt->chan_mask + nchan);
         p->subband_ref = opt->subband_ref;
+        if (opt->input_bits != 0 && opt->input_bits != 8 && opt->input_bits != 16) {
+            delete p;
+            return DDP_E_ARG;
+        }
+        p->in_bytes = opt->input_bits == 16 ? 2 : 1;
     }
     auto bail = [&](ddp_status s) {
         delete p;
@@ -164,9 +169,16 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
 
     // Overflow proofs (INT.5): uint32 sums and uint64 second moments must be exact.
     const int wmax = widths[nwidths - 1];
-    if ((long double)255.0L * nchan * wmax >= 4294967296.0L) return bail(DDP_E_OVERFLOW);
-    if ((long double)255.0L * nchan * 255.0L * nchan * wmax * nsamp_out >= 18446744073709551616.0L)
-        return bail(DDP_E_OVERFLOW);
+    const long double vmax = p->in_bytes == 2 ? 65535.0L : 255.0L;  // largest input sample
+    if (vmax * nchan * wmax >= 4294967296.0L) return bail(DDP_E_OVERFLOW);
+    if (p->integ_mode == DDP_INTEG_SLIDING) {
+        // ns - w + 1 window sums of at most vmax * nchan * w each: their sum fits 64 bits, their squares' sum the
+        // sliding kernel's 96 bits (DdpSlideMom)
+        if (vmax * nchan * wmax * nsamp_out >= 18446744073709551616.0L) return bail(DDP_E_OVERFLOW);
+        if (vmax * nchan * vmax * nchan * wmax * wmax * nsamp_out >= 79228162514264337593543950336.0L) return bail(DDP_E_OVERFLOW);
+    } else if (vmax * nchan * vmax * nchan * wmax * nsamp_out >= 18446744073709551616.0L) {
+        return bail(DDP_E_OVERFLOW);  // floor(ns / w) block sums of at most vmax * nchan * w: squares in 64 bits
+    }
 
     ddp_plan_info& I = p->info;
     std::memset(&I, 0, sizeof(I));
@@ -188,7 +200,8 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     I.sub_stride = p->subband ? round_up(I.nsamp_sub + 32, 32) : 0;
     // SB.4: the intermediate is stored as uint16 whenever that is exact (255 * channels per subband
     // fits 16 bits), which halves its HBM and shared-memory traffic; uint32 otherwise.
-    I.sub_elem_bytes = p->subband ? (255 * (int64_t)p->cps <= 65535 ? 2 : 4) : 0;
+    I.sub_elem_bytes = p->subband ? (p->in_bytes == 1 && 255 * (int64_t)p->cps <= 65535 ? 2 : 4) : 0;
+    I.input_bits = 8 * p->in_bytes;
     I.integration_mode = p->integ_mode;
     I.subband_ref = p->nsub > 0 ? p->subband_ref : 0;
     I.nchan_masked = 0;
@@ -213,7 +226,7 @@ extern "C" ddp_status ddp_plan_create(ddp_plan** out, const double* chan_freq_mh
     // region for the resident merged-staging table (one (kernel, TD, G) at a time; DdpMergeTable)
     p->merge_capacity = round_up(2 * (int64_t)(p->subband ? p->d1.size() : p->delay.size()) * 4 + (1 << 20), 256);
     // channel mask: row map (one int per channel) and the row of zeros a masked channel reads
-    const int64_t mbytes = p->chan_mask.empty() ? 0 : round_up((int64_t)nchan * 4, 256) + round_up(I.in_stride_min, 256);
+    const int64_t mbytes = p->chan_mask.empty() ? 0 : round_up((int64_t)nchan * 4, 256) + round_up(I.in_stride_min * p->in_bytes, 256);
     I.workspace_bytes = tbytes + sbytes + p->merge_capacity + mbytes + 256;
     const double nused = (double)(nchan - I.nchan_masked);  // masked channels are not part of the algorithmic work
     I.adds_dedisp = p->subband ? (double)p->ncoarse * nused * (double)I.nsamp_sub + (double)p->ndm * p->nsub * nsamp_out
@@ -271,8 +284,8 @@ ddp_kernel ddp_slot_kernel(const ddp_plan* p, int slot) {
 DdpKGeom ddp_kgeom(const ddp_plan* p, ddp_kernel k) {
     DdpKGeom g{p->ns, p->ndm, 0, 4};
     switch (k) {
-        case DDP_K_DIRECT: g = {p->ns, p->ndm, p->nchan, 1}; break;
-        case DDP_K_SUB1: g = {(int)p->info.nsamp_sub, p->ncoarse, p->cps, 1}; break;
+        case DDP_K_DIRECT: g = {p->ns, p->ndm, p->nchan, p->in_bytes}; break;
+        case DDP_K_SUB1: g = {(int)p->info.nsamp_sub, p->ncoarse, p->cps, p->in_bytes}; break;
         case DDP_K_SUB2: g = {p->ns, p->nfine, p->nsub, p->info.sub_elem_bytes}; break;
         default: break;
     }

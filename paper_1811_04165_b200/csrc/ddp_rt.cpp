@@ -230,7 +230,7 @@ enum CodeKind { CK_DEDISP_U8 = 0, CK_DEDISP_U32 = 1, CK_INTEG = 2, CK_SNR = 3, C
 CodeKind code_kind(const ddp_plan* p, ddp_kernel k) {
     switch (k) {
         case DDP_K_DIRECT:
-        case DDP_K_SUB1: return CK_DEDISP_U8;
+        case DDP_K_SUB1: return p->in_bytes == 2 ? CK_DEDISP_U16 : CK_DEDISP_U8;  // INPUT_BITS = 16: the uint16 code shapes
         case DDP_K_SUB2: return p->info.sub_elem_bytes == 2 ? CK_DEDISP_U16 : CK_DEDISP_U32;
         case DDP_K_INTEGRATE: return CK_INTEG;
         case DDP_K_ISNR: return CK_ISNR;
@@ -258,7 +258,7 @@ int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
     if (ck == CK_DEDISP_U8 && ddp_u8_single_buffered(p, k, c)) f |= 16;
     if (ck == CK_DEDISP_U8 && ddp_merge_group(c) && c.threads_t * c.threads_dm >= 512) f |= 32;  // REGSPLIT
-    if (ck == CK_DEDISP_U16 && c.staging != 0) {
+    if (ck == CK_DEDISP_U16 && c.staging != 0 && k == DDP_K_SUB2) {  // uint16 INPUT samples can be 65535: no lane sums there
         const int64_t room = 65535 / (255 * (int64_t)p->cps);
         f |= (room >= 4 ? 2 : (room >= 2 ? 1 : 0)) << 2;
     }
@@ -658,7 +658,8 @@ extern "C" ddp_status ddp_plan_bind_workspace(ddp_plan* plan, void* d_workspace,
         r = upload(plan->rowmap_host, &plan->d_rowmap);
         plan->d_zero_row = (unsigned char*)(base + off);
         if (r == CUDA_SUCCESS)
-            r = g_api.p_cuMemsetD32Async((CUdeviceptr)plan->d_zero_row, 0u, (size_t)round_up64(plan->info.in_stride_min, 256) / 4,
+            r = g_api.p_cuMemsetD32Async((CUdeviceptr)plan->d_zero_row, 0u,
+                                         (size_t)round_up64(plan->info.in_stride_min * plan->in_bytes, 256) / 4,
                                          (CUstream)stream);
     }
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "delay table upload: " + cu_err(r));
@@ -1026,7 +1027,7 @@ extern "C" ddp_status ddp_search_host(ddp_plan* plan, const uint8_t* h_in, size_
     ddp_status s = ensure_ctx(plan, plan->device);
     if (s != DDP_OK) return s;
     CUstream st = (CUstream)stream;
-    CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)d_in, h_in, in_stride * (size_t)plan->nchan, st);
+    CUresult r = g_api.p_cuMemcpyHtoDAsync((CUdeviceptr)d_in, h_in, in_stride * (size_t)plan->nchan * (size_t)plan->in_bytes, st);
     if (r != CUDA_SUCCESS) return ddp_fail(plan, DDP_E_CUDA, "H2D copy: " + cu_err(r));
     if ((s = ddp_dedisperse(plan, d_in, in_stride, d_out, out_stride, stream)) != DDP_OK) return s;
     if (d_integ && plan->integ_mode == DDP_INTEG_DECIMATE) {
@@ -1058,7 +1059,7 @@ extern "C" ddp_status ddp_search_host_batches(ddp_plan* plan, const uint8_t* h_i
     ddp_status s = ensure_ctx(plan, plan->device);
     if (s != DDP_OK) return s;
     const ddp_plan_info& I = plan->info;
-    const size_t ns = (size_t)plan->ns, carry = (size_t)I.max_delay;
+    const size_t ns = (size_t)plan->ns, carry = (size_t)I.max_delay, eb = (size_t)plan->in_bytes;  // eb: bytes per sample
     if (h_stride < (size_t)nbatches * ns + carry) return ddp_fail(plan, DDP_E_SHAPE, "h_stride shorter than nbatches * nsamp_out + max_delay");
     if ((s = check_io_dedisp(plan, d_in0, in_stride, d_out, out_stride)) != DDP_OK) return s;
     if ((uintptr_t)d_in1 & 15u) return ddp_fail(plan, DDP_E_SHAPE, "d_in1 misaligned");
@@ -1079,11 +1080,11 @@ extern "C" ddp_status ddp_search_host_batches(ddp_plan* plan, const uint8_t* h_i
         std::memset(&c, 0, sizeof c);
         if (from_host) { c.srcMemoryType = CU_MEMORYTYPE_HOST; c.srcHost = src; }
         else { c.srcMemoryType = CU_MEMORYTYPE_DEVICE; c.srcDevice = (CUdeviceptr)src; }
-        c.srcPitch = spitch;
+        c.srcPitch = spitch * eb;
         c.dstMemoryType = CU_MEMORYTYPE_DEVICE;
         c.dstDevice = (CUdeviceptr)dst;
-        c.dstPitch = in_stride;
-        c.WidthInBytes = width;
+        c.dstPitch = in_stride * eb;
+        c.WidthInBytes = width * eb;
         c.Height = (size_t)plan->nchan;
         return g_api.p_cuMemcpy2DAsync(&c, cs);
     };
@@ -1097,8 +1098,8 @@ extern "C" ddp_status ddp_search_host_batches(ddp_plan* plan, const uint8_t* h_i
         if (b == 0) {
             r = copy2d(true, h_in, h_stride, cur, ns + carry);
         } else {  // carried samples from the other buffer (device to device), then the new ones
-            if (carry) r = copy2d(false, d_in[(b - 1) & 1] + ns, in_stride, cur, carry);
-            if (r == CUDA_SUCCESS) r = copy2d(true, h_in + (size_t)b * ns + carry, h_stride, cur + carry, ns);
+            if (carry) r = copy2d(false, d_in[(b - 1) & 1] + ns * eb, in_stride, cur, carry);
+            if (r == CUDA_SUCCESS) r = copy2d(true, h_in + ((size_t)b * ns + carry) * eb, h_stride, cur + carry * eb, ns);
         }
         if (r == CUDA_SUCCESS) r = g_api.p_cuEventRecord(R->ev_in[b & 1], cs);
         if (r == CUDA_SUCCESS) r = g_api.p_cuStreamWaitEvent(st, R->ev_in[b & 1], 0);

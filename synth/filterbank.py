@@ -121,11 +121,21 @@ def pulse_track(cfg: SearchConfig, pulse: Pulse) -> np.ndarray:
 
 
 def make_filterbank(cfg: SearchConfig, nsamp_in: int, in_stride: int = None,
-                    chunk: int = 64) -> Tuple[np.ndarray, List[Pulse]]:
-    """uint8 [nchan][in_stride] (time fastest; columns >= nsamp_in are zero padding)."""
+                    chunk: int = 64, bits: int = 8) -> Tuple[np.ndarray, List[Pulse]]:
+    """uint8 [nchan][in_stride] (time fastest; columns >= nsamp_in are zero padding).
+    bits = 16 (INPUT_BITS = 16): uint16 samples whose high byte is the 8-bit recipe (noise and
+    pulses) and whose low byte is a second noise stream of the same recipe (seed + 0x10001), zero in the padding."""
     if in_stride is None:
         in_stride = nsamp_in
-    assert in_stride >= nsamp_in
+    assert in_stride >= nsamp_in and bits in (8, 16)
+    if bits == 16:
+        hi, pulses = make_filterbank(cfg, nsamp_in, in_stride, chunk)
+        X16 = hi.astype(np.uint16) << np.uint16(8)
+        lo_seed = cfg.seed + 0x10001
+        for c0 in range(0, cfg.nchan, chunk):
+            c1 = min(cfg.nchan, c0 + chunk)
+            X16[c0:c1, :nsamp_in] |= noise_rows(lo_seed, c0, c1, nsamp_in).astype(np.uint16)
+        return X16, pulses
     X = np.zeros((cfg.nchan, in_stride), dtype=np.uint8)
     for c0 in range(0, cfg.nchan, chunk):
         c1 = min(cfg.nchan, c0 + chunk)

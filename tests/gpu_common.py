@@ -41,11 +41,11 @@ class GpuSearch:
         self.buf = ddp.alloc_buffers(self.plan, device)
         i = self.info
         if X is None:
-            X, self.pulses = filterbank.make_filterbank(cfg, int(i.nsamp_in_required), int(i.in_stride_min))
-        assert X.shape == (i.nchan, i.in_stride_min) and X.dtype == np.uint8
+            X, self.pulses = filterbank.make_filterbank(cfg, int(i.nsamp_in_required), int(i.in_stride_min),
+                                                        bits=int(i.input_bits))
+        assert X.shape == (i.nchan, i.in_stride_min) and X.dtype == (np.uint8 if i.input_bits == 8 else np.uint16)
         self.X = X
-        self.buf["d_in"].copy_(torch.from_numpy(X))
-        torch.cuda.synchronize()
+        self.upload()
 
     def apply_tuned(self, workload):
         """Sets every kernel slot to its shape in tuned_b200.json (what bench.py runs); a shape that is
@@ -61,7 +61,8 @@ class GpuSearch:
 
     def upload(self):
         """Re-uploads self.X after the test changed it in place."""
-        self.buf["d_in"].copy_(self.torch.from_numpy(self.X))
+        host = self.X if self.X.dtype == np.uint8 else self.X.view(np.int16)  # the device tensor is int16-typed
+        self.buf["d_in"].copy_(self.torch.from_numpy(host))
         self.torch.cuda.synchronize()
 
     def dedisperse(self):

@@ -488,6 +488,105 @@ def test_channel_mask_subband_plan():
     g.close()
 
 
+# ---------------------------------------------------------------------------------- INPUT_BITS = 16 (8(f) f4)
+def test_uint16_input_direct_sweep_saturation_mask_and_host_calls():
+    """A 16-bit plan (ddp_options.input_bits = 16): uint16 samples through the uint16 code shapes of the direct
+    kernel -- direct loads, cooperative and TMA staging over sampled shapes, bit-exact against the oracle's uint16
+    sum; the whole pipeline; all-65535 input (the largest totals the plan's overflow proof admits); a channel
+    mask; and the two host entry points, whose copies must move two bytes per sample."""
+    import oracle
+    from synth import filterbank
+    cfg = small_direct(name="u16", nchan=80, nsamp_out=2300, ndm=41, widths=(1, 2, 4, 8), n_pulses=2)
+    g = GpuSearch(cfg, input_bits=16)
+    i = g.info
+    assert i.input_bits == 16 and g.X.dtype == np.uint16 and int(g.X.max()) > 40000
+    g.run_all()
+    Yo = oracle_direct_rows(cfg, g.X)
+    compare_all(g, Yo, what="u16 default")
+    V = g.plan.enumerate_kcfgs(ddp.K_DIRECT)
+    assert {c.staging for c in V} == {0, 1, 2}  # merged staging is for uint8 input
+    seen = set()
+    for c in _sample(V, 60, seed=16):
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        seen.add(c.staging)
+        g.buf["d_out"].fill_(-1)
+        assert np.array_equal(g.dedisperse(), Yo), "u16 direct differs for %r" % c
+    assert seen == {0, 1, 2}
+    keep = g.X.copy()
+    g.X[:] = 65535
+    g.upload()
+    for c in _sample(V, 12, seed=17):
+        g.plan.set_kcfg(ddp.K_DIRECT, c)
+        assert np.all(g.dedisperse() == 65535 * cfg.nchan), "saturated u16 input, %r" % c
+    g.X[:] = keep
+    g.upload()
+    # host entry points
+    h_snr = torch.full((i.ndm, i.nwidths), -3.0, dtype=torch.float32).pin_memory()
+    h_arg = torch.full((i.ndm, i.nwidths), -1, dtype=torch.int32).pin_memory()
+    g.buf["d_in"].zero_()
+    g.plan.search_host(torch.from_numpy(g.X.view(np.int16)).pin_memory(), g.buf["d_in"], g.buf["d_out"], None,
+                       g.buf["d_snr"], g.buf["d_argmax"], h_snr, h_arg)
+    _, So, Ao = oracle_search(Yo, list(cfg.widths), 0)
+    assert_snr_close(h_snr.numpy(), So, "u16 search_host")
+    assert np.array_equal(h_arg.numpy().view(np.uint32), Ao)
+    nb, ns, md = 2, cfg.nsamp_out, i.max_delay
+    nlong = nb * ns + md
+    Xl, _ = filterbank.make_filterbank(cfg, nlong, (nlong + 47) // 16 * 16, bits=16)
+    Ylong = oracle.dedisperse(Xl, oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s), nb * ns)
+    d_in1 = torch.zeros_like(g.buf["d_in"])
+    g.buf["d_in"].zero_()
+    hb_snr = torch.full((nb, i.ndm, i.nwidths), -3.0, dtype=torch.float32).pin_memory()
+    hb_arg = torch.full((nb, i.ndm, i.nwidths), -1, dtype=torch.int32).pin_memory()
+    g.plan.search_host_batches(torch.from_numpy(Xl.view(np.int16)).pin_memory(), nb, g.buf["d_in"], d_in1,
+                               g.buf["d_out"], g.buf["d_snr"], g.buf["d_argmax"], hb_snr, hb_arg)
+    for b in range(nb):
+        _, Sb, Ab = oracle_search(np.ascontiguousarray(Ylong[:, b * ns: (b + 1) * ns]), list(cfg.widths), 0)
+        assert_snr_close(hb_snr[b].numpy(), Sb, "u16 batch %d" % b)
+        assert np.array_equal(hb_arg[b].numpy().view(np.uint32), Ab)
+    g.close()
+    # channel mask on a 16-bit plan
+    mask = np.ones(cfg.nchan, np.uint8)
+    mask[[0, 7, 8, 33, 79]] = 0
+    gm = GpuSearch(cfg, input_bits=16, chan_mask=mask)
+    Xz = gm.X.copy()
+    Xz[mask == 0] = 0
+    gm.X[mask == 0] = 65535
+    gm.upload()
+    Ym = oracle_direct_rows(cfg, Xz)
+    for c in _sample(gm.plan.enumerate_kcfgs(ddp.K_DIRECT), 18, seed=18):
+        gm.plan.set_kcfg(ddp.K_DIRECT, c)
+        gm.buf["d_out"].fill_(-1)
+        assert np.array_equal(gm.dedisperse(), Ym), "masked u16 direct differs for %r" % c
+    gm.close()
+
+
+def test_uint16_input_subband_plan():
+    """A 16-bit two-step plan: the intermediate is uint32 (65535 * channels per subband does not fit 16 bits); S and
+    Y against the oracle over sampled step-1 and step-2 shapes."""
+    cfg = small_subband(name="u16_sb", nchan=96, nsamp_out=2100, ndm=12 * 8,
+                        subband=SubbandPlan(n_subbands=8, n_coarse=12, coarse_first=0.0, coarse_step=8.0,
+                                            n_fine=8, fine_step=0.25))
+    g = GpuSearch(cfg, input_bits=16)
+    assert g.info.input_bits == 16 and g.info.sub_elem_bytes == 4
+    g.run_all()
+    So, Yo = oracle_subband(cfg, g.X)
+    assert np.array_equal(g.subband_intermediate(), So)
+    compare_all(g, Yo, what="u16 subband default")
+    for kernel in (ddp.K_SUB1, ddp.K_SUB2):
+        keep = g.plan.get_kcfg(kernel)
+        seen = set()
+        for c in _sample(g.plan.enumerate_kcfgs(kernel), 30, seed=20 + kernel):
+            g.plan.set_kcfg(kernel, c)
+            seen.add(c.staging)
+            g.buf["d_out"].fill_(-1)
+            Y = g.dedisperse()
+            assert np.array_equal(g.subband_intermediate(), So), "u16 plan: S differs for %r" % c
+            assert np.array_equal(Y, Yo), "u16 plan: Y differs for %s %r" % (ddp.KERNEL_NAMES[kernel], c)
+        assert seen >= {0, 1}
+        g.plan.set_kcfg(kernel, keep)
+    g.close()
+
+
 @pytest.mark.parametrize("kernel", [ddp.K_SUB1, ddp.K_SUB2])
 def test_subband_plan_kernel_configuration_sweep(kernel):
     cfg = small_subband(name="sweep_sb", nchan=128, nsamp_out=2100, ndm=24 * 8,

@@ -150,6 +150,43 @@ def test_subband_centre_reference_plan_tables_equal_oracle_tables():
         ddp.plan_from_config(cfg, cache_dir=None, subband_ref=2)
 
 
+def test_sixteen_bit_plan_host_side(tmp_path):
+    """ddp_options.input_bits = 16 (P:90 INPUT_BITS): geometry, the uint32 intermediate, overflow
+    proofs with 65535 per sample, validity (no merged staging) and offline compilation of the uint16 code shapes."""
+    cfg = configs.scaled(configs.apertif_direct(), name="u16", nchan=64, nsamp_out=2300, ndm=41, widths=(1, 2, 4, 8))
+    p8 = ddp.plan_from_config(cfg, cache_dir=None)
+    p = ddp.plan_from_config(cfg, cache_dir=str(tmp_path), input_bits=16)
+    i8, i = p8.query(), p.query()
+    assert (i8.input_bits, i.input_bits) == (8, 16)
+    assert i.in_stride_min == i8.in_stride_min and i.max_delay == i8.max_delay  # strides are in elements
+    assert np.array_equal(p.get_delays(0), p8.get_delays(0))
+    V = p.enumerate_kcfgs(ddp.K_DIRECT)
+    assert {c.staging for c in V} == {0, 1, 2} and {c.staging for c in p8.enumerate_kcfgs(ddp.K_DIRECT)} >= {3, 4}
+    assert p.check_kcfg(ddp.K_DIRECT, p.get_kcfg(ddp.K_DIRECT))
+    assert not p.check_kcfg(ddp.K_DIRECT, ddp.Kcfg(64, 4, 16, 4, 8, 4, 16))      # merged staging: uint8 only
+    assert not p.check_kcfg(ddp.K_DIRECT, ddp.Kcfg(64, 4, 16, 4, 8, 0, 1))       # vec_bytes >= 4 for uint16
+    for c in (p.get_kcfg(ddp.K_DIRECT), ddp.Kcfg(32, 4, 8, 2, 4, 0, 16), ddp.Kcfg(64, 2, 4, 4, 8, 2, 8)):
+        assert p.check_kcfg(ddp.K_DIRECT, c), c
+        p.compile_kcfg(ddp.K_DIRECT, c)
+    assert any(n.startswith("ddp_dedisp_u16_") for n in os.listdir(tmp_path))
+    p.destroy()
+    p8.destroy()
+    sb = configs.scaled(configs.apertif_subband(), name="u16sb", nchan=96, nsamp_out=2500, ndm=30, widths=(1, 2, 4, 8),
+                        subband=configs.SubbandPlan(n_subbands=8, n_coarse=6, coarse_first=0.0, coarse_step=8.0,
+                                                    n_fine=5, fine_step=0.25))
+    q = ddp.plan_from_config(sb, cache_dir=None, input_bits=16)
+    assert q.query().sub_elem_bytes == 4 and ddp.plan_from_config(sb, cache_dir=None).query().sub_elem_bytes == 2
+    q.compile_kcfg(ddp.K_SUB1, q.get_kcfg(ddp.K_SUB1))
+    q.compile_kcfg(ddp.K_SUB2, q.get_kcfg(ddp.K_SUB2))
+    q.destroy()
+    # 65535 * 1536 channels: the second moments of the widest series would not fit 64 bits
+    with pytest.raises(ddp.DdpError) as e:
+        ddp.plan_from_config(configs.apertif_direct(), cache_dir=None, input_bits=16)
+    assert e.value.status == binding.E_OVERFLOW
+    with pytest.raises(ddp.DdpError):
+        ddp.plan_from_config(cfg, cache_dir=None, input_bits=12)
+
+
 def test_plan_create_rejects_bad_arguments():
     f = np.array([1500.0, 1400.0, 1300.0, 1200.0])
     ok = dict(chan_freq_mhz=f, t_samp_s=1e-3, dm_list=[0.0, 10.0], widths=[1, 2], nsamp_out=64, cache_dir=None)

@@ -300,6 +300,47 @@ def test_subband_centre_reference_tables():
     assert np.array_equal(a1, b1) and np.array_equal(a2, b2)
 
 
+def test_uint16_input_sums():
+    """INPUT_BITS = 16: the same sums over uint16 samples.  Pins: the worked example scaled by
+    257 (every sample v -> 257 v, so every sum scales alike); linearity X = 256 H + L  =>  Y(X) = 256 Y(H) + Y(L)
+    with the uint8 functions (pinned above) on both bytes; brute force with numpy on the ragged small case;
+    saturated input 65535 everywhere; and the same for subband step 1."""
+    f = [1500.0, 1400.0, 1300.0, 1200.0]
+    d = oracle.delay_table(f, [0.0, 10.0, 20.0], 1e-3)
+    X8 = np.array([[(7 * c + 3 * t) % 11 for t in range(8 + 21)] for c in range(4)], dtype=np.uint8)
+    Y8 = oracle.dedisperse(X8, d, 8)
+    assert np.array_equal(oracle.dedisperse((X8.astype(np.uint16) * 257), d, 8), Y8 * 257)
+    cfg = configs.tiny()
+    delay = oracle.delay_table(cfg.chan_freq_mhz(), cfg.dm_list(), cfg.t_samp_s)
+    nin = cfg.nsamp_out + int(delay.max())
+    X, _ = filterbank.make_filterbank(cfg, nin, nin + 5, bits=16)
+    assert X.dtype == np.uint16 and X.max() > 255
+    H, L = (X >> 8).astype(np.uint8), (X & 0xFF).astype(np.uint8)
+    rows = delay[[0, 3, cfg.ndm - 1]]
+    Y = oracle.dedisperse(X, rows, cfg.nsamp_out)
+    assert np.array_equal(Y, 256 * oracle.dedisperse(H, rows, cfg.nsamp_out) + oracle.dedisperse(L, rows, cfg.nsamp_out))
+    t = np.arange(cfg.nsamp_out)
+    brute = np.zeros(cfg.nsamp_out, dtype=np.int64)
+    for c in range(cfg.nchan):
+        brute += X[c, t + rows[2, c]]
+    assert np.array_equal(Y[2], brute)
+    sat = np.full((cfg.nchan, nin), 65535, dtype=np.uint16)
+    assert (oracle.dedisperse(sat, rows, cfg.nsamp_out) == 65535 * cfg.nchan).all()
+    # subband step 1
+    nsub, A = 8, np.array([0.0, 4.0, 8.0])
+    d1, d2 = oracle.subband_tables(cfg.chan_freq_mhz(), cfg.t_samp_s, nsub, A, np.array([0.0, 0.5, 1.0]))
+    ns1 = cfg.nsamp_out + int(d2.max())
+    Xs, _ = filterbank.make_filterbank(cfg, ns1 + int(d1.max()), bits=16)
+    S = oracle.subband_step1(Xs, d1, nsub, ns1)
+    Hs, Ls = (Xs >> 8).astype(np.uint8), (Xs & 0xFF).astype(np.uint8)
+    assert np.array_equal(S, 256 * oracle.subband_step1(Hs, d1, nsub, ns1) + oracle.subband_step1(Ls, d1, nsub, ns1))
+    cps = cfg.nchan // nsub
+    b = np.zeros(ns1, dtype=np.int64)
+    for c in range(5 * cps, 6 * cps):
+        b += Xs[c, np.arange(ns1) + d1[2, c]]
+    assert np.array_equal(S[2, 5], b)
+
+
 # ----------------------------------------------------------------------------- INT
 def test_integrate_invariants():
     rng = np.random.default_rng(31)
