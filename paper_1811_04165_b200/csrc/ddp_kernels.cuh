@@ -382,11 +382,15 @@ __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
 // ------------------------------------------------------------------------------------ packed staged dedispersion
 // uint8 input, STAGING 1 (cooperative loads) or 2 (TMA bulk copies).  The inner loop is built for the
 // sm_100a issue limits measured in profiles/: one LDS.32 brings FOUR consecutive samples of one
-// (channel, trial) to a thread, LOP3 / PRMT split them into two registers of 2 x 16-bit lanes
-// (bytes 0,2 and bytes 1,3) and two IMADs (x * 1 + acc, the 1 being a run-time value so that the
-// adds go to the fma pipe while the extractions use the alu pipe) accumulate them: 5 issued
-// instructions per 4 adds.  16-bit lanes are exact for <= 257 channels (255 * 257 = 65535), so they
-// are flushed into uint32 totals every 256 channels (WIDE) or unpacked once at the end (!WIDE).
+// (channel, trial) to a thread; bytes 0 and 2 are masked out by a LOP3 (alu pipe) and added to the
+// "even" register of 2 x 16-bit lanes by an IMAD (x * 1 + acc, the 1 being a run-time value so that the
+// add goes to the fma pipe); bytes 1 and 3 are added to the "odd" register by ONE LEA.HI
+// (acc + (w >> 8), alu pipe) -- byte 2 rides along in bits 8..23 and is subtracted again when the lanes
+// are unpacked (the even register's upper lane is exactly its sum; all of it exact mod 2^32).  That is
+// 4 issued instructions per 4 adds, two of them on the alu pipe, one each on the fma pipe and the LSU
+// (the round-1 form, LOP3 + PRMT + IADD3 + IMAD, had 2.5 on the alu pipe, which is the pipe the kernel
+// is bound by: 22.6 -> 20.5 ms at cfg3).  16-bit lanes are exact for <= 257 channels (255 * 257 = 65535),
+// so they are flushed into uint32 totals every 256 channels (WIDE) or unpacked once at the end (!WIDE).
 //
 // Per chunk of U channels the block stages, for each channel, the window its TD trials need --
 // [tile_t + dmin, tile_t + TT + dmax), from the 16-byte aligned-down start -- as FOUR copies
@@ -559,7 +563,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_u16* orow = (ddp_u16*)p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    const ddp_u32 oo = accO[j][k];
+                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);  // lanes (b1, b3): see the inner loop
                     const ddp_u32 lo = __byte_perm(accE[j][k], oo, 0x5410u), hi = __byte_perm(accE[j][k], oo, 0x7632u);
                     const int t = tile_t + 4 * (wb + 32 * k);
                     if (t + 3 < p.ns) {
@@ -575,7 +579,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_u32* orow = p.out + (ddp_i64)g * p.out_group_stride + (ddp_i64)dm * p.out_dm_stride;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    const ddp_u32 oo = accO[j][k];
+                    const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);  // lanes (b1, b3): see the inner loop
                     ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = oo & 0xffffu, v2 = accE[j][k] >> 16, v3 = oo >> 16;
                     const int t = tile_t + 4 * (wb + 32 * k);
                     if (t + 3 < p.ns) {
@@ -648,11 +652,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 w = wp[32 * k];
                     const ddp_u32 e = w & 0x00ff00ffu;
-                    // even lanes by IADD3 (alu pipe; ptxas folds two of them into one three-input add),
-                    // odd lanes by IMAD with a run-time 1 (fma pipe)
-                    const ddp_u32 o = __byte_perm(w, 0u, 0x4341u);
-                    accE[j][k] += e;
-                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accO[j][k]) : "r"(o), "r"(one));
+                    // even lanes: LOP3 (alu) + IMAD with a run-time 1 (fma); odd lanes: acc += w >> 8 in ONE alu
+                    // instruction (LEA.HI), the words' bytes 2 riding along in bits 8..23: emit() takes them out
+                    // again (accE's upper lane holds exactly their sum; everything is exact mod 2^32)
+                    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(accE[j][k]) : "r"(e), "r"(one));
+                    accO[j][k] += w >> 8;
                 }
             }
         }
