@@ -468,8 +468,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it)
     ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [NBC][U][4][winw]
-    ddp_u32* offs = copies + (size_t)NBC * U * 4 * winw;         // [NBC][TD][U] byte offsets into ddp_smem
-    int* dls = (int*)(offs + (((size_t)NBC * TD * U + 3) & ~(size_t)3));  // [2][TD][SC], 16-byte aligned
+    ddp_u32* offs = copies + (size_t)NBC * U * 4 * winw;         // [2][TD][U] byte offsets into ddp_smem
+    int* dls = (int*)(offs + (((size_t)2 * TD * U + 3) & ~(size_t)3));    // [2][TD][SC], 16-byte aligned
     unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
     ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
     const int nchunks = p.nred / U;
@@ -531,7 +531,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     };
     auto prep_offs = [&](int c) {
-        ddp_u32* ob = offs + (size_t)(c & (NBC - 1)) * TD * U;
+        ddp_u32* ob = offs + (size_t)(c & 1) * TD * U;
         const ddp_u32 cbase = (ddp_u32)((size_t)(c & (NBC - 1)) * U * 4 * winw);
         const int s = (c * U) / SC;
         const int* d = dls + (size_t)(s & 1) * TD * SC + (c * U - s * SC);
@@ -616,11 +616,9 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
         if constexpr (!SINGLE) ddp_mbar_wait(&mbar[0], 0u);
     }
-    if constexpr (!SINGLE) {
-        stage(0);
-        prep_offs(0);
-        __syncthreads();
-    }
+    if constexpr (!SINGLE) stage(0);
+    prep_offs(0);
+    if constexpr (!SINGLE) __syncthreads();
 
     for (int c = 0; c < nchunks; ++c) {
         const int r0 = c * U;
@@ -632,8 +630,10 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 ddp_mbar_wait(&mbar[c & 1], (ddp_u32)((c >> 1) & 1));
             }
             stage(c);
-            prep_offs(c);
             __syncthreads();
+            // the offsets of the next chunk depend on the delays only: written here, between the barriers, so that
+            // their loads and stores are in flight beside the sums instead of in front of a barrier
+            if (c + 1 < nchunks) prep_offs(c + 1);
         } else if (c + 1 < nchunks) {
             if constexpr (STAGING == 2) {
                 if (warp == 0 && c + 2 < nchunks) tma_issue(c + 2);  // slot c & 1 was converted during iteration c - 1
@@ -642,7 +642,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
             stage(c + 1);
             prep_offs(c + 1);
         }
-        const ddp_u32* ob = offs + ((size_t)(c & (NBC - 1)) * TD + ty * DPT) * U;
+        const ddp_u32* ob = offs + ((size_t)(c & 1) * TD + ty * DPT) * U;
 #pragma unroll
         for (int j = 0; j < DPT; ++j) {
 #pragma unroll

@@ -498,10 +498,10 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += (4 + 2 * 16 + 2) * 8 + 128;                      // mbarriers, scheduler state
                 return b;
             }
-            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [nb][TD][U], dls [2][TD][64], raw, mbar
+            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [2][TD][U], dls [2][TD][64], raw, mbar
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
                 auto layout = [&](size_t nb) {
-                    size_t b = nb * 4 * row * c.unroll + ((nb * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+                    size_t b = nb * 4 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
                     if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
                     return b;
                 };
