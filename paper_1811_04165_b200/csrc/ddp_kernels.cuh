@@ -401,7 +401,7 @@ __device__ __forceinline__ void ddp_dedisp_body(const DdpDedispParams& p) {
 // offsets are computed once per chunk by one thread each (table `offs`), from the tile's delays
 // kept in shared memory per superchunk of 64 channels (`dls`).  Copies, offsets and delays are
 // double buffered: chunk c+1 is staged while chunk c is summed, one __syncthreads per chunk.
-template <int VW, bool GLOBAL>
+template <int VW, bool GLOBAL, bool SKIP0>
 __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst, int cstride) {
     ddp_u32 w[VW + 1];
     if constexpr (GLOBAL) {  // read-only global data: LDG through the non-coherent path
@@ -428,11 +428,11 @@ __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst
         w[VW] = src[VW];
     }
 #pragma unroll
-    for (int o = 0; o < 4; ++o) {
+    for (int o = SKIP0 ? 1 : 0; o < 4; ++o) {  // SKIP0: copy 0 is the source itself (the TMA raw slot), dst holds copies 1..3
         ddp_u32 x[VW];
 #pragma unroll
         for (int i = 0; i < VW; ++i) x[i] = o == 0 ? w[i] : ddp_shf_r(w[i], w[i + 1], 8u * o);
-        ddp_u32* d = dst + o * cstride;
+        ddp_u32* d = dst + (SKIP0 ? o - 1 : o) * cstride;
         if constexpr (VW == 4) *(uint4*)d = make_uint4(x[0], x[1], x[2], x[3]);
         else if constexpr (VW == 2) *(uint2*)d = make_uint2(x[0], x[1]);
         else d[0] = x[0];
@@ -453,6 +453,11 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     // then summed, two barriers per chunk; the TMA raw slots stay double buffered, so the copy of
     // chunk c+1 is still in flight while chunk c is processed.
     constexpr int NBC = SINGLE ? 1 : 2;
+    // RAW0: single-buffered with TMA, the unshifted copy is not made: windows whose delay is a multiple of four
+    // bytes are read from the TMA raw slot itself (it is not overwritten before the chunk's sums are done: the
+    // copy of chunk c + 1 goes to the other slot), which saves a quarter of the staging stores and of the buffer
+    constexpr bool RAW0 = SINGLE && STAGING == 2;
+    constexpr int NCP = RAW0 ? 3 : 4;  // shifted copies kept per row
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int nthreads = blockDim.x * blockDim.y;
     const int tid = ty * blockDim.x + tx;
@@ -467,8 +472,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     const ddp_u32 one = (ddp_u32)p.one;
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it)
-    ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [NBC][U][4][winw]
-    ddp_u32* offs = copies + (size_t)NBC * U * 4 * winw;         // [2][TD][U] byte offsets into ddp_smem
+    ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [NBC][U][NCP][winw]
+    ddp_u32* offs = copies + (size_t)NBC * U * NCP * winw;       // [2][TD][U] byte offsets into ddp_smem
     int* dls = (int*)(offs + (((size_t)2 * TD * U + 3) & ~(size_t)3));    // [2][TD][SC], 16-byte aligned
     unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
     ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
@@ -514,7 +519,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     // Each row is split over `parts` warps (a power of two), so the per-row set-up is done once per warp.
     const int parts_log2 = nwarps > U ? 31 - __clz(nwarps / U) : 0;
     auto stage = [&](int c) {
-        ddp_u32* cb = copies + (size_t)(c & (NBC - 1)) * U * 4 * winw;
+        ddp_u32* cb = copies + (size_t)(c & (NBC - 1)) * U * NCP * winw;
         for (int unit = warp; unit < (U << parts_log2); unit += nwarps) {
             const int u = unit >> parts_log2, part = unit & ((1 << parts_log2) - 1);
             ddp_i64 a0;
@@ -525,14 +530,15 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 src = (const ddp_u32*)(raw + ((size_t)(c & 1) * U + u) * (win + 16));
             else
                 src = (const ddp_u32*)(ddp_in_row<ddp_u8>(p, g, c * U + u) + a0);
-            ddp_u32* dst = cb + (size_t)u * 4 * winw;
+            ddp_u32* dst = cb + (size_t)u * NCP * winw;
             for (int v = ((part << 5) + lane) * VW; v < lenw; v += (32 << parts_log2) * VW)
-                ddp_shift_store<VW, STAGING == 1>(src + v, dst + v, winw);
+                ddp_shift_store<VW, STAGING == 1, RAW0>(src + v, dst + v, winw);
         }
     };
     auto prep_offs = [&](int c) {
         ddp_u32* ob = offs + (size_t)(c & 1) * TD * U;
-        const ddp_u32 cbase = (ddp_u32)((size_t)(c & (NBC - 1)) * U * 4 * winw);
+        const ddp_u32 cbase = (ddp_u32)((size_t)(c & (NBC - 1)) * U * NCP * winw);
+        const ddp_u32 rbase = (ddp_u32)((raw - ddp_smem) >> 2) + (ddp_u32)((size_t)(c & 1) * U * ((win + 16) >> 2));  // words
         const int s = (c * U) / SC;
         const int* d = dls + (size_t)(s & 1) * TD * SC + (c * U - s * SC);
         for (int idx = tid; idx < TD * U; idx += nthreads) {
@@ -540,7 +546,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
             const int dmin = d[u];
             const int dd = d[(j < nd ? j : nd - 1) * SC + u];
             const int pos = (int)(((ddp_i64)tile_t + dmin) & 15) + (dd - dmin);
-            ob[idx] = (cbase + (ddp_u32)((u * 4 + (pos & 3)) * winw + (pos >> 2))) * 4u;
+            if (RAW0 && (pos & 3) == 0) ob[idx] = (rbase + (ddp_u32)(u * ((win + 16) >> 2) + (pos >> 2))) * 4u;
+            else ob[idx] = (cbase + (ddp_u32)((u * NCP + (pos & 3) - (RAW0 ? 1 : 0)) * winw + (pos >> 2))) * 4u;
         }
     };
 

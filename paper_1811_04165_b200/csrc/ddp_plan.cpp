@@ -501,7 +501,8 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
             if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [2][TD][U], dls [2][TD][64], raw, mbar
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
                 auto layout = [&](size_t nb) {
-                    size_t b = nb * 4 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+                    const size_t ncp = nb == 1 && c.staging == 2 ? 3 : 4;  // single-buffered with TMA: the unshifted copy is the raw slot (RAW0)
+                    size_t b = nb * ncp * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
                     if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
                     return b;
                 };
