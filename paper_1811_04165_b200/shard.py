@@ -32,6 +32,34 @@ def dm_rows_of_rank(ndm: int, rank: int, world: int, multiple: int = 1) -> Tuple
     return lo * multiple, (lo + base + (1 if rank < extra else 0)) * multiple
 
 
+def plan_for_rank(cfg, rank: int, world: int, **plan_kw):
+    """(plan, lo, hi): the plan of rank `rank` when ONE beam's DM trials are split over `world` GPUs (SURVEY 8(e),
+    8(f) f3).  A direct plan gets the slice dm_list[lo:hi]; a subband plan gets whole coarse trials (a slice of the
+    coarse grid with all its fine trials), so lo and hi are multiples of n_fine.  Delays are relative to the highest
+    channel frequency whatever the slice (DD.3), so the rows a rank computes are bit for bit the rows lo..hi-1 of the
+    one-GPU search; every rank reads the same input (its plan needs only its own largest delay of it) and the S/N
+    tables meet in gather_rows.  The coarse DMs of a slice are coarse_first + lo/n_fine * step + a * step: identical to
+    the one-GPU grid when first and step are dyadic (as in BASELINE.json), else equal up to the last bit of a DM."""
+    import numpy as np
+    from .binding import plan_create
+    sb = getattr(cfg, "subband", None)
+    if sb is not None:
+        lo, hi = dm_rows_of_rank(sb.n_coarse * sb.n_fine, rank, world, sb.n_fine)
+        a0, na = lo // sb.n_fine, (hi - lo) // sb.n_fine
+        if na == 0:
+            return None, lo, hi
+        plan = plan_create(cfg.chan_freq_mhz(), cfg.t_samp_s, None, cfg.widths, cfg.nsamp_out, n_subbands=sb.n_subbands,
+                           n_coarse=na, coarse_dm_first=sb.coarse_first + a0 * sb.coarse_step,
+                           coarse_dm_step=sb.coarse_step, n_fine=sb.n_fine, fine_dm_step=sb.fine_step, **plan_kw)
+        return plan, lo, hi
+    lo, hi = dm_rows_of_rank(cfg.ndm, rank, world)
+    if hi == lo:
+        return None, lo, hi
+    plan = plan_create(cfg.chan_freq_mhz(), cfg.t_samp_s, np.ascontiguousarray(cfg.dm_list()[lo:hi]), cfg.widths,
+                       cfg.nsamp_out, **plan_kw)
+    return plan, lo, hi
+
+
 def gather_rows(local, ndm: int, device=None):
     """The [ndm][nW] table of a search whose DM rows were split with dm_rows_of_rank: every rank passes its own rows
     (a float32 or int32 tensor [hi - lo][nW]); all ranks get the whole table.  This gather of at most a few hundred

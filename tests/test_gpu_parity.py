@@ -488,6 +488,38 @@ def test_channel_mask_subband_plan():
     g.close()
 
 
+# ---------------------------------------------------------------------------------- DM rows split over ranks (8(f) f3)
+@pytest.mark.parametrize("subband", [False, True])
+def test_dm_sharded_search_equals_the_one_gpu_search(subband):
+    """shard.plan_for_rank: one beam's DM trials split over 3 ranks.  Only one GPU is here, so the three ranks' plans
+    run in turn on it, each on the same input (a rank's plan needs only its own largest delay of it); their rows,
+    stacked, must be the oracle's rows of the whole search, and the S/N tables likewise (what gather_rows
+    concatenates; its exchange itself is covered by the gloo test)."""
+    from paper_1811_04165_b200.shard import plan_for_rank
+    cfg = small_subband(name="shard_sb", ndm=6 * 5) if subband else small_direct(name="shard_d")
+    whole = GpuSearch(cfg)
+    Yo = oracle_subband(cfg, whole.X)[1] if subband else oracle_direct_rows(cfg, whole.X)
+    _, So, Ao = oracle_search(Yo, list(cfg.widths), 0)
+    world, rows, snrs, args = 3, [], [], []
+    for r in range(world):
+        plan, lo, hi = plan_for_rank(cfg, r, world)
+        i = plan.query()
+        assert i.ndm == hi - lo and i.in_stride_min <= whole.info.in_stride_min
+        buf = ddp.alloc_buffers(plan, "cuda:0")
+        buf["d_in"].copy_(torch.from_numpy(np.ascontiguousarray(whole.X[:, : i.in_stride_min])))
+        plan.dedisperse(buf["d_in"], buf["d_out"])
+        plan.integrate_snr(buf["d_out"], buf["d_snr"], buf["d_argmax"])
+        torch.cuda.synchronize()
+        rows.append(u32(buf["d_out"])[:, : i.nsamp_out])
+        snrs.append(buf["d_snr"].cpu().numpy())
+        args.append(u32(buf["d_argmax"]))
+        plan.destroy()
+    assert np.array_equal(np.concatenate(rows, axis=0), Yo)
+    assert_snr_close(np.concatenate(snrs, axis=0), So, "sharded search")
+    assert np.array_equal(np.concatenate(args, axis=0), Ao)
+    whole.close()
+
+
 # ---------------------------------------------------------------------------------- INPUT_BITS = 16 (8(f) f4)
 def test_uint16_input_direct_sweep_saturation_mask_and_host_calls():
     """A 16-bit plan (ddp_options.input_bits = 16): uint16 samples through the uint16 code shapes of the direct

@@ -43,6 +43,44 @@ def test_dm_row_partition_is_exact_contiguous_and_block_aligned():
     assert gather_rows(t, 3) is t                                          # no process group: identity
 
 
+def test_plans_of_a_dm_sharded_search_tile_the_one_gpu_plan():
+    """plan_for_rank: the delay tables of the ranks' plans, stacked, are the one-GPU plan's tables (direct: rows of
+    the delay table; subband: coarse rows of the step-1 table, one shared step-2 table), and every rank needs no
+    more input than the whole search."""
+    import numpy as np
+    import paper_1811_04165_b200 as ddp
+    from paper_1811_04165_b200.shard import plan_for_rank
+    from synth import configs
+    from synth.configs import SubbandPlan
+    direct = configs.scaled(configs.apertif_direct(), name="shard_d", nchan=64, nsamp_out=2000, ndm=37, widths=(1, 2, 4))
+    sub = configs.scaled(configs.apertif_direct(), name="shard_s", nchan=96, nsamp_out=2000, ndm=7 * 5, widths=(1, 2, 4),
+                         subband=SubbandPlan(n_subbands=8, n_coarse=7, coarse_first=0.0, coarse_step=8.0, n_fine=5,
+                                             fine_step=0.25))
+    for cfg in (direct, sub):
+        whole = ddp.plan_from_config(cfg, cache_dir=None)
+        wi = whole.query()
+        for world in (1, 2, 3, 8):
+            tabs, covered = [], 0
+            for r in range(world):
+                plan, lo, hi = plan_for_rank(cfg, r, world, cache_dir=None)
+                assert lo == covered
+                covered = hi
+                if plan is None:
+                    assert lo == hi
+                    continue
+                i = plan.query()
+                assert i.ndm == hi - lo and i.nsamp_in_required <= wi.nsamp_in_required
+                if cfg.subband is None:
+                    tabs.append(plan.get_delays(0))
+                else:
+                    tabs.append(plan.get_delays(1))
+                    assert np.array_equal(plan.get_delays(2), whole.get_delays(2))
+                plan.destroy()
+            assert covered == cfg.ndm
+            assert np.array_equal(np.concatenate(tabs, axis=0), whole.get_delays(0 if cfg.subband is None else 1))
+        whole.destroy()
+
+
 def test_combine_without_process_group_is_identity():
     assert combine(3.5, 7.0) == (3.5, 7.0)
 
