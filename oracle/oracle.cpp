@@ -23,7 +23,9 @@
 // injected pulse recovered at its DM and width on BJ cfg0; sliding boxcar: constant / impulse closed forms,
 // numpy cumulative-sum difference, block sums are its samples at multiples of w, a misaligned pulse is
 // recovered at its true width; channel mask: pure-Python brute force over the kept channels, complement
-// identity; consecutive batches with carried samples == one long dedispersion.
+// identity; consecutive batches with carried samples == one long dedispersion; 16-bit input (the _u16
+// functions): worked example scaled by 257, linearity over the two bytes against the pinned uint8 functions,
+// numpy brute force, saturated input.
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -shared -fPIC oracle.cpp -o liboracle.so
 #include <cmath>
