@@ -14,9 +14,10 @@
 #define DDP_AOT_ISNR(S, D, T) DDP_DEFINE_ISNR(ddp_isnr_s##S##_d##D##_t##T, S, D, T)
 
 // plan defaults (ddp_plan.cpp::default_kcfgs); W = code flags (bit 0 wide flush, bit 1 uint16 result,
-// bits 2-3 log2 lane-sum group of the packed uint16 kernel)
+// bits 2-3 log2 lane-sum group of the packed uint16 kernel, bit 4 single buffer, bit 6 diagonal time tiles of step 1)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 1)
 DDP_AOT_U8(16, 2, 8, 1, 16, 256, 2)
+DDP_AOT_U8(16, 2, 8, 1, 16, 256, 66)   // the same with diagonal time tiles (chosen per plan from its step-1 delays)
 DDP_AOT_U16(4, 8, 8, 2, 16, 256, 8)
 DDP_AOT_U32(4, 4, 4, 0, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 0, 16, 256)
@@ -41,9 +42,9 @@ DDP_AOT_SNR(4, 1, 1, 2, 16, 256)
 DDP_AOT_U8(16, 4, 16, 2, 16, 512, 1)   // cfg1 direct, best packed shape [64,8,16,4,16,TMA,16]
 DDP_AOT_U8(16, 8, 8, 2, 16, 512, 17)   // cfg3 direct   [128,4,16,8,8,TMA,16], wide flush, single-buffered copies
 DDP_AOT_U8(16, 8, 4, 2, 16, 512, 1)    // cfg3 direct, best double-buffered shape [64,8,16,8,4,TMA,16]
-DDP_AOT_U8(16, 8, 4, 2, 16, 512, 18)   // cfg2 sub1     [128,4,16,8,4,TMA,16], uint16 result, single-buffered copies
-DDP_AOT_U8(16, 8, 4, 2, 8, 512, 18)    // cfg2 sub1, 8-byte staging loads [128,4,16,8,4,TMA,8], uint16 result, single-buffered copies
-DDP_AOT_U8(16, 8, 2, 2, 16, 512, 2)    // cfg2 sub1, best double-buffered shape [128,4,16,8,2,TMA,16]
+DDP_AOT_U8(16, 8, 16, 2, 16, 512, 82)  // cfg2 sub1     [128,4,16,8,16,TMA,16], uint16 result, diagonal time tiles, single-buffered copies
+DDP_AOT_U8(16, 8, 8, 2, 16, 512, 66)   // cfg2 sub1, best double-buffered shape with diagonal tiles [128,4,16,8,8,TMA,16]
+DDP_AOT_U8(16, 8, 4, 2, 16, 512, 18)   // cfg2 sub1 without diagonal tiles (an ascending band) [128,4,16,8,4,TMA,16], single-buffered copies
 DDP_AOT_U16(8, 4, 8, 2, 16, 256, 8)    // cfg2 sub2     [32,8,8,4,8,TMA,16], lane-sum group 4
 DDP_AOT_INTEG(16, 2, 1, 0, 16, 256)    // integrate     [16|64,2,16,2,1,direct,16]
 DDP_AOT_SNR(8, 1, 1, 0, 8, 256)        // snr cfg1/cfg2 [64,2,8,1,1,direct,8]

@@ -82,6 +82,7 @@ struct ddp_plan {
     // configurations + validity caches
     ddp_kcfg kcfg[DDP_K_COUNT];
     mutable std::map<int, int> spread_cache[3];              // dedisp kernel -> (TD -> max window spread)
+    mutable std::map<int, std::pair<int, int>> diag_cache;   // step 1, TD -> (max spread of the delays relative to a subband's first row, max shift D_last - D_first), (-1, -1) = not usable
     mutable std::map<std::pair<int, int>, DdpMergeTable> merge_tables[3];  // host copies, built on first use
     int64_t merge_capacity = 0;                               // bytes of the workspace region for the resident table
     unsigned char* d_merge = nullptr;                         // device: resident merge table (one (kernel, TD, G) at a time)
@@ -106,6 +107,9 @@ int ddp_slide_nb(const ddp_plan* p, const ddp_kcfg& c);                 // slidi
 int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // staged row window (elements)
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c);  // packed uint8 kernel: one copy buffer
+// Subband step 1, packed uint8 kernel: time tiles aligned to the input with a per-trial output shift (code flag
+// bit 6, "DIAG").  *shift_max = largest D_last - D_first over the DM tiles and subbands (extra time tiles of the grid).
+bool ddp_sub1_diag(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, int* rel_spread = nullptr, int* shift_max = nullptr);
 // Merged staging (staging genes 3 / 4: G = 2 / 4 adjacent rows pre-summed exactly; uint8 dedispersion only).
 inline int ddp_merge_group(const ddp_kcfg& c) { return c.staging == 3 ? 2 : (c.staging == 4 ? 4 : 0); }
 // producer warps the merged kernel adds to its threads_t x threads_dm consumer threads (4 or 12 warps)

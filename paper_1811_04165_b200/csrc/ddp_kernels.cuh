@@ -439,7 +439,7 @@ __device__ __forceinline__ void ddp_shift_store(const ddp_u32* src, ddp_u32* dst
     }
 }
 
-template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE, bool OUT16, bool SINGLE>
+template <int SPT, int DPT, int U, int STAGING, int VEC, bool WIDE, bool OUT16, bool SINGLE, bool DIAG>
 __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p) {
     static_assert(SPT >= 4 && VEC >= 4, "packed staging works on whole 4-sample words");
     static_assert(!(WIDE && OUT16), "a uint16 result never needs the wide flush");
@@ -464,12 +464,26 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     const int warp = tid >> 5, lane = tid & 31, nwarps = nthreads >> 5;
     const int TT = blockDim.x * SPT, TD = blockDim.y * DPT;
     const int g = blockIdx.z;
-    const int tile_t = blockIdx.x * TT;
     const int tile_dm = blockIdx.y * TD;
     const int nd = (tile_dm + TD < p.ndm ? TD : p.ndm - tile_dm);  // live trials of this tile (>= 1)
     const int* dl = p.delay + (ddp_i64)g * p.delay_group_off + (ddp_i64)tile_dm * p.delay_dm_stride;
     const int win = p.win, winw = win >> 2;
     const ddp_u32 one = (ddp_u32)p.one;
+    // DIAG ("diagonal" time tiles; subband step 1, where one coarse trial moves a whole subband by hundreds of
+    // samples): the tile is laid out in INPUT-aligned time u = t + D_j, D_j = trial j's delay of the group's first
+    // reduction row, so that the trials of a tile read almost the same window of every row -- the staged window
+    // shrinks from TT + (spread of the delays over the tile) to TT + (spread of the delays RELATIVE to the first
+    // row: 233 instead of 5616 samples at BJ:cfg2 with 32 trials).  Trial j then owns the output samples
+    // t = u - D_j, a per-trial shift of its stores; everything between is the same kernel on relative delays.
+    // D_j is rounded down so that D_j - D_0 is a multiple of 4: the shifted stores stay whole aligned vectors
+    // (the relative delays grow by at most 3 samples for it).
+    const int tile_o = blockIdx.x * TT;  // first output sample of the tile's FIRST trial
+    int tile_t = tile_o;                 // first (input-aligned) sample of the tile
+    if constexpr (DIAG) {
+        const int D0 = __ldg(dl), Dl = __ldg(dl + (ddp_i64)(nd - 1) * p.delay_dm_stride);
+        if ((ddp_i64)tile_o >= (ddp_i64)p.ns + (Dl - D0)) return;  // block-uniform: past the last trial's last sample
+        tile_t += D0;
+    }
 
     // shared-memory carve-up (ddp_smem_bytes mirrors it)
     ddp_u32* copies = (ddp_u32*)ddp_smem;                        // [NBC][U][NCP][winw]
@@ -477,6 +491,8 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     int* dls = (int*)(offs + (((size_t)2 * TD * U + 3) & ~(size_t)3));    // [2][TD][SC], 16-byte aligned
     unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
     ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
+    int* dmm = STAGING == 2 ? (int*)(mbar + 2) : (int*)raw;            // DIAG: [2][2][SC] smallest / largest relative delay of a row
+    int* dsh = dmm + 4 * SC;                                           // DIAG: [TD] D_j - D_0, the output shift of trial j
     const int nchunks = p.nred / U;
 
     auto load_dls = [&](int s) {
@@ -484,14 +500,41 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         const int r0 = s * SC;
         for (int idx = tid; idx < TD * SC; idx += nthreads) {
             const int j = idx / SC, cc = idx - j * SC;
-            if (r0 + cc < p.nred) d[idx] = dl[(ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride + r0 + cc];
+            const int* drow = dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride;
+            if (r0 + cc < p.nred) {
+                int v = drow[r0 + cc];
+                if constexpr (DIAG) {
+                    const int Dj = __ldg(drow), D0 = __ldg(dl);
+                    v -= Dj - ((Dj - D0) & 3);
+                }
+                d[idx] = v;
+            }
+        }
+    };
+    // DIAG: rounded relative delays are not monotone in the trial index, so the window of a row is bounded by
+    // their true minimum / maximum over the tile's trials (one thread per row of the superchunk)
+    auto minmax_dls = [&](int s) {
+        const int* d = dls + (size_t)(s & 1) * TD * SC;
+        for (int cc = tid; cc < SC && s * SC + cc < p.nred; cc += nthreads) {  // blocks may have fewer than SC threads
+            int lo = d[cc], hi = lo;
+            for (int j = 1; j < nd; ++j) {
+                const int v = d[j * SC + cc];
+                lo = v < lo ? v : lo;
+                hi = v > hi ? v : hi;
+            }
+            dmm[(s & 1) * 2 * SC + cc] = lo;
+            dmm[(s & 1) * 2 * SC + SC + cc] = hi;
         }
     };
     // staged extent of reduction row r: aligned start (elements from the row start) and words to stage
     auto row_extent = [&](int r, ddp_i64& a0, int& lenw) {
         const int s = r / SC;
         const int* d = dls + (size_t)(s & 1) * TD * SC + (r - s * SC);
-        const int dmin = d[0], dmax = d[(nd - 1) * SC];  // delays do not decrease with the trial index
+        int dmin = d[0], dmax = d[(nd - 1) * SC];  // delays do not decrease with the trial index
+        if constexpr (DIAG) {
+            dmin = dmm[(s & 1) * 2 * SC + (r - s * SC)];
+            dmax = dmm[(s & 1) * 2 * SC + SC + (r - s * SC)];
+        }
         a0 = ((ddp_i64)tile_t + dmin) & ~(ddp_i64)15;
         // words this row's own trials read (p.win bounds it for the worst row of the plan), whole uint4s
         int need = (((int)((ddp_i64)tile_t + dmin - a0) + (dmax - dmin)) >> 2) + (TT >> 2) + 1;
@@ -543,7 +586,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         const int* d = dls + (size_t)(s & 1) * TD * SC + (c * U - s * SC);
         for (int idx = tid; idx < TD * U; idx += nthreads) {
             const int j = idx / U, u = idx - j * U;
-            const int dmin = d[u];
+            const int dmin = DIAG ? dmm[(s & 1) * 2 * SC + (c * U - s * SC) + u] : d[u];
             const int dd = d[(j < nd ? j : nd - 1) * SC + u];
             const int pos = (int)(((ddp_i64)tile_t + dmin) & 15) + (dd - dmin);
             if (RAW0 && (pos & 3) == 0) ob[idx] = (rbase + (ddp_u32)(u * ((win + 16) >> 2) + (pos >> 2))) * 4u;
@@ -572,8 +615,9 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);  // lanes (b1, b3): see the inner loop
                     const ddp_u32 lo = __byte_perm(accE[j][k], oo, 0x5410u), hi = __byte_perm(accE[j][k], oo, 0x7632u);
-                    const int t = tile_t + 4 * (wb + 32 * k);
-                    if (t + 3 < p.ns) {
+                    const int t = tile_o + 4 * (wb + 32 * k) - (DIAG ? dsh[ty * DPT + j] : 0);
+                    if (DIAG && t < 0) {  // a shifted trial's samples in front of the series (t is a multiple of 4)
+                    } else if (t + 3 < p.ns) {
                         *(uint2*)(orow + t) = make_uint2(lo, hi);
                     } else {
                         if (t < p.ns) orow[t] = (ddp_u16)lo;
@@ -588,8 +632,9 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
                 for (int k = 0; k < K; ++k) {
                     const ddp_u32 oo = accO[j][k] - ((accE[j][k] >> 16) << 8);  // lanes (b1, b3): see the inner loop
                     ddp_u32 v0 = accE[j][k] & 0xffffu, v1 = oo & 0xffffu, v2 = accE[j][k] >> 16, v3 = oo >> 16;
-                    const int t = tile_t + 4 * (wb + 32 * k);
-                    if (t + 3 < p.ns) {
+                    const int t = tile_o + 4 * (wb + 32 * k) - (DIAG ? dsh[ty * DPT + j] : 0);
+                    if (DIAG && t < 0) {  // a shifted trial's samples in front of the series (t is a multiple of 4)
+                    } else if (t + 3 < p.ns) {
                         if (add) {
                             const uint4 o = *(const uint4*)(orow + t);
                             v0 += o.x; v1 += o.y; v2 += o.z; v3 += o.w;
@@ -615,7 +660,15 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     }
     load_dls(0);
+    if constexpr (DIAG) {
+        for (int j = tid; j < TD; j += nthreads)
+            dsh[j] = (__ldg(dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride) - __ldg(dl)) & ~3;
+    }
     __syncthreads();
+    if constexpr (DIAG) {
+        minmax_dls(0);
+        __syncthreads();
+    }
     if constexpr (STAGING == 2) {
         if (warp == 0) {
             tma_issue(0);
@@ -630,6 +683,9 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     for (int c = 0; c < nchunks; ++c) {
         const int r0 = c * U;
         if (r0 % SC == 0 && r0 + SC < p.nred) load_dls(r0 / SC + 1);
+        if constexpr (DIAG) {  // one chunk (and a barrier) after the load, at least one barrier before the first use
+            if (r0 % SC == U && r0 - U + SC < p.nred) minmax_dls((r0 - U) / SC + 1);
+        }
         if constexpr (SINGLE) {
             // every thread has left chunk c - 1 (barrier at the end of the last iteration)
             if constexpr (STAGING == 2) {
@@ -2075,7 +2131,8 @@ __device__ __forceinline__ void ddp_isnr_slide_body(const DdpIsnrParams& p) {
 // uint8 / uint16 input with staging takes the packed kernels; everything else the generic one.
 // FLAGS: bit 0 WIDE (uint8 packed: reduction longer than 256 rows), bit 1 OUT16 (uint16 result: the
 // narrow subband intermediate), bits 2-3 log2 of the uint16 packed kernel's lane-sum group, bit 4 SINGLE
-// (uint8 packed: one buffer of shifted copies, chosen by the host when two do not fit), bit 5 REGSPLIT (merged
+// (uint8 packed: one buffer of shifted copies, chosen by the host when two do not fit), bit 6 DIAG (uint8 packed,
+// subband step 1: time tiles aligned to the input, per-trial output shift), bit 5 REGSPLIT (merged
 // kernel with 512 consumer threads + 8 producer warps: setmaxnreg moves registers from the producers to the consumers).
 template <typename IN_T, int SPT, int DPT, int UNROLL, int STAGING, int VEC, int FLAGS>
 __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
@@ -2083,7 +2140,7 @@ __device__ __forceinline__ void ddp_dedisp_entry(const DdpDedispParams& p) {
     if constexpr (sizeof(IN_T) == 1 && STAGING >= 3)
         ddp_dedisp_merge_body<SPT, DPT, UNROLL, (STAGING == 3 ? 2 : 4), WIDE, OUT16, (FLAGS & 32) != 0>(p);
     else if constexpr (sizeof(IN_T) == 1 && STAGING != 0)
-        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16, SINGLE>(p);
+        ddp_dedisp_packed_body<SPT, DPT, UNROLL, STAGING, VEC, WIDE, OUT16, SINGLE, (FLAGS & 64) != 0>(p);
     else if constexpr (sizeof(IN_T) == 2 && STAGING != 0)
         ddp_dedisp_packed16_body<SPT, DPT, UNROLL, STAGING, VEC, 1 << ((FLAGS >> 2) & 3)>(p);
     else

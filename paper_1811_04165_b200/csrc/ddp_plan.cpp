@@ -317,6 +317,46 @@ int ddp_spread_max(const ddp_plan* p, ddp_kernel k, int TD) {
     p->spread_cache[which][TD] = mx;
     return mx;
 }
+// Step 1 with "diagonal" time tiles (ddp_kernels.cuh, DIAG): per DM tile and subband the delays relative to the
+// subband's first channel, rel[a][c] = d1[a][c] - d1[a][first], spread over the tile by far less than the delays
+// themselves (a coarse trial moves the whole subband).  Usable when no relative delay is negative (the first channel
+// of every subband is its earliest: the staged window never starts in front of the row) and worth it when it shrinks
+// the window by more than half.
+bool ddp_sub1_diag(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, int* rel_spread, int* shift_max) {
+    if (k != DDP_K_SUB1 || c.staging == 0 || ddp_merge_group(c) || p->in_bytes != 1) return false;
+    const int TD = c.threads_dm * c.dms_per_thread;
+    auto it = p->diag_cache.find(TD);
+    if (it == p->diag_cache.end()) {
+        int spread = 0, shift = 0;
+        bool ok = true;
+        const int nc = p->nchan, cps = p->cps;
+        for (int lo = 0; lo < p->ncoarse && ok; lo += TD) {
+            const int hi = std::min(lo + TD, p->ncoarse);
+            for (int s = 0; s < p->nsub && ok; ++s) {
+                const int c0 = s * cps;
+                const int D0 = p->d1[(size_t)lo * nc + c0];
+                shift = std::max(shift, p->d1[(size_t)(hi - 1) * nc + c0] - D0);
+                for (int r = 0; r < cps; ++r) {
+                    int mn = INT32_MAX, mx = INT32_MIN;
+                    for (int a = lo; a < hi; ++a) {
+                        const int Da = p->d1[(size_t)a * nc + c0];  // the kernel shifts trial a by Da rounded down to D0 + a multiple of 4
+                        const int rel = p->d1[(size_t)a * nc + c0 + r] - (Da - ((Da - D0) & 3));
+                        mn = std::min(mn, rel);
+                        mx = std::max(mx, rel);
+                    }
+                    if (mn < 0) { ok = false; break; }
+                    spread = std::max(spread, mx - mn);
+                }
+            }
+        }
+        it = p->diag_cache.emplace(TD, ok ? std::make_pair(spread, shift) : std::make_pair(-1, -1)).first;
+    }
+    if (it->second.first < 0) return false;
+    if (2 * it->second.first + 64 >= ddp_spread_max(p, k, TD)) return false;
+    if (rel_spread) *rel_spread = it->second.first;
+    if (shift_max) *shift_max = it->second.second;
+    return true;
+}
 // Merged staging.  One scan of the delay table per (kernel, TD, G): for every DM tile of TD trials and every
 // group of G adjacent reduction rows, the distinct tuples tau[m] = (d[j][r0+m] - d[j][r0]) - (same for the tile's
 // first trial) over the tile's trials ("variants"), which variant every trial uses, and its window offset
@@ -470,11 +510,25 @@ int ddp_dedisp_win(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const int AL = 16 / g.in_bytes;
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
     const int64_t TD = (int64_t)c.threads_dm * c.dms_per_thread;
-    if (g.in_bytes == 1)  // packed kernel: 16-byte carry + shifted-copy tail, in bytes, multiple of 16
+    if (g.in_bytes == 1) {  // packed kernel: 16-byte carry + shifted-copy tail, in bytes, multiple of 16
+        int rel = 0;
+        if (ddp_sub1_diag(p, k, c, &rel)) return (int)round_up(TT + rel + 32, 16);
         return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 32, 16);
+    }
     if (g.in_bytes == 2 && c.staging != 0)  // packed uint16 kernel: 8-element carry + 4 spare words, multiple of 8
         return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 16, 8);
     return (int)round_up(TT + ddp_spread_max(p, k, (int)TD) + 2 * AL, AL);
+}
+// ddp_dedisp_packed_body with nb buffers of shifted copies: copies [nb][U][4 or 3][win], offs [2][TD][U],
+// dls [2][TD][64], TMA: raw [2][U][win + 16] + mbarriers, DIAG: dmm [2][2][64] + dsh [TD]
+static size_t packed_u8_layout(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, size_t nb) {
+    const size_t row = (size_t)ddp_dedisp_win(p, k, c);
+    const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
+    const size_t ncp = nb == 1 && c.staging == 2 ? 3 : 4;  // single-buffered with TMA: the unshifted copy is the raw slot (RAW0)
+    size_t b = nb * ncp * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
+    if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
+    if (ddp_sub1_diag(p, k, c)) b += (4 * 64 + TD) * 4;
+    return b;
 }
 size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const int64_t TT = (int64_t)c.threads_t * c.samples_per_thread;
@@ -498,17 +552,10 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
                 b += (4 + 2 * 16 + 2) * 8 + 128;                      // mbarriers, scheduler state
                 return b;
             }
-            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body: copies [nb][U][4][win], offs [2][TD][U], dls [2][TD][64], raw, mbar
-                const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
-                auto layout = [&](size_t nb) {
-                    const size_t ncp = nb == 1 && c.staging == 2 ? 3 : 4;  // single-buffered with TMA: the unshifted copy is the raw slot (RAW0)
-                    size_t b = nb * ncp * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
-                    if (c.staging == 2) b += 2 * (size_t)c.unroll * (row + 16) + 16;
-                    return b;
-                };
+            if (g.in_bytes == 1) {  // ddp_dedisp_packed_body
                 // two buffers of shifted copies when they fit, else one (ddp_u8_single_buffered)
-                const size_t two = layout(2);
-                return two <= DDP_SMEM_LIMIT ? two : layout(1);
+                const size_t two = packed_u8_layout(p, k, c, 2);
+                return two <= DDP_SMEM_LIMIT ? two : packed_u8_layout(p, k, c, 1);
             }
             if (g.in_bytes == 2) {  // ddp_dedisp_packed16_body: copies [NB][U][2][win/2] words, offs [TD][nred4], mbar [NB]
                 const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
@@ -542,11 +589,7 @@ size_t ddp_smem_bytes(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
 // summed); a configuration whose two buffers exceed 227 KB runs with one, if that fits.
 bool ddp_u8_single_buffered(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     if (c.staging == 0 || ddp_merge_group(c) || ddp_kgeom(p, k).in_bytes != 1) return false;
-    const size_t row = (size_t)ddp_dedisp_win(p, k, c);
-    const size_t TD = (size_t)c.threads_dm * c.dms_per_thread;
-    size_t two = 8 * row * c.unroll + ((2 * TD * c.unroll + 3) & ~(size_t)3) * 4 + 2 * TD * 64 * 4;
-    if (c.staging == 2) two += 2 * (size_t)c.unroll * (row + 16) + 16;
-    return two > DDP_SMEM_LIMIT;
+    return packed_u8_layout(p, k, c, 2) > DDP_SMEM_LIMIT;
 }
 
 // Validity rules (from Table 3 P:136-152 + sm_100a limits).

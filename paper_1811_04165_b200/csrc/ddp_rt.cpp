@@ -250,7 +250,8 @@ const char* kind_type(CodeKind ck) { return ck == CK_DEDISP_U8 ? "ddp_u8" : (ck 
 //   bits 2-3      packed uint16 kernel (step 2): log2 of how many subband words are summed in 16-bit
 //                 lanes before they are split, the largest of {1, 2, 4} that cannot overflow;
 //   bit 4  SINGLE packed uint8 kernel with one buffer of shifted copies (two do not fit in 227 KB);
-//   bit 5  REGSPLIT merged kernel with 512 consumer threads: setmaxnreg hands the producers' spare registers to them.
+//   bit 5  REGSPLIT merged kernel with 512 consumer threads: setmaxnreg hands the producers' spare registers to them;
+//   bit 6  DIAG   packed uint8 kernel, subband step 1: time tiles aligned to the input, per-trial output shift.
 int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     const CodeKind ck = code_kind(p, k);
     int f = 0;
@@ -258,6 +259,7 @@ int code_flags(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c) {
     if (k == DDP_K_SUB1 && p->info.sub_elem_bytes == 2) f |= 2;
     if (ck == CK_DEDISP_U8 && ddp_u8_single_buffered(p, k, c)) f |= 16;
     if (ck == CK_DEDISP_U8 && ddp_merge_group(c) && c.threads_t * c.threads_dm >= 512) f |= 32;  // REGSPLIT
+    if (ck == CK_DEDISP_U8 && ddp_sub1_diag(p, k, c)) f |= 64;  // DIAG: input-aligned time tiles, per-trial output shift
     if (ck == CK_DEDISP_U16 && c.staging != 0 && k == DDP_K_SUB2) {  // uint16 INPUT samples can be 65535: no lane sums there
         const int64_t room = 65535 / (255 * (int64_t)p->cps);
         f |= (room >= 4 ? 2 : (room >= 2 ? 1 : 0)) << 2;
@@ -826,7 +828,9 @@ ddp_status launch_dedisp(const ddp_plan* p, ddp_kernel k, const ddp_kcfg& c, Ddp
         const int64_t grid = std::min<int64_t>(nunits, (int64_t)per_sm * nsm);
         return launch(p, K, (unsigned)grid, 1, 1, (unsigned)threads, 1u, smem, io.stream, &q);
     }
-    return launch(p, K, cdiv(q.ns, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,
+    int shift_max = 0;  // DIAG: the tile grid also covers the samples the last trial of a tile owns beyond the first one's
+    ddp_sub1_diag(p, k, c, nullptr, &shift_max);
+    return launch(p, K, cdiv((int64_t)q.ns + shift_max, TT), cdiv(q.ndm, TD), groups, (unsigned)c.threads_t, (unsigned)c.threads_dm,
                   ddp_smem_bytes(p, k, c), io.stream, &q);
 }
 

@@ -488,6 +488,41 @@ def test_channel_mask_subband_plan():
     g.close()
 
 
+def test_subband_step1_diagonal_tiles_and_the_ascending_band_fallback():
+    """Staged step 1 lays its time tiles out in input-aligned time with a per-trial output shift when the delays
+    relative to a subband's first channel spread far less than the delays themselves.  Covered
+    here: a plan with a coarse DM step large enough to switch it on at every DM-tile size (windows of several
+    tiles' length without it), ragged first / last tiles, a ragged DM tile; and the same band in ASCENDING channel
+    order, where the first channel of a subband is its latest and the plain layout must be used -- S and Y
+    against the oracle for sampled staged shapes of both."""
+    import dataclasses
+    base = small_subband(name="diag_sb", nchan=192, nsamp_out=3100, ndm=21 * 4,
+                         subband=SubbandPlan(n_subbands=8, n_coarse=21, coarse_first=0.0, coarse_step=24.0,
+                                             n_fine=4, fine_step=0.5))
+    # 96 channels per subband: two delay superchunks of 64 rows, the second one's window bounds are made while the
+    # first is summed
+    long_sb = small_subband(name="diag_sb96", nchan=384, nsamp_out=2200, ndm=17 * 2,
+                            subband=SubbandPlan(n_subbands=4, n_coarse=17, coarse_first=0.0, coarse_step=24.0,
+                                                n_fine=2, fine_step=0.5))
+    for cfg in (base, dataclasses.replace(base, name="diag_sb_ascending", f_hi_mhz=base.f_lo_mhz, f_lo_mhz=base.f_hi_mhz),
+                long_sb):
+        g = GpuSearch(cfg)
+        So, Yo = oracle_subband(cfg, g.X)
+        V = [c for c in g.plan.enumerate_kcfgs(ddp.K_SUB1) if c.staging in (1, 2)]
+        picks = _sample(V, 40, seed=31)
+        # blocks of fewer threads than a delay superchunk has rows (64): the per-row min / max of the relative
+        # delays must still cover every row (a 32-thread block once left half of them unset)
+        picks += _sample([c for c in V if c.threads_t * c.threads_dm <= 64], 12, seed=32)
+        assert {c.staging for c in picks} == {1, 2}
+        for c in picks:
+            g.plan.set_kcfg(ddp.K_SUB1, c)
+            g.buf["d_out"].fill_(-1)
+            Y = g.dedisperse()
+            assert np.array_equal(g.subband_intermediate(), So), "%s: S differs for %r" % (cfg.name, c)
+            assert np.array_equal(Y, Yo), "%s: Y differs for %r" % (cfg.name, c)
+        g.close()
+
+
 # ---------------------------------------------------------------------------------- DM rows split over ranks (8(f) f3)
 @pytest.mark.parametrize("subband", [False, True])
 def test_dm_sharded_search_equals_the_one_gpu_search(subband):

@@ -187,6 +187,30 @@ def test_sixteen_bit_plan_host_side(tmp_path):
         ddp.plan_from_config(cfg, cache_dir=None, input_bits=12)
 
 
+def test_step1_diagonal_tiles_are_chosen_from_the_delay_tables(tmp_path):
+    """Code flag bit 6 (DIAG) of the packed step-1 kernel: on at BJ:cfg2 (the window of 32 coarse trials shrinks from
+    TT + 5616 to TT + ~236 samples, so 8 channels per chunk fit twice where 4 fitted once), off for the same band in
+    ascending channel order (relative delays negative) and for direct loads; visible in the kernel's name."""
+    import dataclasses
+    cfg = configs.apertif_subband()
+    p = ddp.plan_from_config(cfg, cache_dir=str(tmp_path))
+    c = ddp.Kcfg(128, 4, 16, 8, 8, 2, 16)
+    assert p.check_kcfg(ddp.K_SUB1, c)       # two buffers of 8 rows: invalid before (V6, test_validity_rules_named_cases)
+    p.compile_kcfg(ddp.K_SUB1, c)
+    p.compile_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 8, 0, 16))
+    names = sorted(os.listdir(tmp_path))
+    assert any(n.startswith("ddp_dedisp_u8_s16_d8_u8_g2_v16_t512_w66.") for n in names), names   # OUT16 | DIAG
+    assert any(n.startswith("ddp_dedisp_u8_s16_d2_u8_g0_v16_t256_w2.") for n in names), names    # direct loads: OUT16 only
+    p.destroy()
+    asc = dataclasses.replace(cfg, f_hi_mhz=cfg.f_lo_mhz, f_lo_mhz=cfg.f_hi_mhz)
+    q = ddp.plan_from_config(asc, cache_dir=str(tmp_path / "asc"))
+    assert not q.check_kcfg(ddp.K_SUB1, c)   # without the diagonal layout the windows are 7.7 KB again
+    c4 = ddp.Kcfg(128, 4, 16, 8, 4, 2, 16)
+    q.compile_kcfg(ddp.K_SUB1, c4)
+    assert any(n.startswith("ddp_dedisp_u8_s16_d8_u4_g2_v16_t512_w18.") for n in os.listdir(tmp_path / "asc"))  # OUT16 | SINGLE
+    q.destroy()
+
+
 def test_plan_create_rejects_bad_arguments():
     f = np.array([1500.0, 1400.0, 1300.0, 1200.0])
     ok = dict(chan_freq_mhz=f, t_samp_s=1e-3, dm_list=[0.0, 10.0], widths=[1, 2], nsamp_out=64, cache_dir=None)
@@ -336,12 +360,15 @@ def test_validity_rules_named_cases():
         assert not plan.check_kcfg(ddp.K_SUB1, c), why
     # V4: 48 channels per subband -> unroll 16 divides, and sub2 (32 subbands) accepts 16 too
     assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 16, 0, 16))
-    # V6: the same shape staged needs 16 rows x 4 shifted copies of a ~2.5 KB window; two buffers of
-    # them exceed 227 KB, one fits, so the shape is valid and runs single-buffered ...
+    # V6: the same shape staged is valid: 16 rows x shifted copies of a ~1.3 KB window (diagonal time tiles,
+    # DESIGN.md 6.1c; ~2.5 KB and single-buffered without them)
     assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(64, 4, 16, 2, 16, 1, 16))
-    # ... while 8 rows of the 7.7 KB windows of a 2048 x 32 tile do not fit even once
+    # a 2048 x 32 tile: 2.3 KB windows with the diagonal layout, so 4 and 8 rows per chunk fit (without it the
+    # windows are 7.7 KB and 8 rows do not fit even once: test_step1_diagonal_tiles_are_chosen_from_the_delay_tables);
+    # 16 rows of a 4096-sample tile's 4.4 KB windows do not fit
     assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(128, 4, 16, 8, 4, 2, 16))
-    assert not plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(128, 4, 16, 8, 8, 2, 16))
+    assert plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(128, 4, 16, 8, 8, 2, 16))
+    assert not plan.check_kcfg(ddp.K_SUB1, ddp.Kcfg(256, 2, 16, 16, 16, 2, 16))
     # uint32-input kernels need vec_bytes >= 4
     assert not plan.check_kcfg(ddp.K_SUB2, ddp.Kcfg(128, 2, 4, 4, 4, 0, 1))
     # the direct kernel is not part of a subband plan
