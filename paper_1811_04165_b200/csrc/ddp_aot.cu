@@ -23,6 +23,7 @@ DDP_AOT_U32(4, 4, 4, 0, 16, 256)
 DDP_AOT_INTEG(4, 1, 1, 0, 16, 256)
 DDP_AOT_SNR(4, 1, 4, 0, 16, 256)
 DDP_AOT_ISNR(16, 1, 256)
+DDP_AOT_ISNR(16, 1, 512)   // cfg1 / cfg2 tuned [32,16,16,1,1,direct,16]: 128 blocks of 16 rows
 // one instance of every staging mode per kernel (SASS evidence: LDS / UBLKCP paths)
 DDP_AOT_U8(8, 4, 8, 0, 4, 256, 0)
 DDP_AOT_U8(16, 4, 8, 1, 16, 256, 0)
