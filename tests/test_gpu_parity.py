@@ -521,6 +521,23 @@ def test_subband_step1_diagonal_tiles_and_the_ascending_band_fallback():
             assert np.array_equal(g.subband_intermediate(), So), "%s: S differs for %r" % (cfg.name, c)
             assert np.array_equal(Y, Yo), "%s: Y differs for %r" % (cfg.name, c)
         g.close()
+    # the diagonal layout with zapped channels (masked rows read the workspace's row of zeros, which is only
+    # in_stride_min long: the shifted tiles must not read past it)
+    mask = np.ones(base.nchan, np.uint8)
+    mask[[0, 1, 23, 24, 100, 191]] = 0
+    g = GpuSearch(base, chan_mask=mask)
+    Xz = g.X.copy()
+    Xz[mask == 0] = 0
+    g.X[mask == 0] = 255
+    g.upload()
+    So, Yo = oracle_subband(base, Xz)
+    for c in _sample([c for c in g.plan.enumerate_kcfgs(ddp.K_SUB1) if c.staging in (1, 2)], 16, seed=33):
+        g.plan.set_kcfg(ddp.K_SUB1, c)
+        g.buf["d_out"].fill_(-1)
+        Y = g.dedisperse()
+        assert np.array_equal(g.subband_intermediate(), So), "masked, diagonal: S differs for %r" % c
+        assert np.array_equal(Y, Yo), "masked, diagonal: Y differs for %r" % c
+    g.close()
 
 
 # ---------------------------------------------------------------------------------- DM rows split over ranks (8(f) f3)
