@@ -492,8 +492,15 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
     unsigned char* raw = (unsigned char*)(dls + (size_t)2 * TD * SC);  // TMA: [2][U][win + 16]
     ddp_u64* mbar = (ddp_u64*)(raw + (size_t)2 * U * (win + 16));      // TMA: [2]
     int* dmm = STAGING == 2 ? (int*)(mbar + 2) : (int*)raw;            // DIAG: [2][2][SC] smallest / largest relative delay of a row
-    int* dsh = dmm + 4 * SC;                                           // DIAG: [TD] D_j - D_0, the output shift of trial j
+    int* dsh = dmm + 4 * SC;                                           // DIAG: [TD] D_j - D_0 rounded down to a multiple of 4, the output shift of trial j
     const int nchunks = p.nred / U;
+    int diag_d0 = 0;
+    if constexpr (DIAG) {
+        diag_d0 = __ldg(dl);
+        for (int j = tid; j < TD; j += nthreads)
+            dsh[j] = (__ldg(dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride) - diag_d0) & ~3;
+        __syncthreads();
+    }
 
     auto load_dls = [&](int s) {
         int* d = dls + (size_t)(s & 1) * TD * SC;
@@ -501,14 +508,7 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         for (int idx = tid; idx < TD * SC; idx += nthreads) {
             const int j = idx / SC, cc = idx - j * SC;
             const int* drow = dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride;
-            if (r0 + cc < p.nred) {
-                int v = drow[r0 + cc];
-                if constexpr (DIAG) {
-                    const int Dj = __ldg(drow), D0 = __ldg(dl);
-                    v -= Dj - ((Dj - D0) & 3);
-                }
-                d[idx] = v;
-            }
+            if (r0 + cc < p.nred) d[idx] = DIAG ? drow[r0 + cc] - (dsh[j] + diag_d0) : drow[r0 + cc];
         }
     };
     // DIAG: rounded relative delays are not monotone in the trial index, so the window of a row is bounded by
@@ -660,10 +660,6 @@ __device__ __forceinline__ void ddp_dedisp_packed_body(const DdpDedispParams& p)
         }
     }
     load_dls(0);
-    if constexpr (DIAG) {
-        for (int j = tid; j < TD; j += nthreads)
-            dsh[j] = (__ldg(dl + (ddp_i64)(j < nd ? j : nd - 1) * p.delay_dm_stride) - __ldg(dl)) & ~3;
-    }
     __syncthreads();
     if constexpr (DIAG) {
         minmax_dls(0);
